@@ -1,0 +1,456 @@
+"""Pins for the CPU oracle (oracle/gf_oracle.cpp) against what the paper and the mathematics fix.
+
+The paper (arXiv:1412.1498) prints no worked numerical example, so every pin here is a closed form, an invariant, a
+library routine, or brute force ("What pins each part").  None of these tests touches the CUDA path.
+"""
+import numpy as np
+import pytest
+
+import gf_inputs as gi
+import oracle
+from _util import (dag, embed_su2, flat, from_c, gauge_transform, grid, lex_coords, parity, plaquettes,
+                   random_su3, random_unit_quaternions, shift, su2_matrix, to_c)
+
+SUBGROUPS = [(0, 1), (1, 2), (0, 2)]
+D = {"landau": 4, "coulomb": 3}
+
+
+def rough(dims, r=0.4, seed=11):
+    return gi.make_links(dims, r, seed)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# measure: F (eq. 1.1) and theta (eqs. 1.2, 1.3)
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_unit_links_F1_theta0(gauge):
+    dims = (4, 6, 4, 2)
+    V = int(np.prod(dims))
+    U = from_c(np.broadcast_to(np.eye(3, dtype=complex), (V, 4, 3, 3)).copy())
+    F, th = oracle.measure(U, dims, gauge)
+    assert F == 1.0 and th == 0.0
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_pure_gauge_transformed_back_F1_theta0(gauge):
+    # U = G(x) G(x+mu)^dag is pure gauge; transforming with g = G^dag gives unit links: F = 1 (pins the d in the
+    # normalisation, reading A1) and theta = 0.
+    dims = (4, 4, 6, 4)
+    G = gi.make_gauge(dims, seed=7)
+    V = G.shape[0]
+    Uc = gauge_transform(np.broadcast_to(np.eye(3, dtype=complex), (V, 4, 3, 3)).copy(), G, dims)
+    F0, th0 = oracle.measure(from_c(Uc), dims, gauge)
+    assert F0 < 0.2 and th0 > 1.0  # a Haar-random gauge: F ~ 0, theta = O(10)
+    back = gauge_transform(Uc, dag(G), dims)
+    F, th = oracle.measure(from_c(back), dims, gauge)
+    assert abs(F - 1.0) < 1e-12 and th < 1e-24
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_abelian_closed_form(gauge):
+    # U_mu(x) = exp(i alpha_mu(x) T), T = diag(1,-1,0).  Then Re Tr U = 2 cos(alpha) + 1 and, from eq. 1.3,
+    # Delta(x) = 2i S(x) T with S(x) = sum_{nu<d} [sin alpha_nu(x-nu) - sin alpha_nu(x)], so Tr Delta Delta^dag = 8 S^2.
+    dims = (4, 6, 2, 4)
+    d = D[gauge]
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(5)
+    alpha = rng.uniform(-np.pi, np.pi, size=(V, 4))
+    Uc = np.zeros((V, 4, 3, 3), dtype=complex)
+    Uc[:, :, 0, 0] = np.exp(1j * alpha)
+    Uc[:, :, 1, 1] = np.exp(-1j * alpha)
+    Uc[:, :, 2, 2] = 1.0
+    F, th = oracle.measure(from_c(Uc), dims, gauge)
+    F_ref = np.sum(2 * np.cos(alpha[:, :d]) + 1) / (d * 3 * V)
+    S = np.zeros(V)
+    for nu in range(d):
+        S += shift(np.sin(alpha[:, nu]), dims, nu, -1) - np.sin(alpha[:, nu])
+    th_ref = np.sum(8 * S ** 2) / (3 * V)
+    assert abs(F - F_ref) < 1e-14
+    assert abs(th - th_ref) < 1e-12 * th_ref
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_theta_from_K_traceless_form_and_trace_identity(gauge):
+    # Delta = -[(K - K^dag) - (1/3) Tr(K - K^dag)] with K of eq. 1.5 (reading A2), and
+    # sum_x Re Tr K(x) = 2 sum_{x, mu<d} Re Tr U_mu(x).
+    dims = (4, 4, 4, 4)
+    d = D[gauge]
+    U = rough(dims)
+    V = U.shape[0]
+    F, th = oracle.measure(U, dims, gauge)
+    tot_K, th_K = 0.0, 0.0
+    for s in range(V):
+        K = oracle.site_K(U, dims, gauge, s)
+        Dl = oracle.site_delta(U, dims, gauge, s)
+        X = K - K.conj().T
+        X = -(X - np.trace(X) / 3 * np.eye(3))
+        assert np.abs(X - Dl).max() < 1e-14
+        tot_K += np.trace(K).real
+        th_K += np.sum(np.abs(X) ** 2)
+    assert abs(tot_K / (2 * d * 3 * V) - F) < 1e-14
+    assert abs(th_K / (3 * V) - th) < 1e-13 * th
+
+
+def test_site_K_matches_numpy_roll():
+    # K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dag]: index/wrap check against an np.roll restatement on an asymmetric lattice
+    dims = (4, 6, 2, 8)
+    U = rough(dims)
+    Uc = to_c(U)
+    for gauge in ("landau", "coulomb"):
+        K = np.zeros((U.shape[0], 3, 3), dtype=complex)
+        for mu in range(D[gauge]):
+            K += Uc[:, mu] + dag(shift(Uc[:, mu], dims, mu, -1))
+        for s in [0, 1, 3, 4, 23, 24, 47, 48, 200, U.shape[0] - 1]:
+            assert np.abs(oracle.site_K(U, dims, gauge, s) - K[s]).max() < 1e-14
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_measure_invariant_under_global_rotation(gauge):
+    dims = (4, 4, 4, 4)
+    U = rough(dims)
+    g = random_su3(np.random.default_rng(3), 1)[0]
+    Ug = from_c(g @ to_c(U) @ g.conj().T)
+    F0, t0 = oracle.measure(U, dims, gauge)
+    F1, t1 = oracle.measure(Ug, dims, gauge)
+    assert abs(F0 - F1) < 1e-14 and abs(t0 - t1) < 1e-12 * t0
+
+
+def test_theta_order_of_magnitude_on_random_gauge():
+    dims = (4, 4, 4, 4)
+    F, th = oracle.measure(gi.make_links(dims, 0.3, 1), dims, "landau")
+    assert abs(F) < 0.1 and 5 < th < 30
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SU(2) subgroup maximiser (eqs. 1.4-1.6) and the overrelaxation power
+# ---------------------------------------------------------------------------------------------------------------------
+def test_su2_maximiser_brute_force_2to4():
+    # omega = 1: g_opt maximises Re Tr[g K] over the embedded SU(2); 1e5 random g' never beat it, and the best of a
+    # cloud concentrated around g_opt approaches it from below.
+    dims = (2, 2, 2, 2)
+    U = gi.make_links(dims, 0.6, 3)
+    rng = np.random.default_rng(0)
+    cloud = random_unit_quaternions(rng, 100000)
+    for s in range(16):
+        K = oracle.site_K(U, dims, "landau", s)
+        for (i, j) in SUBGROUPS:
+            K1, G1, a = oracle.su2_step(K, np.eye(3), i, j, 1.0)
+            f_opt = np.trace(K1).real
+            assert abs(f_opt - np.trace(embed_su2(su2_matrix(a), i, j) @ K).real) < 1e-13
+            blk = K[np.ix_([i, j], [i, j])]
+            third = K[3 - i - j, 3 - i - j].real
+            f_rand = np.einsum("nab,ba->n", su2_matrix(cloud), blk).real + third
+            assert f_rand.max() <= f_opt + 1e-13
+            near = a[None, :] + 1e-3 * rng.normal(size=(20000, 4))
+            near /= np.linalg.norm(near, axis=1, keepdims=True)
+            f_near = np.einsum("nab,ba->n", su2_matrix(near), blk).real + third
+            assert f_near.max() <= f_opt + 1e-13
+            assert f_opt - f_near.max() < 1e-4 * abs(f_opt)
+            # stationarity: a second step on the updated K returns g = 1
+            _, _, a2 = oracle.su2_step(K1, G1, i, j, 1.0)
+            assert abs(a2[0] - 1) < 1e-15 and np.abs(a2[1:]).max() < 1e-15
+            K = K1
+
+
+def test_su2_closed_form_eq_1_6():
+    # If the 2x2 block of K is k.V with V in SU(2), eq. 1.6 gives g = block^dag (det block^dag)^(-1/2) = V^dag.
+    rng = np.random.default_rng(1)
+    for (i, j) in SUBGROUPS:
+        for _ in range(20):
+            V2 = su2_matrix(random_unit_quaternions(rng, 1)[0])
+            k = rng.uniform(0.5, 7.0)
+            K = rng.normal(size=(3, 3)) + 1j * rng.normal(size=(3, 3))
+            K[np.ix_([i, j], [i, j])] = k * V2
+            blk_dag = (k * V2).conj().T
+            g_ref = blk_dag / np.sqrt(np.linalg.det(blk_dag))
+            if g_ref[0, 0].real * V2.conj().T[0, 0].real < 0:  # branch of the square root
+                g_ref = -g_ref
+            _, G1, a = oracle.su2_step(K, np.eye(3), i, j, 1.0)
+            assert np.abs(su2_matrix(a) - g_ref).max() < 1e-14
+            assert np.abs(G1 - embed_su2(g_ref, i, j)).max() < 1e-14
+
+
+def test_su2_power_group_properties():
+    rng = np.random.default_rng(2)
+    for a in random_unit_quaternions(rng, 200):
+        g = su2_matrix(a)
+        assert np.abs(oracle.su2_power(a, 1.0) - a).max() < 1e-15
+        assert np.abs(su2_matrix(oracle.su2_power(a, 2.0)) - g @ g).max() < 4e-15
+        w1, w2 = rng.uniform(0.2, 0.9, size=2)
+        lhs = su2_matrix(oracle.su2_power(a, w1)) @ su2_matrix(oracle.su2_power(a, w2))
+        assert np.abs(lhs - su2_matrix(oracle.su2_power(a, w1 + w2))).max() < 4e-15
+        p = oracle.su2_power(a, 1.7)
+        assert abs(np.dot(p, p) - 1) < 4e-15
+
+
+def test_su2_power_against_eigendecomposition():
+    # library pin: g = W diag(e^{i phi}, e^{-i phi}) W^dag  =>  g^omega = W diag(e^{i omega phi}, e^{-i omega phi}) W^dag
+    rng = np.random.default_rng(4)
+    for a in random_unit_quaternions(rng, 100):
+        for omega in (1.0, 1.5, 1.7, 1.99):
+            lam, W = np.linalg.eig(su2_matrix(a))
+            phi = np.angle(lam)  # principal branch in (-pi, pi], the pair is +-phi with |phi| in [0, pi]
+            ref = W @ np.diag(np.exp(1j * omega * phi)) @ np.linalg.inv(W)
+            assert np.abs(su2_matrix(oracle.su2_power(a, omega)) - ref).max() < 1e-13
+
+
+def test_su2_power_small_angle_limits():
+    # reading A7: s -> 0 with a0 > 0 tends to (1, omega a_k); a0 = -1 (phi = pi, axis undefined) is left at g = 1
+    for s in (1e-3, 1e-8, 1e-200, 0.0):
+        a = np.array([np.sqrt(1 - s * s), s, 0.0, 0.0])
+        p = oracle.su2_power(a, 1.7)
+        assert np.isfinite(p).all()
+        assert abs(p[1] - np.sin(1.7 * np.arctan2(s, a[0]))) <= 1e-15 * max(s, 1e-300) + 1e-300
+        assert abs(p[0] - np.cos(1.7 * np.arctan2(s, a[0]))) < 1e-15
+    p = oracle.su2_power(np.array([-1.0, 0.0, 0.0, 0.0]), 1.7)
+    assert np.array_equal(p, [1.0, 0.0, 0.0, 0.0])
+    K = np.zeros((3, 3), dtype=complex)  # |r| = 0: the subgroup is skipped (g = 1)
+    K1, G1, a = oracle.su2_step(K, np.eye(3), 0, 1, 1.7)
+    assert np.array_equal(a, [1.0, 0.0, 0.0, 0.0]) and np.array_equal(G1, np.eye(3))
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# half-sweep / sweep
+# ---------------------------------------------------------------------------------------------------------------------
+def _G_of_site(U, dims, gauge, s, omega):
+    K = oracle.site_K(U, dims, gauge, s)
+    G = np.eye(3, dtype=complex)
+    for (i, j) in SUBGROUPS:
+        K, G, _ = oracle.su2_step(K, G, i, j, omega)
+    return G
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("par", [0, 1])
+def test_half_sweep_is_the_gauge_transformation_by_G(gauge, par):
+    # A half-sweep must equal U_mu(x) -> g(x) U_mu(x) g(x+mu)^dag with g = G(x) on the updated parity and 1 elsewhere
+    # (eq. 1.1): pins the x-mu indexing, G vs G^dag, "all four directions" (reading A9) and write-exactly-once.
+    dims = (4, 2, 6, 4)
+    U = rough(dims, 0.5, 9)
+    V = U.shape[0]
+    p = parity(dims)
+    g = np.broadcast_to(np.eye(3, dtype=complex), (V, 3, 3)).copy()
+    for s in np.nonzero(p == par)[0]:
+        g[s] = _G_of_site(U, dims, gauge, s, 1.7)
+    ref = gauge_transform(to_c(U), g, dims)
+    W = U.copy()
+    oracle.half_sweep(W, dims, gauge, par, 1.7)
+    assert np.abs(to_c(W) - ref).max() < 5e-15
+    assert np.abs(to_c(W) - to_c(U)).reshape(V, 4, -1).max(axis=2).min() > 1e-6  # every link was touched
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_sweep_gauge_invariance_and_unitarity(gauge):
+    dims = (4, 4, 4, 6)
+    U = rough(dims, 0.5, 13)
+    W = U.copy()
+    oracle.sweeps(W, dims, gauge, 1.7, n=3)
+    assert np.abs(W - U).max() > 1e-3
+    for (mu, nu, a, b) in [(0, 1, 1, 1), (0, 2, 1, 1), (0, 3, 1, 1), (1, 2, 1, 1), (1, 3, 1, 1), (2, 3, 1, 1),
+                           (0, 1, 1, 2), (2, 3, 2, 1), (1, 3, 2, 2), (0, 2, 2, 2)]:
+        t0 = oracle.wilson_traces(U, dims, mu, nu, a, b)
+        t1 = oracle.wilson_traces(W, dims, mu, nu, a, b)
+        assert np.abs(t0 - t1).max() < 1e-12
+    for mu in range(4):
+        assert np.abs(oracle.polyakov_traces(U, dims, mu) - oracle.polyakov_traces(W, dims, mu)).max() < 1e-12
+    uu, dt = oracle.unitarity(W, dims)
+    assert uu < 1e-12 and dt < 1e-12
+
+
+def test_oracle_observables_match_numpy():
+    # the observables used as pins are themselves pinned against an np.roll restatement
+    dims = (4, 2, 6, 4)
+    U = rough(dims)
+    pl = plaquettes(to_c(U), dims)
+    for (mu, nu), tr in pl.items():
+        assert np.abs(oracle.wilson_traces(U, dims, mu, nu, 1, 1) - tr).max() < 1e-13
+    Uc = to_c(U)
+    for mu in range(4):
+        P = np.broadcast_to(np.eye(3, dtype=complex), (U.shape[0], 3, 3)).copy()
+        for k in range(dims[mu]):
+            P = P @ shift(Uc[:, mu], dims, mu, k)
+        assert np.abs(oracle.polyakov_traces(U, dims, mu) - np.trace(P, axis1=-2, axis2=-1)).max() < 1e-13
+    Ubad = U.copy()
+    Ubad[5, 2] *= 1.001
+    uu, dt = oracle.unitarity(Ubad, dims)
+    assert 1e-3 < uu < 3e-3 and 2e-3 < dt < 4e-3
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_relaxation_is_monotone(gauge):
+    # omega = 1: every single site update maximises its local functional, so F never decreases (eqs. 1.4-1.6)
+    dims = (4, 4, 2, 4)
+    U = rough(dims, 0.6, 21)
+    V = U.shape[0]
+    p = parity(dims)
+    F_prev = oracle.measure(U, dims, gauge)[0]
+    for par in (0, 1):
+        for s in np.nonzero(p == par)[0]:
+            oracle.site_update(U, dims, gauge, s, 1.0)
+            F = oracle.measure(U, dims, gauge)[0]
+            assert F >= F_prev - 1e-15
+            F_prev = F
+    for _ in range(10):
+        oracle.sweeps(U, dims, gauge, 1.0, n=1)
+        F = oracle.measure(U, dims, gauge)[0]
+        assert F >= F_prev - 1e-15
+        F_prev = F
+
+
+def test_half_sweep_independent_of_site_order():
+    dims = (4, 4, 4, 4)
+    U = rough(dims)
+    p = parity(dims)
+    for par in (0, 1):
+        A = U.copy()
+        oracle.half_sweep(A, dims, "landau", par, 1.7)
+        B = U.copy()
+        order = np.nonzero(p == par)[0]
+        np.random.default_rng(8).shuffle(order)
+        for s in order:
+            oracle.site_update(B, dims, "landau", s, 1.7)
+        assert np.array_equal(A, B)
+        U = A
+
+
+def test_translation_by_two_sites_commutes_with_sweep():
+    dims = (4, 6, 4, 8)
+    U = rough(dims)
+    A = U.copy()
+    oracle.sweeps(A, dims, "landau", 1.7, n=1)
+    for mu in range(4):
+        B = np.ascontiguousarray(shift(U, dims, mu, 2))
+        oracle.sweeps(B, dims, "landau", 1.7, n=1)
+        assert np.array_equal(B, shift(A, dims, mu, 2))
+
+
+def test_F_from_odd_K_after_sweep():
+    dims = (4, 4, 4, 4)
+    U = rough(dims)
+    oracle.sweeps(U, dims, "landau", 1.7, n=1)
+    p = parity(dims)
+    tot = sum(np.trace(oracle.site_K(U, dims, "landau", s)).real for s in np.nonzero(p == 1)[0])
+    assert abs(tot / (4 * 3 * U.shape[0]) - oracle.measure(U, dims, "landau")[0]) < 1e-14
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# fix (Algorithm 1)
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_fix_converges_on_pure_gauge(gauge):
+    dims = (4, 4, 4, 4)
+    U = gi.make_links(dims, 0.0, 17)  # roughness 0: U = G(x) G(x+mu)^dag exactly
+    done, hist = oracle.fix(U, dims, gauge, 1.7, 1e-20, 2000, 5)
+    assert done < 2000 and hist[-1, 2] < 1e-20 and abs(hist[-1, 1] - 1.0) < 1e-10
+    assert hist[0, 0] == 0 and hist[-1, 0] == done and np.all(np.diff(hist[:, 0]) == 5)
+
+
+def test_fix_semantics_and_convergence_properties():
+    dims = (4, 4, 4, 4)
+    U = rough(dims, 0.3, 23)
+    W = U.copy()
+    done, hist = oracle.fix(W, dims, "landau", 1.7, 1e-13, 3000, 10)
+    assert done % 10 == 0 and hist[-1, 2] < 1e-13 and hist[-2, 2] >= 1e-13
+    # gauge invariance across the whole run
+    assert np.abs(oracle.wilson_traces(U, dims, 0, 3, 1, 1) - oracle.wilson_traces(W, dims, 0, 3, 1, 1)).max() < 1e-11
+    # at the maximum K(x) is Hermitian up to i.c.1: every subgroup's r1 = r2 = r3 = 0
+    for s in (0, 7, 100, 255):
+        K = oracle.site_K(W, dims, "landau", s)
+        for (i, j) in SUBGROUPS:
+            _, _, a = oracle.su2_step(K, np.eye(3), i, j, 1.0)
+            assert np.abs(a[1:]).max() < 1e-6
+    # theta decays geometrically at late times
+    th = hist[-6:, 2]
+    ratios = th[1:] / th[:-1]
+    assert np.all(ratios < 1.0) and ratios.max() / ratios.min() < 30
+    # already converged: zero sweeps; eps = 0: fixed sweep count, capped
+    done2, hist2 = oracle.fix(W, dims, "landau", 1.7, 1e-13, 3000, 10)
+    assert done2 == 0 and len(hist2) == 1
+    done3, hist3 = oracle.fix(U.copy(), dims, "landau", 1.7, 0.0, 25, 10)
+    assert done3 == 25 and list(hist3[:, 0]) == [0, 10, 20, 25]
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Coulomb gauge (reading A9)
+# ---------------------------------------------------------------------------------------------------------------------
+def test_coulomb_time_slices_decouple():
+    dims = (4, 4, 4, 6)
+    U = rough(dims, 0.5, 31)
+    V = U.shape[0]
+    t_of = lex_coords(dims)[:, 3]
+    A = U.copy()
+    oracle.sweeps(A, dims, "coulomb", 1.7, n=3)
+    # perturb the spatial links of slice t' = 2 only
+    P = U.copy()
+    rng = np.random.default_rng(0)
+    sel = np.nonzero(t_of == 2)[0]
+    Pc = to_c(P)
+    Pc[sel[:, None], np.arange(3)[None, :]] = random_su3(rng, len(sel) * 3).reshape(len(sel), 3, 3, 3)
+    P = from_c(Pc)
+    B = P.copy()
+    oracle.sweeps(B, dims, "coulomb", 1.7, n=3)
+    other = t_of != 2
+    assert np.array_equal(A[other][:, :3], B[other][:, :3])  # spatial links of the other slices: bit-identical
+    assert not np.array_equal(A[~other][:, :3], B[~other][:, :3])
+    # temporal plaquettes are invariant (the temporal links ARE transformed)
+    for mu in range(3):
+        assert np.abs(oracle.wilson_traces(U, dims, mu, 3, 1, 1) - oracle.wilson_traces(A, dims, mu, 3, 1, 1)).max() < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# 12-real storage emulation (reading A13) and reunitarisation (reading A12)
+# ---------------------------------------------------------------------------------------------------------------------
+def test_storage12_emulation():
+    dims = (4, 4, 4, 4)
+    U = rough(dims)
+    A, B = U.copy(), U.copy()
+    oracle.project12(B, dims)
+    assert np.abs(A - B).max() < 1e-14  # exact SU(3) input: row 2 already is conj(row0 x row1)
+    oracle.sweeps(A, dims, "landau", 1.7, n=1, storage=18)
+    oracle.sweeps(B, dims, "landau", 1.7, n=1, storage=12)
+    assert np.abs(A - B).max() < 1e-14
+    Bc = to_c(B)
+    assert np.abs(Bc[..., 2, :] - np.conj(np.cross(Bc[..., 0, :], Bc[..., 1, :]))).max() < 3e-16
+    B2 = B.copy()
+    oracle.project12(B2, dims)
+    assert np.array_equal(B2, B)  # row 2 is stored exactly as rebuilt from the stored rows 0 and 1
+
+
+def test_reunitarize():
+    dims = (4, 4, 2, 2)
+    U = rough(dims)
+    A = U.copy()
+    oracle.reunitarize(A, dims)
+    assert np.abs(A - U).max() < 2e-15  # identity on exact SU(3)
+    rng = np.random.default_rng(6)
+    N = (U + 1e-3 * rng.normal(size=U.shape)).astype(np.float64)
+    R = N.copy()
+    oracle.reunitarize(R, dims)
+    uu, dt = oracle.unitarity(R, dims)
+    assert uu < 2e-15 and dt < 2e-15
+    R2 = R.copy()
+    oracle.reunitarize(R2, dims)
+    assert np.abs(R2 - R).max() < 2e-15  # idempotent
+    # library pin: Gram-Schmidt on rows 0,1 == QR of the transposed 2-row block with positive diagonal
+    Nc, Rc = to_c(N).reshape(-1, 3, 3), to_c(R).reshape(-1, 3, 3)
+    for k in range(0, Nc.shape[0], 37):
+        q, r = np.linalg.qr(Nc[k, :2].T)
+        q = q * (np.diag(r) / np.abs(np.diag(r)))[None, :]
+        assert np.abs(q.T - Rc[k, :2]).max() < 1e-14
+        assert np.abs(np.conj(np.cross(Rc[k, 0], Rc[k, 1])) - Rc[k, 2]).max() < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# float32 instantiation
+# ---------------------------------------------------------------------------------------------------------------------
+def test_f32_oracle_tracks_f64():
+    dims = (4, 4, 4, 4)
+    U = rough(dims)
+    U32 = U.astype(np.float32)
+    A = U32.astype(np.float64)
+    oracle.sweeps(A, dims, "landau", 1.75, n=1, storage=12)
+    oracle.sweeps(U32, dims, "landau", 1.75, n=1, storage=12)
+    assert np.abs(U32.astype(np.float64) - A).max() < 2e-5
+    F64, t64 = oracle.measure(A, dims, "landau")
+    F32, t32 = oracle.measure(U32, dims, "landau")
+    assert abs(F64 - F32) < 1e-5 * abs(F64) and abs(t64 - t32) < 1e-3 * t64
