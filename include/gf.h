@@ -1,0 +1,121 @@
+/* gf.h — C ABI of libgf: the data-parallel hot path of lattice Landau/Coulomb gauge fixing by overrelaxation on one
+ * NVIDIA B200 (sm_100a), after N. Cardoso, "Coulomb and Landau Gauge Fixing in GPUs using CUDA and MILC",
+ * arXiv:1412.1498 (cited below as PAPER.md:<line>, the text under /root/reference).
+ *
+ * What the library computes (eqs. 1.1-1.6; Algorithm 1):
+ *   - the checkerboarded SU(3) overrelaxation sweep: for every site x of one parity, K(x) = sum_mu [U_mu(x) +
+ *     U_mu(x-mu)^dagger] (eq. 1.5; mu = 0..3 Landau, mu = 0..2 Coulomb), local maximisation of
+ *     Re Tr[g K] (eq. 1.4) over the three SU(2) subgroups (eq. 1.6), each raised to the overrelaxation
+ *     power omega, then g(x) applied to U_mu(x) and U_mu(x-mu) for all four mu (Alg. 1 l.7-8);
+ *   - the reduction that gives F (eq. 1.1) and theta (eqs. 1.2-1.3);
+ *   - link reunitarisation every k sweeps;
+ *   - the driver loop of Algorithm 1 with a measurement cadence.
+ * Readings taken where the paper is silent or ambiguous are listed in DESIGN.md (A1-A20).
+ *
+ * Conventions
+ *   - Every function returns 0 (GF_OK) or a negative GF_E* code; nothing throws, nothing aborts.
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host pointers.  The caller owns all device
+ *     memory: the library never allocates or frees device memory and keeps no pointer to a links buffer after the
+ *     call that received it returns (copies are ordered on the context's stream).  gf_ctx itself (plus a few bytes of
+ *     pinned host memory for the two result scalars) is host memory owned by the library until gf_destroy.
+ *   - All work is enqueued on the cuda_stream given to gf_create (a cudaStream_t passed as void*; NULL = default
+ *     stream).  Calls documented "async" return without waiting for the device.
+ *   - Canonical (external) link layout, used by every set/get call regardless of the internal storage:
+ *         links[site][mu][row][col][re,im],  site = x + nx*(y + ny*(z + nz*t))   (x fastest),
+ *     mu = 0..3 = (x,y,z,t) with mu = 3 temporal; 18 reals per link, element type double (GF_FP64) or
+ *     float (GF_FP32).  U_mu(x) is the link from x to x+mu.  Total 72*V elements, V = nx*ny*nz*nt.
+ *   - Site parity is (x+y+z+t)&1 in both gauges; a sweep updates parity 0 ("even") first, then parity 1
+ *     (PAPER.md:134).
+ */
+#ifndef GF_H
+#define GF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gf_ctx gf_ctx; /* opaque */
+
+enum { GF_LANDAU = 0, GF_COULOMB = 1 };
+enum { GF_FP64 = 0, GF_FP32 = 1 };      /* PAPER.md:140 (SP/DP) */
+/* storage: 18 (full 3x3) or 12 (rows 0,1 stored; row 2 = conj(row0 x row1) rebuilt at every load) reals per link,
+ * PAPER.md:128, 144 */
+
+enum {
+  GF_OK = 0,
+  GF_EINVAL = -1,       /* null pointer, n < 0, check_every < 1, omega outside [1,2), bad option */
+  GF_EODD = -2,         /* an extent is odd or < 2 (all lattice dimensions must be even) */
+  GF_EUNSUPPORTED = -3, /* storage not in {12,18}, unknown gauge / precision, V >= 2^31 */
+  GF_ENOMEM = -4,       /* workspace too small or misaligned (256-byte alignment required) */
+  GF_ECUDA = -5,        /* a CUDA call failed; text via gf_last_error */
+  GF_ENUMERIC = -6      /* F or theta came back NaN/Inf */
+};
+
+/* Bytes of device workspace gf_create needs for this lattice: the internal-layout link field, the partial-sum
+ * scratch of the F/theta reduction, the result scalars and two staging buffers for the *_host calls.
+ * Returns 0 if the arguments are invalid. */
+size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage);
+
+/* Create a context.  dev_workspace: caller-owned device memory of at least gf_workspace_bytes(...) bytes, 256-byte
+ * aligned, which must stay valid until gf_destroy.  cuda_stream: the stream all work of this context runs on.
+ * The link field is undefined until gf_set_links[_host].  Errors: GF_EINVAL, GF_EODD, GF_EUNSUPPORTED, GF_ENOMEM,
+ * GF_ECUDA. */
+int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec, int storage, void* dev_workspace,
+              size_t workspace_bytes, void* cuda_stream);
+
+/* Canonical layout (device) -> internal layout.  With storage = 12 only rows 0 and 1 are kept.  Resets the sweep
+ * counter used by the reunitarisation cadence.  Async. */
+int gf_set_links(gf_ctx* ctx, const void* dev_links);
+/* Internal layout -> canonical layout (device), 18 reals per link always (row 2 rebuilt if storage = 12).  Async. */
+int gf_get_links(gf_ctx* ctx, void* dev_links_out);
+/* Same, from / to HOST memory (pinned memory makes the copies asynchronous and faster, pageable works): the field is
+ * streamed through the workspace's staging buffers in chunks, copy and reorder overlapped.  gf_get_links_host
+ * synchronises the stream before returning; gf_set_links_host returns once the host buffer has been consumed. */
+int gf_set_links_host(gf_ctx* ctx, const void* host_links);
+int gf_get_links_host(gf_ctx* ctx, void* host_links_out);
+
+/* n overrelaxation sweeps (Algorithm 1 l.3-12): each sweep is the parity-0 half-sweep then the
+ * parity-1 half-sweep with overrelaxation parameter omega in [1,2); after global sweep number s the links are
+ * reunitarised if reunit_every > 0 and s % reunit_every == 0.  n = 0 is a no-op.  Async. */
+int gf_ovr_sweep(gf_ctx* ctx, int n, double omega);
+
+/* F (eq. 1.1, normalised by the d directions summed) and theta (eqs. 1.2-1.3) of the links as they stand, written to
+ * host out-params.  FP64 accumulation in both precisions, deterministic summation order.  Synchronises the stream.
+ * GF_ENUMERIC if either value is not finite (the values are still written). */
+int gf_measure(gf_ctx* ctx, double* F, double* theta);
+
+/* Algorithm 1 with a measurement cadence: measure; while theta >= eps and sweeps < max_sweeps: do
+ * min(check_every, remaining) sweeps, measure.  *sweeps_done = sweeps performed (0 if already converged).  eps = 0
+ * gives a fixed-sweep run.  The (sweep, F, theta) triple of every measurement is kept and can be read with
+ * gf_get_history.  Synchronises the stream at every measurement. */
+int gf_fix(gf_ctx* ctx, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done);
+/* Copies up to cap triples {sweep, F, theta} (3 doubles each) of the last gf_fix into hist (host); *n = number of
+ * measurements the run made (may exceed cap). */
+int gf_get_history(gf_ctx* ctx, double* hist, int cap, int* n);
+
+/* Project every link back onto SU(3): Gram-Schmidt on rows 0,1, row 2 = conj(row0 x row1).  Async. */
+int gf_reunitarize(gf_ctx* ctx);
+/* k = 0 (default): never; k > 0: reunitarise after every k-th sweep inside gf_ovr_sweep / gf_fix. */
+int gf_set_reunit_every(gf_ctx* ctx, int k);
+
+/* Tuning knobs for benchmarking kernel variants; the defaults are the fastest measured.  GF_EINVAL on unknown keys. */
+enum {
+  GF_OPT_SWEEP_VARIANT = 1, /* which half-sweep kernel: 0 = default for this (prec, storage) */
+  GF_OPT_BLOCK_THREADS = 2  /* threads per block of the half-sweep kernel (multiple of 32; 0 = default) */
+};
+int gf_set_option(gf_ctx* ctx, int key, int value);
+
+/* Number of kernels this context has launched since gf_create (for benchmark bookkeeping). */
+long long gf_kernel_launches(const gf_ctx* ctx);
+
+void gf_destroy(gf_ctx* ctx);
+const char* gf_strerror(int code);
+/* Text of the last failure on this context (CUDA error string for GF_ECUDA); valid until the next call. */
+const char* gf_last_error(const gf_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF_H */

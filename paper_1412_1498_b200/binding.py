@@ -1,0 +1,254 @@
+"""Thin ctypes binding of libgf (include/gf.h).  Argument marshalling only: every step of the hot path runs in the
+CUDA kernels behind the C ABI.  PyTorch is used for device memory and streams, nothing else.
+
+The module-level functions carry the C names (gf_create, gf_set_links, gf_ovr_sweep, gf_measure, gf_fix,
+gf_get_links, ...) and take raw pointers / ints; `GaugeFixer` is a small convenience owner of a context plus the torch
+workspace tensor it lives in.  There is no CPU fallback: if libgf.so cannot be built or loaded, importing fails.
+"""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_longlong, c_size_t, c_void_p
+
+from . import build as _build
+
+GF_LANDAU, GF_COULOMB = 0, 1
+GF_FP64, GF_FP32 = 0, 1
+GF_OK, GF_EINVAL, GF_EODD, GF_EUNSUPPORTED, GF_ENOMEM, GF_ECUDA, GF_ENUMERIC = 0, -1, -2, -3, -4, -5, -6
+GF_OPT_SWEEP_VARIANT, GF_OPT_BLOCK_THREADS = 1, 2
+
+SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "gf_set_links_host",
+           "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
+           "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error"]
+
+
+def _load() -> ctypes.CDLL:
+    lib = ctypes.CDLL(_build.build())
+    lib.gf_workspace_bytes.restype = c_size_t
+    lib.gf_workspace_bytes.argtypes = [c_int] * 6
+    lib.gf_create.restype = c_int
+    lib.gf_create.argtypes = [POINTER(c_void_p)] + [c_int] * 7 + [c_void_p, c_size_t, c_void_p]
+    for name in ("gf_set_links", "gf_get_links", "gf_set_links_host", "gf_get_links_host"):
+        getattr(lib, name).restype = c_int
+        getattr(lib, name).argtypes = [c_void_p, c_void_p]
+    lib.gf_ovr_sweep.restype = c_int
+    lib.gf_ovr_sweep.argtypes = [c_void_p, c_int, c_double]
+    lib.gf_measure.restype = c_int
+    lib.gf_measure.argtypes = [c_void_p, POINTER(c_double), POINTER(c_double)]
+    lib.gf_fix.restype = c_int
+    lib.gf_fix.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int)]
+    lib.gf_get_history.restype = c_int
+    lib.gf_get_history.argtypes = [c_void_p, POINTER(c_double), c_int, POINTER(c_int)]
+    lib.gf_reunitarize.restype = c_int
+    lib.gf_reunitarize.argtypes = [c_void_p]
+    lib.gf_set_reunit_every.restype = c_int
+    lib.gf_set_reunit_every.argtypes = [c_void_p, c_int]
+    lib.gf_set_option.restype = c_int
+    lib.gf_set_option.argtypes = [c_void_p, c_int, c_int]
+    lib.gf_kernel_launches.restype = c_longlong
+    lib.gf_kernel_launches.argtypes = [c_void_p]
+    lib.gf_destroy.restype = None
+    lib.gf_destroy.argtypes = [c_void_p]
+    lib.gf_strerror.restype = c_char_p
+    lib.gf_strerror.argtypes = [c_int]
+    lib.gf_last_error.restype = c_char_p
+    lib.gf_last_error.argtypes = [c_void_p]
+    return lib
+
+
+lib = _load()
+
+
+class GFError(RuntimeError):
+    def __init__(self, code: int, detail: str = ""):
+        self.code = code
+        msg = lib.gf_strerror(code).decode()
+        super().__init__(f"libgf error {code} ({msg})" + (f": {detail}" if detail else ""))
+
+
+# ---- the C ABI, same names, raw arguments (return codes are returned, not raised) -------------------------------------
+def gf_workspace_bytes(nx, ny, nz, nt, prec, storage) -> int:
+    return int(lib.gf_workspace_bytes(nx, ny, nz, nt, prec, storage))
+
+
+def gf_create(nx, ny, nz, nt, gauge, prec, storage, dev_workspace: int, workspace_bytes: int, cuda_stream: int):
+    """Returns (rc, ctx_handle)."""
+    h = c_void_p()
+    rc = lib.gf_create(byref(h), nx, ny, nz, nt, gauge, prec, storage, c_void_p(dev_workspace), workspace_bytes,
+                       c_void_p(cuda_stream))
+    return rc, h
+
+
+def gf_set_links(ctx, dev_links: int) -> int:
+    return lib.gf_set_links(ctx, c_void_p(dev_links))
+
+
+def gf_get_links(ctx, dev_links_out: int) -> int:
+    return lib.gf_get_links(ctx, c_void_p(dev_links_out))
+
+
+def gf_set_links_host(ctx, host_links: int) -> int:
+    return lib.gf_set_links_host(ctx, c_void_p(host_links))
+
+
+def gf_get_links_host(ctx, host_links_out: int) -> int:
+    return lib.gf_get_links_host(ctx, c_void_p(host_links_out))
+
+
+def gf_ovr_sweep(ctx, n: int, omega: float) -> int:
+    return lib.gf_ovr_sweep(ctx, n, omega)
+
+
+def gf_measure(ctx):
+    """Returns (rc, F, theta)."""
+    F, th = c_double(), c_double()
+    rc = lib.gf_measure(ctx, byref(F), byref(th))
+    return rc, F.value, th.value
+
+
+def gf_fix(ctx, omega: float, eps: float, max_sweeps: int, check_every: int):
+    """Returns (rc, sweeps_done)."""
+    done = c_int()
+    rc = lib.gf_fix(ctx, omega, eps, max_sweeps, check_every, byref(done))
+    return rc, done.value
+
+
+def gf_get_history(ctx, cap: int = 100000):
+    """Returns (rc, [(sweep, F, theta), ...])."""
+    buf = (c_double * (3 * cap))()
+    n = c_int()
+    rc = lib.gf_get_history(ctx, buf, cap, byref(n))
+    m = min(n.value, cap)
+    return rc, [(int(buf[3 * i]), buf[3 * i + 1], buf[3 * i + 2]) for i in range(m)]
+
+
+def gf_reunitarize(ctx) -> int:
+    return lib.gf_reunitarize(ctx)
+
+
+def gf_set_reunit_every(ctx, k: int) -> int:
+    return lib.gf_set_reunit_every(ctx, k)
+
+
+def gf_set_option(ctx, key: int, value: int) -> int:
+    return lib.gf_set_option(ctx, key, value)
+
+
+def gf_kernel_launches(ctx) -> int:
+    return int(lib.gf_kernel_launches(ctx))
+
+
+def gf_destroy(ctx) -> None:
+    lib.gf_destroy(ctx)
+
+
+def gf_strerror(code: int) -> str:
+    return lib.gf_strerror(code).decode()
+
+
+def gf_last_error(ctx) -> str:
+    return lib.gf_last_error(ctx).decode()
+
+
+# ---- convenience owner ---------------------------------------------------------------------------------------------------
+_GAUGE = {"landau": GF_LANDAU, "coulomb": GF_COULOMB}
+_PREC = {"f64": GF_FP64, "f32": GF_FP32}
+
+
+class GaugeFixer:
+    """Owns a gf_ctx and the torch workspace tensor behind it.  All methods marshal arguments and check return codes."""
+
+    def __init__(self, dims, gauge="landau", prec="f64", storage=18, device="cuda:0", stream=None):
+        import torch
+
+        self.torch = torch
+        self.dims = tuple(int(d) for d in dims)
+        self.gauge, self.prec, self.storage = gauge, prec, int(storage)
+        self.device = torch.device(device)
+        self.dtype = torch.float64 if prec == "f64" else torch.float32
+        self.volume = 1
+        for d in self.dims:
+            self.volume *= d
+        nbytes = gf_workspace_bytes(*self.dims, _PREC[prec], self.storage)
+        if nbytes == 0:
+            # let gf_create produce the precise error code
+            nbytes = 256
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            rc, self.ctx = gf_create(*self.dims, _GAUGE[gauge], _PREC[prec], self.storage, self.workspace.data_ptr(),
+                                     nbytes, self.stream.cuda_stream)
+        if rc != GF_OK:
+            self.ctx = None
+            raise GFError(rc)
+
+    def _check(self, rc):
+        if rc != GF_OK:
+            raise GFError(rc, gf_last_error(self.ctx))
+
+    def new_links_buffer(self):
+        """An uninitialised device tensor in the canonical layout (V,4,3,3,2)."""
+        return self.torch.empty((self.volume, 4, 3, 3, 2), dtype=self.dtype, device=self.device)
+
+    def set_links(self, links):
+        assert links.is_cuda and links.is_contiguous() and links.dtype == self.dtype and links.numel() == self.volume * 72
+        self._check(gf_set_links(self.ctx, links.data_ptr()))
+
+    def get_links(self, out=None):
+        if out is None:
+            out = self.new_links_buffer()
+        assert out.is_cuda and out.is_contiguous() and out.dtype == self.dtype and out.numel() == self.volume * 72
+        self._check(gf_get_links(self.ctx, out.data_ptr()))
+        return out
+
+    def set_links_host(self, links):
+        """links: CPU torch tensor or numpy array (pinned memory recommended), canonical layout."""
+        ptr = links.data_ptr() if hasattr(links, "data_ptr") else links.ctypes.data
+        self._check(gf_set_links_host(self.ctx, ptr))
+
+    def get_links_host(self, out):
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        self._check(gf_get_links_host(self.ctx, ptr))
+        return out
+
+    def ovr_sweep(self, n, omega):
+        self._check(gf_ovr_sweep(self.ctx, int(n), float(omega)))
+
+    def measure(self):
+        rc, F, th = gf_measure(self.ctx)
+        self._check(rc)
+        return F, th
+
+    def fix(self, omega, eps, max_sweeps, check_every):
+        rc, done = gf_fix(self.ctx, float(omega), float(eps), int(max_sweeps), int(check_every))
+        self._check(rc)
+        return done
+
+    def history(self):
+        rc, h = gf_get_history(self.ctx)
+        self._check(rc)
+        return h
+
+    def reunitarize(self):
+        self._check(gf_reunitarize(self.ctx))
+
+    def set_reunit_every(self, k):
+        self._check(gf_set_reunit_every(self.ctx, int(k)))
+
+    def set_option(self, key, value):
+        self._check(gf_set_option(self.ctx, int(key), int(value)))
+
+    def kernel_launches(self):
+        return gf_kernel_launches(self.ctx)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            gf_destroy(self.ctx)
+            self.ctx = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,327 @@
+// gf_api.cu — the C ABI of include/gf.h: context, argument checking, the Algorithm 1 driver loop.
+// Every step of the hot path runs in the kernels of gf_kernels.cu; this file only sequences launches.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/gf.h"
+#include "gf_internal.h"
+
+using namespace gf;
+
+namespace {
+constexpr size_t ALIGN = 256;
+constexpr size_t STAGING_BYTES = 64u << 20;  // each of the two staging buffers used by the *_host calls
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Sizes {
+  size_t links, partials, result, staging, total;
+};
+
+bool valid_lattice(int nx, int ny, int nz, int nt, int* err) {
+  const int n[4] = {nx, ny, nz, nt};
+  long long V = 1;
+  for (int d = 0; d < 4; ++d) {
+    if (n[d] < 2 || (n[d] & 1)) { *err = GF_EODD; return false; }
+    V *= n[d];
+    if (V >= (1LL << 31)) { *err = GF_EUNSUPPORTED; return false; }
+  }
+  return true;
+}
+
+Geo make_geo(int nx, int ny, int nz, int nt) {
+  Geo g;
+  g.n[0] = nx; g.n[1] = ny; g.n[2] = nz; g.n[3] = nt;
+  g.nh0 = nx / 2;
+  g.vh = (int)((long long)nx * ny * nz * nt / 2);
+  g.nblk = (g.vh + 31) / 32;
+  g.s1 = g.nh0; g.s2 = g.nh0 * ny; g.s3 = g.nh0 * ny * nz;
+  return g;
+}
+
+Sizes sizes_of(const Geo& g, int prec, int storage) {
+  Sizes s;
+  const size_t csize = prec == GF_FP64 ? 16 : 8;
+  s.links = align_up((size_t)2 * g.nblk * 4 * (storage / 2) * 32 * csize);
+  s.partials = align_up((size_t)measure_num_partials(g) * sizeof(double2));
+  s.result = align_up(2 * sizeof(double));
+  s.staging = align_up(STAGING_BYTES);
+  s.total = s.links + s.partials + s.result + 2 * s.staging;
+  return s;
+}
+}  // namespace
+
+struct gf_ctx {
+  KernelArgs k;
+  Sizes sz;
+  char* staging[2];
+  cudaEvent_t staging_free[2];
+  double* host_result;  // pinned, 2 doubles
+  int reunit_every;
+  long long sweeps_total;  // sweeps since the last gf_set_links (reunitarisation cadence)
+  long long launches;
+  std::vector<double> history;
+  long long history_n;
+  char err[256];
+};
+
+namespace {
+int fail_cuda(gf_ctx* c, cudaError_t e, const char* where) {
+  snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e));
+  return GF_ECUDA;
+}
+int fail(gf_ctx* c, int code, const char* msg) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+  return code;
+}
+size_t elem_size(const gf_ctx* c) { return c->k.prec == GF_FP64 ? sizeof(double) : sizeof(float); }
+long long volume(const gf_ctx* c) { return 2LL * c->k.geo.vh; }
+}  // namespace
+
+extern "C" {
+
+size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage) {
+  int err;
+  if (!valid_lattice(nx, ny, nz, nt, &err)) return 0;
+  if ((prec != GF_FP64 && prec != GF_FP32) || (storage != 18 && storage != 12)) return 0;
+  return sizes_of(make_geo(nx, ny, nz, nt), prec, storage).total;
+}
+
+int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec, int storage, void* dev_workspace,
+              size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return GF_EINVAL;
+  *out = nullptr;
+  int err;
+  if (!valid_lattice(nx, ny, nz, nt, &err)) return err;
+  if (gauge != GF_LANDAU && gauge != GF_COULOMB) return GF_EUNSUPPORTED;
+  if (prec != GF_FP64 && prec != GF_FP32) return GF_EUNSUPPORTED;
+  if (storage != 18 && storage != 12) return GF_EUNSUPPORTED;
+  if (!dev_workspace) return GF_EINVAL;
+  const Geo g = make_geo(nx, ny, nz, nt);
+  const Sizes sz = sizes_of(g, prec, storage);
+  if (workspace_bytes < sz.total || ((uintptr_t)dev_workspace % ALIGN) != 0) return GF_ENOMEM;
+
+  gf_ctx* c = new (std::nothrow) gf_ctx();
+  if (!c) return GF_ENOMEM;
+  c->k.geo = g;
+  c->k.stream = (cudaStream_t)cuda_stream;
+  c->k.prec = prec; c->k.storage = storage; c->k.gauge = gauge;
+  c->k.variant = 0; c->k.block_threads = 0;
+  c->sz = sz;
+  char* base = (char*)dev_workspace;
+  c->k.links = base;
+  c->k.partials = base + sz.links;
+  c->k.result = base + sz.links + sz.partials;
+  c->staging[0] = base + sz.links + sz.partials + sz.result;
+  c->staging[1] = c->staging[0] + sz.staging;
+  c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
+  c->err[0] = 0;
+  c->host_result = nullptr;
+  c->staging_free[0] = c->staging_free[1] = nullptr;
+  cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocDefault);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[0], cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[1], cudaEventDisableTiming);
+  // padding lanes of the last 32-site block must read as zeros
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->k.links, 0, sz.links, c->k.stream);
+  if (e != cudaSuccess) {
+    gf_destroy(c);
+    return GF_ECUDA;
+  }
+  *out = c;
+  return GF_OK;
+}
+
+void gf_destroy(gf_ctx* c) {
+  if (!c) return;
+  if (c->host_result) cudaFreeHost(c->host_result);
+  for (int i = 0; i < 2; ++i)
+    if (c->staging_free[i]) cudaEventDestroy(c->staging_free[i]);
+  delete c;
+}
+
+int gf_set_links(gf_ctx* c, const void* dev_links) {
+  if (!c) return GF_EINVAL;
+  if (!dev_links) return fail(c, GF_EINVAL, "gf_set_links: null links");
+  cudaError_t e = launch_reorder(c->k, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links");
+  c->launches += 1;
+  c->sweeps_total = 0;
+  return GF_OK;
+}
+
+int gf_get_links(gf_ctx* c, void* dev_links_out) {
+  if (!c) return GF_EINVAL;
+  if (!dev_links_out) return fail(c, GF_EINVAL, "gf_get_links: null output");
+  cudaError_t e = launch_reorder(c->k, false, dev_links_out, 0, volume(c), nullptr);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_get_links");
+  c->launches += 1;
+  return GF_OK;
+}
+
+// Host <-> device through the two staging buffers: chunk i uses buffer i&1; the copy of chunk i+1 overlaps the reorder
+// kernel of chunk i when the host memory is pinned.
+static int links_host(gf_ctx* c, void* host, bool in) {
+  const size_t link_bytes = 18 * elem_size(c);
+  const long long sites_per_chunk = (long long)(STAGING_BYTES / (4 * link_bytes));
+  const long long V = volume(c);
+  cudaError_t e = cudaSuccess;
+  int i = 0;
+  for (long long s0 = 0; s0 < V && e == cudaSuccess; s0 += sites_per_chunk, ++i) {
+    const long long s1 = s0 + sites_per_chunk < V ? s0 + sites_per_chunk : V;
+    const size_t bytes = (size_t)(s1 - s0) * 4 * link_bytes;
+    char* h = (char*)host + (size_t)s0 * 4 * link_bytes;
+    char* st = c->staging[i & 1];
+    if (in) {
+      e = cudaMemcpyAsync(st, h, bytes, cudaMemcpyHostToDevice, c->k.stream);
+      if (e == cudaSuccess) e = launch_reorder(c->k, true, nullptr, s0, s1, st);
+    } else {
+      e = launch_reorder(c->k, false, nullptr, s0, s1, st);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h, st, bytes, cudaMemcpyDeviceToHost, c->k.stream);
+    }
+    c->launches += 1;
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, in ? "gf_set_links_host" : "gf_get_links_host");
+  return GF_OK;
+}
+
+int gf_set_links_host(gf_ctx* c, const void* host_links) {
+  if (!c) return GF_EINVAL;
+  if (!host_links) return fail(c, GF_EINVAL, "gf_set_links_host: null links");
+  c->sweeps_total = 0;
+  return links_host(c, const_cast<void*>(host_links), true);
+}
+
+int gf_get_links_host(gf_ctx* c, void* host_links_out) {
+  if (!c) return GF_EINVAL;
+  if (!host_links_out) return fail(c, GF_EINVAL, "gf_get_links_host: null output");
+  return links_host(c, host_links_out, false);
+}
+
+int gf_reunitarize(gf_ctx* c) {
+  if (!c) return GF_EINVAL;
+  cudaError_t e = launch_reunit(c->k);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_reunitarize");
+  c->launches += 1;
+  return GF_OK;
+}
+
+int gf_set_reunit_every(gf_ctx* c, int k) {
+  if (!c) return GF_EINVAL;
+  if (k < 0) return fail(c, GF_EINVAL, "gf_set_reunit_every: k < 0");
+  c->reunit_every = k;
+  return GF_OK;
+}
+
+int gf_set_option(gf_ctx* c, int key, int value) {
+  if (!c) return GF_EINVAL;
+  switch (key) {
+    case GF_OPT_SWEEP_VARIANT:
+      if (value < 0) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
+      c->k.variant = value;
+      return GF_OK;
+    case GF_OPT_BLOCK_THREADS:
+      if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
+      c->k.block_threads = value;
+      return GF_OK;
+    default:
+      return fail(c, GF_EINVAL, "gf_set_option: unknown key");
+  }
+}
+
+int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
+  if (!c) return GF_EINVAL;
+  if (n < 0) return fail(c, GF_EINVAL, "gf_ovr_sweep: n < 0");
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
+  for (int i = 0; i < n; ++i) {
+    for (int parity = 0; parity < 2; ++parity) {  // even first
+      cudaError_t e = launch_halfsweep(c->k, parity, omega);
+      if (e != cudaSuccess) return fail_cuda(c, e, "gf_ovr_sweep");
+      c->launches += 1;
+    }
+    c->sweeps_total += 1;
+    if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) {
+      int rc = gf_reunitarize(c);
+      if (rc != GF_OK) return rc;
+    }
+  }
+  return GF_OK;
+}
+
+int gf_measure(gf_ctx* c, double* F, double* theta) {
+  if (!c) return GF_EINVAL;
+  if (!F || !theta) return fail(c, GF_EINVAL, "gf_measure: null out-param");
+  cudaError_t e = launch_measure(c->k);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(c->host_result, c->k.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->k.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_measure");
+  c->launches += 2;
+  *F = c->host_result[0];
+  *theta = c->host_result[1];
+  if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_measure: non-finite F or theta");
+  return GF_OK;
+}
+
+int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done) {
+  if (!c) return GF_EINVAL;
+  if (!sweeps_done) return fail(c, GF_EINVAL, "gf_fix: null sweeps_done");
+  if (check_every < 1 || max_sweeps < 0 || !(eps >= 0.0))
+    return fail(c, GF_EINVAL, "gf_fix: need check_every >= 1, max_sweeps >= 0, eps >= 0");
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_fix: omega outside [1,2)");
+  c->history.clear();
+  c->history_n = 0;
+  *sweeps_done = 0;
+  int done = 0;
+  double F, th;
+  int rc = gf_measure(c, &F, &th);  // Algorithm 1 l.1
+  auto record = [&]() {
+    c->history.push_back((double)done);
+    c->history.push_back(F);
+    c->history.push_back(th);
+    c->history_n += 1;
+  };
+  if (rc != GF_OK) return rc;
+  record();
+  while (!(th < eps) && done < max_sweeps) {  // Algorithm 1 l.2
+    const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+    rc = gf_ovr_sweep(c, n, omega);
+    if (rc != GF_OK) return rc;
+    done += n;
+    *sweeps_done = done;
+    rc = gf_measure(c, &F, &th);  // Algorithm 1 l.13
+    if (rc != GF_OK) return rc;
+    record();
+  }
+  return GF_OK;
+}
+
+int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
+  if (!c) return GF_EINVAL;
+  if (!n || (cap > 0 && !hist) || cap < 0) return fail(c, GF_EINVAL, "gf_get_history: bad arguments");
+  *n = (int)c->history_n;
+  const long long m = c->history_n < cap ? c->history_n : cap;
+  if (m > 0) memcpy(hist, c->history.data(), (size_t)m * 3 * sizeof(double));
+  return GF_OK;
+}
+
+long long gf_kernel_launches(const gf_ctx* c) { return c ? c->launches : 0; }
+
+const char* gf_strerror(int code) {
+  switch (code) {
+    case GF_OK: return "ok";
+    case GF_EINVAL: return "invalid argument";
+    case GF_EODD: return "lattice extents must be even and >= 2";
+    case GF_EUNSUPPORTED: return "unsupported gauge / precision / storage / volume";
+    case GF_ENOMEM: return "workspace too small or misaligned";
+    case GF_ECUDA: return "CUDA error";
+    case GF_ENUMERIC: return "non-finite F or theta";
+    default: return "unknown error";
+  }
+}
+
+const char* gf_last_error(const gf_ctx* c) { return c ? c->err : ""; }
+
+}  // extern "C"

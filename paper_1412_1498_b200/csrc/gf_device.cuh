@@ -1,0 +1,235 @@
+// gf_device.cuh — device-side building blocks of libgf (sm_100a): complex 3x3 arithmetic in registers, the internal
+// link layout, checkerboard indexing, the SU(2) subgroup / overrelaxation step and row reconstruction.
+// Equation and line numbers refer to arXiv:1412.1498 as PAPER.md:<line>; readings A1-A20 are listed in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gf {
+
+// ---- scalar traits ------------------------------------------------------------------------------------------------------
+template <class T> struct Cplx;
+template <> struct Cplx<double> { using type = double2; };
+template <> struct Cplx<float> { using type = float2; };
+template <class T> using cplx_t = typename Cplx<T>::type;
+
+template <class T> __device__ __forceinline__ cplx_t<T> mk(T a, T b) { cplx_t<T> z; z.x = a; z.y = b; return z; }
+
+// z += a*b
+template <class C> __device__ __forceinline__ void cfma(C& z, const C a, const C b) {
+  z.x = fma(a.x, b.x, z.x); z.x = fma(-a.y, b.y, z.x);
+  z.y = fma(a.x, b.y, z.y); z.y = fma(a.y, b.x, z.y);
+}
+// z += a*conj(b)
+template <class C> __device__ __forceinline__ void cfma_cj(C& z, const C a, const C b) {
+  z.x = fma(a.x, b.x, z.x); z.x = fma(a.y, b.y, z.x);
+  z.y = fma(a.y, b.x, z.y); z.y = fma(-a.x, b.y, z.y);
+}
+// a*b
+template <class C> __device__ __forceinline__ C cmul(const C a, const C b) {
+  C z; z.x = a.x * b.x; z.x = fma(-a.y, b.y, z.x); z.y = a.x * b.y; z.y = fma(a.y, b.x, z.y); return z;
+}
+// conj(a*b - c*d)
+template <class C> __device__ __forceinline__ C cross_cj(const C a, const C b, const C c, const C d) {
+  C z;
+  z.x = a.x * b.x; z.x = fma(-a.y, b.y, z.x); z.x = fma(-c.x, d.x, z.x); z.x = fma(c.y, d.y, z.x);
+  z.y = c.x * d.y; z.y = fma(c.y, d.x, z.y); z.y = fma(-a.x, b.y, z.y); z.y = fma(-a.y, b.x, z.y);
+  return z;
+}
+// row 2 = conj(row0 x row1): third row of an SU(3) matrix from the stored two (12-real storage, A13)
+template <class C> __device__ __forceinline__ void rebuild_row2(C (&u)[9]) {
+  u[6] = cross_cj(u[1], u[5], u[2], u[4]);
+  u[7] = cross_cj(u[2], u[3], u[0], u[5]);
+  u[8] = cross_cj(u[0], u[4], u[1], u[3]);
+}
+
+// ---- geometry and the internal layout ------------------------------------------------------------------------------------
+// Internal layout ("AoSoA-32"): the V/2 sites of one parity are numbered by the checkerboard index
+//   cb = (x + nx*(y + ny*(z + nz*t))) / 2                                   (even/odd kept separate)
+// and grouped in blocks of 32 consecutive cb.  One block of one direction is NELEM*32 complex numbers, element-major:
+//   links[parity][cb/32][mu][elem][cb%32]          elem = 3*row+col, NELEM = 9 (18 reals) or 6 (12 reals: rows 0,1)
+// so a warp that owns 32 consecutive sites reads element e of link mu as one contiguous 32*sizeof(complex) run
+// (512 B in FP64, full 32-byte sectors), and the four forward links of those sites are one contiguous
+// 4*NELEM*32*sizeof(complex) chunk (18 KB for FP64/18).  The last block is padded when V/2 is not a multiple of 32.
+struct Geo {
+  int n[4];     // nx, ny, nz, nt
+  int nh0;      // nx/2: sites of one parity per x-row
+  int vh;       // V/2 sites per parity
+  int nblk;     // ceil(vh/32)
+  int s1, s2, s3;  // checkerboard strides of a step in y, z, t: nh0, nh0*ny, nh0*ny*nz
+};
+
+template <int NELEM>
+__device__ __forceinline__ size_t link_offset(const Geo& g, int parity, int cb, int mu) {
+  return ((((size_t)parity * g.nblk + (size_t)(cb >> 5)) * 4 + mu) * NELEM) * 32 + (cb & 31);
+}
+
+struct Site {
+  int xh, y, z, t, x;
+};
+__device__ __forceinline__ Site site_of(const Geo& g, int parity, int cb) {
+  Site s;
+  unsigned q = (unsigned)cb;
+  s.xh = q % (unsigned)g.nh0; q /= (unsigned)g.nh0;
+  s.y = q % (unsigned)g.n[1]; q /= (unsigned)g.n[1];
+  s.z = q % (unsigned)g.n[2];
+  s.t = q / (unsigned)g.n[2];
+  s.x = 2 * s.xh + ((s.y + s.z + s.t + parity) & 1);
+  return s;
+}
+// checkerboard index (in the OTHER parity) of x - mu, periodic
+__device__ __forceinline__ int cb_down(const Geo& g, const Site& s, int cb, int mu) {
+  switch (mu) {
+    case 0: {
+      int xm = s.x == 0 ? g.n[0] - 1 : s.x - 1;
+      return cb - s.xh + (xm >> 1);
+    }
+    case 1: return s.y == 0 ? cb + g.s1 * (g.n[1] - 1) : cb - g.s1;
+    case 2: return s.z == 0 ? cb + g.s2 * (g.n[2] - 1) : cb - g.s2;
+    default: return s.t == 0 ? cb + g.s3 * (g.n[3] - 1) : cb - g.s3;
+  }
+}
+
+// ---- link load / store in the internal layout ------------------------------------------------------------------------------
+template <int NELEM, bool FULL, class C>
+__device__ __forceinline__ void load_link(const C* __restrict__ p, C (&u)[9]) {
+#pragma unroll
+  for (int e = 0; e < NELEM; ++e) u[e] = p[e * 32];
+  if (NELEM == 6 && FULL) rebuild_row2(u);
+}
+template <int NELEM, class C>
+__device__ __forceinline__ void store_link(C* __restrict__ p, const C (&u)[9]) {
+#pragma unroll
+  for (int e = 0; e < NELEM; ++e) p[e * 32] = u[e];
+}
+
+// ---- SU(2) subgroup step with overrelaxation -------------------------------------------------------------------------------
+template <class T> __device__ __forceinline__ T tiny_of();
+template <> __device__ __forceinline__ double tiny_of<double>() { return 2.2250738585072014e-308 * 1152921504606846976.0; }
+template <> __device__ __forceinline__ float tiny_of<float>() { return 1.17549435e-38f * 1152921504606846976.0f; }
+
+__device__ __forceinline__ void sincos_(double a, double* s, double* c) { sincos(a, s, c); }
+__device__ __forceinline__ void sincos_(float a, float* s, float* c) { sincosf(a, s, c); }
+__device__ __forceinline__ double atan2_(double y, double x) { return atan2(y, x); }
+__device__ __forceinline__ float atan2_(float y, float x) { return atan2f(y, x); }
+__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+__device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+
+// The quaternion (c; q1,q2,q3) of g^omega where g maximises Re Tr[g M] over SU(2) for the 2x2 block M of K
+// (eqs. 1.4-1.6 on the SU(2)-proportional part r of the block, reading A5; exact power, principal branch, A6):
+//   r0 = Re(M00+M11), r1 = -Im(M01+M10), r2 = Re(M10-M01), r3 = -Im(M00-M11);   a = r/|r|;
+//   phi = atan2(|a_vec|, a0);  g^omega = (cos(omega phi); a_vec sin(omega phi)/|a_vec|).
+// |r| cancels in both phi and the direction of a_vec, so it is never formed: phi = atan2(S, r0), S = |r_vec|.
+template <class T>
+__device__ __forceinline__ void su2_overrelax(T r0, T r1, T r2, T r3, T omega, T& c, T& q1, T& q2, T& q3) {
+  const T S2 = r1 * r1 + r2 * r2 + r3 * r3;
+  const T S = sqrt_(S2);
+  if (S <= tiny_of<T>() * fabs(r0)) {  // reading A7 (includes |r| = 0 and phi = pi: g = 1)
+    if (r0 > T(0)) {
+      const T phi = atan2_(S, r0);
+      T sn;
+      sincos_(omega * phi, &sn, &c);
+      const T f = omega / r0;  // limit of sin(omega phi)/s, with a_k = r_k/|r|, |r| -> r0
+      q1 = r1 * f; q2 = r2 * f; q3 = r3 * f;
+    } else {
+      c = T(1); q1 = q2 = q3 = T(0);
+    }
+    return;
+  }
+  const T phi = atan2_(S, r0);
+  T sn;
+  sincos_(omega * phi, &sn, &c);
+  const T f = sn / S;
+  q1 = r1 * f; q2 = r2 * f; q3 = r3 * f;
+}
+
+// One subgroup step on rows/cols (I,J): K <- gK, G <- gG with g = [[c+i q3, q2+i q1], [-q2+i q1, c-i q3]] embedded.
+template <int I, int J, bool UPDATE_K, class T, class C>
+__device__ __forceinline__ void su2_step(C (&K)[9], C (&G)[9], T omega) {
+  const T r0 = K[I * 3 + I].x + K[J * 3 + J].x;
+  const T r1 = -(K[I * 3 + J].y + K[J * 3 + I].y);
+  const T r2 = K[J * 3 + I].x - K[I * 3 + J].x;
+  const T r3 = -(K[I * 3 + I].y - K[J * 3 + J].y);
+  T c, q1, q2, q3;
+  su2_overrelax(r0, r1, r2, r3, omega, c, q1, q2, q3);
+  const C g00 = mk<T>(c, q3), g01 = mk<T>(q2, q1), g10 = mk<T>(-q2, q1), g11 = mk<T>(c, -q3);
+#pragma unroll
+  for (int col = 0; col < 3; ++col) {
+    if (UPDATE_K) {
+      const C ki = K[I * 3 + col], kj = K[J * 3 + col];
+      C a = cmul(g00, ki); cfma(a, g01, kj);
+      C b = cmul(g10, ki); cfma(b, g11, kj);
+      K[I * 3 + col] = a; K[J * 3 + col] = b;
+    }
+    const C gi = G[I * 3 + col], gj = G[J * 3 + col];
+    C a = cmul(g00, gi); cfma(a, g01, gj);
+    C b = cmul(g10, gi); cfma(b, g11, gj);
+    G[I * 3 + col] = a; G[J * 3 + col] = b;
+  }
+}
+
+// G = g3 g2 g1 for one site from its K (Algorithm 1 l.5-6; subgroup order (0,1),(1,2),(0,2), reading A4; A8)
+template <class T, class C>
+__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], C (&G)[9], T omega) {
+#pragma unroll
+  for (int e = 0; e < 9; ++e) G[e] = mk<T>((e % 4 == 0) ? T(1) : T(0), T(0));
+  su2_step<0, 1, true>(K, G, omega);
+  su2_step<1, 2, true>(K, G, omega);
+  su2_step<0, 2, false>(K, G, omega);
+}
+
+// rows 0..NROW-1 of G.U
+template <int NROW, class C>
+__device__ __forceinline__ void mul_left(const C (&G)[9], const C (&u)[9], C (&out)[9]) {
+#pragma unroll
+  for (int i = 0; i < NROW; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      C z = cmul(G[i * 3], u[j]);
+      cfma(z, G[i * 3 + 1], u[3 + j]);
+      cfma(z, G[i * 3 + 2], u[6 + j]);
+      out[i * 3 + j] = z;
+    }
+}
+// rows 0..NROW-1 of U.G^dagger  (needs only rows 0..NROW-1 of U)
+template <int NROW, class C>
+__device__ __forceinline__ void mul_right_adj(const C (&u)[9], const C (&G)[9], C (&out)[9]) {
+#pragma unroll
+  for (int i = 0; i < NROW; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      C z;
+      z.x = u[i * 3].x * G[j * 3].x; z.x = fma(u[i * 3].y, G[j * 3].y, z.x);
+      z.y = u[i * 3].y * G[j * 3].x; z.y = fma(-u[i * 3].x, G[j * 3].y, z.y);
+      cfma_cj(z, u[i * 3 + 1], G[j * 3 + 1]);
+      cfma_cj(z, u[i * 3 + 2], G[j * 3 + 2]);
+      out[i * 3 + j] = z;
+    }
+}
+
+// Gram-Schmidt on rows 0,1; row 2 = conj(row0 x row1)  (reunitarisation, reading A12)
+template <class T, class C>
+__device__ __forceinline__ void reunitarize(C (&u)[9]) {
+  T n0 = u[0].x * u[0].x + u[0].y * u[0].y + u[1].x * u[1].x + u[1].y * u[1].y + u[2].x * u[2].x + u[2].y * u[2].y;
+  T i0 = T(1) / sqrt_(n0);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) { u[j].x *= i0; u[j].y *= i0; }
+  C p = mk<T>(T(0), T(0));
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {  // p = sum conj(row0_j) row1_j
+    p.x = fma(u[j].x, u[3 + j].x, p.x); p.x = fma(u[j].y, u[3 + j].y, p.x);
+    p.y = fma(u[j].x, u[3 + j].y, p.y); p.y = fma(-u[j].y, u[3 + j].x, p.y);
+  }
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    u[3 + j].x -= p.x * u[j].x - p.y * u[j].y;
+    u[3 + j].y -= p.x * u[j].y + p.y * u[j].x;
+  }
+  T n1 = u[3].x * u[3].x + u[3].y * u[3].y + u[4].x * u[4].x + u[4].y * u[4].y + u[5].x * u[5].x + u[5].y * u[5].y;
+  T i1 = T(1) / sqrt_(n1);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) { u[3 + j].x *= i1; u[3 + j].y *= i1; }
+  rebuild_row2(u);
+}
+
+}  // namespace gf

@@ -1,0 +1,71 @@
+"""CPU-side checks of the C-ABI library: it builds, loads, exports every symbol include/gf.h declares, and rejects bad
+arguments with the documented codes before touching the device (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import paper_1412_1498_b200 as gf
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "gf.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(gf_[a-z_0-9]+)\s*\(", header))
+    assert declared == set(gf.SYMBOLS), declared ^ set(gf.SYMBOLS)
+    lib = ctypes.CDLL(os.path.join(ROOT, "paper_1412_1498_b200", "libgf.so"))
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_workspace_bytes():
+    # links 4V*L + partials + result + 2 staging buffers of 64 MiB
+    for dims, prec, storage, L in [((8, 8, 8, 8), gf.GF_FP64, 18, 144), ((8, 8, 8, 8), gf.GF_FP32, 12, 48),
+                                   ((64, 64, 64, 128), gf.GF_FP64, 18, 144), ((48, 48, 48, 96), gf.GF_FP64, 12, 96)]:
+        V = dims[0] * dims[1] * dims[2] * dims[3]
+        n = gf.gf_workspace_bytes(*dims, prec, storage)
+        assert 4 * V * L + (128 << 20) <= n <= 4 * V * L + (128 << 20) + (8 << 20)
+    assert gf.gf_workspace_bytes(7, 8, 8, 8, 0, 18) == 0
+    assert gf.gf_workspace_bytes(8, 8, 8, 8, 0, 8) == 0
+    assert gf.gf_workspace_bytes(8, 8, 8, 8, 2, 18) == 0
+
+
+def test_create_rejects_bad_arguments_before_touching_the_device():
+    big = 1 << 40
+    assert gf.gf_create(7, 8, 8, 8, 0, 0, 18, 256, big, 0)[0] == gf.GF_EODD
+    assert gf.gf_create(8, 8, 0, 8, 0, 0, 18, 256, big, 0)[0] == gf.GF_EODD
+    assert gf.gf_create(8, 8, 8, 8, 2, 0, 18, 256, big, 0)[0] == gf.GF_EUNSUPPORTED
+    assert gf.gf_create(8, 8, 8, 8, 0, 3, 18, 256, big, 0)[0] == gf.GF_EUNSUPPORTED
+    assert gf.gf_create(8, 8, 8, 8, 0, 0, 8, 256, big, 0)[0] == gf.GF_EUNSUPPORTED   # 8-real storage is not built
+    assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 0, big, 0)[0] == gf.GF_EINVAL
+    assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 256, 1024, 0)[0] == gf.GF_ENOMEM
+    assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 264, big, 0)[0] == gf.GF_ENOMEM        # misaligned
+    assert gf.gf_create(2048, 2048, 2048, 2, 0, 0, 18, 256, big, 0)[0] == gf.GF_EUNSUPPORTED  # V >= 2^31
+
+
+def test_null_context_is_einval():
+    assert gf.gf_ovr_sweep(None, 1, 1.5) == gf.GF_EINVAL
+    assert gf.gf_measure(None)[0] == gf.GF_EINVAL
+    assert gf.gf_fix(None, 1.5, 1e-10, 10, 1)[0] == gf.GF_EINVAL
+    assert gf.gf_set_links(None, 256) == gf.GF_EINVAL
+    assert gf.gf_get_links(None, 256) == gf.GF_EINVAL
+    assert gf.gf_reunitarize(None) == gf.GF_EINVAL
+    assert gf.gf_kernel_launches(None) == 0
+    gf.gf_destroy(None)
+    for code in range(0, -7, -1):
+        assert gf.gf_strerror(code) not in ("", "unknown error")
+
+
+def test_product_does_not_import_oracle():
+    # the product path must never route through the oracle (or any CPU fallback)
+    pkg = os.path.join(ROOT, "paper_1412_1498_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.replace("no oracle", ""), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".h")):
+            assert "paper_1412_1498_b200 import" not in open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1412_1498_b200" not in open(os.path.join(ROOT, "oracle", f)).read()
