@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the overrelaxation gauge-fixing hot path (arXiv:1412.1498, Algorithm 1) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl ours|reference]
+
+A STEP is one pass of the whole hot path at the workload's own cadence: `check_every` overrelaxation sweeps (each an
+even and an odd half-sweep: rows a0-a5 of SURVEY.md §8(a); reunitarisation a6 where the config asks for it) followed by
+one F/theta measurement (a7), i.e. one turn of the gf_fix loop (a8).  The default workload is BASELINE.json configs[4]
+(64^3 x 128, FP64, 18-real links, Landau, omega = 1.8, F/theta every 20 sweeps): the largest config, the one the
+roofline target is quoted on, and it fits one GPU (19.3 GB of links).  The field evolves from step to step, as it does
+in the real run (W + K = 8 steps = 160 of the config's 200 sweeps).
+
+  value      site-updates/s, links resident in HBM, CUDA events on the library's stream, max over ranks.
+  e2e        the same metric through the C-ABI host entry points: every step copies the canonical field from pinned
+             host memory (gf_set_links_host), runs the step, and copies the fixed field back (gf_get_links_host).
+  roofline   the half-sweep kernel: algorithmic bytes per launch (16 L per site-update x V/2 sites) / mean launch
+             duration measured here with CUDA events around the back-to-back half-sweep launches of each step.
+  cpu_baseline / --impl reference: the CPU oracle as it stands on the box's host cores, on a bounded sample.
+
+Multi-GPU: the path does not shard in this build ("replicas only"); --gpus N runs N independent replicas,
+one process per GPU, no data-path collective; `value` is the aggregate.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ovr_site_updates_per_s"
+UNIT = "site-updates/s"
+LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48}
+# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the committed ncu --set full capture
+# (profiles/): filled per config once a capture exists, else null.
+NCU_TRAFFIC_BYTES = {}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, read+write copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def get_cfg(name):
+    import gf_inputs as gi
+
+    return dict(next(c for c in gi.CONFIGS if c["name"] == name))
+
+
+def workload_name(cfg):
+    d = cfg["dims"]
+    return (f"BASELINE.json configs[{cfg['name'][3:]}]: {d[0]}x{d[1]}x{d[2]}x{d[3]} SU(3) {cfg['gauge']} "
+            f"{cfg['prec']} {cfg['storage']}-real omega={cfg['omega']} roughness={cfg['roughness']} seed={cfg['seed']}")
+
+
+# ---- clocks ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); smax.append(float(c[2])); power.append(float(c[3]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            # "under load": samples in the upper half of the observed power range
+            lo, hi = min(power), max(power)
+            load = [s for s, p in zip(sm, power) if p >= lo + 0.5 * (hi - lo)] or sm
+            load.sort()
+            out.update(sm_mhz=load[len(load) // 2], sm_max_mhz=max(smax), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=hi)
+        return out
+
+
+# ---- the oracle on host cores (cpu_baseline and --impl reference) --------------------------------------------------------
+def oracle_sample_dims(cfg):
+    """A slab of the workload's lattice: same x,y,z cross-section, 8 time slices (or the whole lattice if smaller)."""
+    d = cfg["dims"]
+    return (d[0], d[1], d[2], min(d[3], 8))
+
+
+class OracleRun:
+    """The oracle as it stands (oracle/, OpenMP over the sites of one parity) on a bounded sample of the workload."""
+
+    def __init__(self, cfg):
+        import numpy as np
+
+        import gf_inputs as gi
+        import oracle
+
+        self.np, self.oracle, self.cfg = np, oracle, cfg
+        self.dims = oracle_sample_dims(cfg)
+        self.V = gi.volume(self.dims)
+        dt = np.float32 if cfg["prec"] == "f32" else np.float64
+        U = gi.make_links(self.dims, cfg["roughness"], cfg["seed"], dtype=dt)
+        self.U = np.ascontiguousarray(U.astype(np.float64))  # reading A18: the FP64 oracle on the rounded input
+        if cfg["storage"] == 12:
+            oracle.project12(self.U, self.dims)
+        self.cores = oracle.num_threads()
+        self.sweeps_done = 0
+        self.sample = (f"oracle (g++ -O2, {self.cores} OpenMP threads), {self.dims[0]}x{self.dims[1]}x{self.dims[2]}x"
+                       f"{self.dims[3]} slab of the workload lattice, same generator / gauge / storage / omega; "
+                       f"one step = {cfg['check_every']} sweeps + 1 F/theta measurement (the GPU arm's cadence)")
+
+    def step(self):
+        c = self.cfg
+        n = c["check_every"]
+        self.oracle.sweeps(self.U, self.dims, c["gauge"], c["omega"], n=n, storage=c["storage"],
+                           reunit_every=c["reunit_every"], first_sweep=self.sweeps_done)
+        self.sweeps_done += n
+        return self.oracle.measure(self.U, self.dims, c["gauge"])
+
+    def time_steps(self, steps, warmup):
+        for _ in range(warmup):
+            self.step()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            self.step()
+        dt = time.perf_counter() - t0
+        return self.V * self.cfg["check_every"] * steps / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores with the arm's metric/config.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    cfg = get_cfg(args.config)
+    run = OracleRun(cfg)
+    value, dt = run.time_steps(args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": run.sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": run.cores, "kind": "oracle", "sample": run.sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---- the CUDA path -----------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+
+    import gf_inputs as gi
+    import paper_1412_1498_b200 as gf
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = get_cfg(args.config)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    V = gi.volume(dims)
+    L = LINK_BYTES[(prec, storage)]
+    n_sw = cfg["check_every"]
+    omega = cfg["omega"]
+
+    fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
+    if args.variant:
+        fx.set_option(gf.GF_OPT_SWEEP_VARIANT, args.variant)
+    if args.block:
+        fx.set_option(gf.GF_OPT_BLOCK_THREADS, args.block)
+    fx.set_reunit_every(cfg["reunit_every"])
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"] + 1000 * rank, prec,
+                         torch.cuda.current_stream().cuda_stream)
+    fx.set_links(canon)
+    torch.cuda.synchronize()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731  (the library runs on torch's current stream)
+
+    def step(timers=None):
+        if timers is None:
+            fx.ovr_sweep(n_sw, omega)
+            return fx.measure()
+        a, b, c = ev(), ev(), ev()
+        a.record()
+        fx.ovr_sweep(n_sw, omega)
+        b.record()
+        r = fx.measure()  # synchronises the stream
+        c.record()
+        timers.append((a, b, c))
+        return r
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between barriers
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    launches0 = fx.kernel_launches()
+    timers = []
+    t0, t1 = ev(), ev()
+    t0.record()
+    for _ in range(args.steps):
+        F, th = step(timers)
+    t1.record()
+    barrier()
+    launches = fx.kernel_launches() - launches0
+    clocks = sampler.stop()
+    ms_total = t0.elapsed_time(t1)
+    ms_sweeps = sum(a.elapsed_time(b) for a, b, _ in timers)
+    ms_measure = sum(b.elapsed_time(c) for _, b, c in timers)
+    n_reunit = 0 if not cfg["reunit_every"] else sum(
+        1 for s in range((args.warmup) * n_sw + 1, (args.warmup + args.steps) * n_sw + 1) if s % cfg["reunit_every"] == 0)
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * V * n_sw * args.steps / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel (half-sweep): 2*n_sw launches per step, back to back on the stream
+    peak, peak_src = load_peaks()
+    n_half = 2 * n_sw * args.steps
+    bytes_per_launch = 16 * L * (V // 2)
+    # the reunitarisation launches inside the sweep region (config 2 only) are subtracted at their algorithmic cost
+    ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
+    achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "ovr_halfsweep_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg["name"]), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_per_launch, "ms_per_launch": ms_half,
+                "launches_timed": n_half, "share_of_step": ms_sweeps / ms_total,
+                "measure_ms": ms_measure / args.steps,
+                "measure_gbs": 4 * V * L / (ms_measure / args.steps * 1e-3) / 1e9,
+                "whole_step_gbs": (16 * V * L * n_sw + 4 * V * L) / (ms_total / args.steps * 1e-3) / 1e9}
+    roofline["whole_step_frac"] = roofline["whole_step_gbs"] / peak
+
+    # ---- end to end through the host entry points (pinned host memory, copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty((V, 4, 3, 3, 2), dtype=fx.dtype).pin_memory()
+        host.copy_(canon)
+        del canon
+        torch.cuda.empty_cache()
+        n_e2e = max(1, min(args.steps, args.e2e_steps))
+
+        def e2e_step():
+            fx.set_links_host(host)
+            fx.ovr_sweep(n_sw, omega)
+            r = fx.measure()
+            fx.get_links_host(host)
+            return r
+
+        e2e_step()  # warm-up
+        barrier()
+        w0 = time.perf_counter()
+        e0, e1 = ev(), ev()
+        e0.record()
+        for _ in range(n_e2e):
+            e2e_step()
+        e1.record()
+        barrier()
+        wall = time.perf_counter() - w0
+        ms_e2e = max(e0.elapsed_time(e1), wall * 1e3)  # host-side copies of pageable chunks would not show in events
+        if dist is not None:
+            t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.item())
+        nbytes = V * 72 * (8 if prec == "f64" else 4)
+        e2e = {"value": world * V * n_sw * n_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes + 16, "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e,
+               "what": "gf_set_links_host (pinned) + %d sweeps + gf_measure + gf_get_links_host (pinned)" % n_sw}
+        del host
+    fx.close()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- the oracle beside it, on this box's host cores (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        run = OracleRun(cfg)
+        v, dt = run.time_steps(1, 0)
+        cpu = {"value": v, "unit": UNIT, "cores": run.cores, "kind": "oracle", "sample": run.sample, "seconds": dt}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": prec, "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "step": f"{n_sw} sweeps + 1 F/theta measurement",
+                   "sites": V, "l2": "inputs exceed L2 (field %.2f GB vs 126 MB)" % (4 * V * L / 1e9)
+                   if 4 * V * L > 4 * 126e6 else "field fits L2: not an HBM measurement", "parallelism": "replicas only",
+                   "final_F": F, "final_theta": th},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg4", help="cfg0..cfg4 of BASELINE.json (default: the largest, cfg4)")
+    ap.add_argument("--variant", type=int, default=0, help="GF_OPT_SWEEP_VARIANT (kernel studies)")
+    ap.add_argument("--block", type=int, default=0, help="GF_OPT_BLOCK_THREADS (kernel studies)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

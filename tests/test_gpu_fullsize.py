@@ -1,0 +1,116 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 2, 3, 4), in the launch configuration bench.py times.
+
+The oracle cannot sweep 33.5 M sites in seconds, so the links after one sweep are checked on SAMPLED outputs the oracle
+can compute one by one: a 6^4 patch of the big lattice (origin with all-even coordinates, so local parity = global
+parity) is handed to the oracle as a small periodic lattice.  After one sweep (even, then odd half-sweep) a link
+U_mu(x) depends only on links stored at sites within [x-2, x+2] per coordinate:
+    U_mu(x) <- G_e/o(x) U_mu(x) G_o/e(x+mu)^dag;  G_o(y) needs the links touching y after the even half-sweep, i.e.
+    G_e(y +- nu), which need the original links stored at y +- nu and y +- nu - nu'.
+For x with local coordinates in {2,3}^4 all of these lie at local coordinates 0..5 and none is reached through the
+patch's own periodic wrap, so the oracle's result there equals the big lattice's (Algorithm 1).
+Patches are placed in the bulk and across the global periodic boundaries.  F and theta are global sums: they are
+compared with the oracle's measure of the full field (a read-only pass the host finishes in seconds).
+
+Inputs come from the device build of the seeded generator (gf_inputs, not part of the CUDA path); the oracle is fed
+copies of that generator output, never anything the product wrote.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import gf_inputs as gi
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+PATCH = 6
+TOL_LINK = {"f64": 1e-12, "f32": 2e-5}
+
+
+def lex(c, dims):
+    return c[0] + dims[0] * (c[1] + dims[1] * (c[2] + dims[2] * c[3]))
+
+
+def patch_sites(origin, dims):
+    """global lexicographic index of every site of the 6^4 patch, in the patch's own lexicographic order"""
+    out = np.empty(PATCH ** 4, dtype=np.int64)
+    i = 0
+    for t, z, y, x in itertools.product(range(PATCH), repeat=4):
+        c = [(origin[0] + x) % dims[0], (origin[1] + y) % dims[1], (origin[2] + z) % dims[2], (origin[3] + t) % dims[3]]
+        out[i] = lex(c, dims)
+        i += 1
+    return out
+
+
+def inner_local():
+    """patch-local lexicographic indices of the sites with local coordinates in {2,3}^4"""
+    return np.array([x + PATCH * (y + PATCH * (z + PATCH * t))
+                     for t, z, y, x in itertools.product((2, 3), repeat=4)], dtype=np.int64)
+
+
+def origins(dims, rng, n_bulk=4):
+    o = [(0, 0, 0, 0), tuple(d - 2 for d in dims), (dims[0] - 4, 0, dims[2] - 2, 2), (2, dims[1] - 2, 0, dims[3] - 4)]
+    for _ in range(n_bulk):
+        o.append(tuple(int(2 * rng.integers(0, d // 2)) for d in dims))
+    return o
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4"])
+def test_fullsize_one_sweep_sampled(name):
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    cfg = next(c for c in gi.CONFIGS if c["name"] == name)
+    dims, prec, storage, gauge, omega = cfg["dims"], cfg["prec"], cfg["storage"], cfg["gauge"], cfg["omega"]
+    V = gi.volume(dims)
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=storage)
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], prec,
+                         torch.cuda.current_stream().cuda_stream)
+    fx.set_links(canon)
+
+    # ---- oracle inputs: generator output for the patches (and the whole field for F, theta), copied BEFORE the sweep
+    rng = np.random.default_rng(2024)
+    patches = []
+    for o in origins(dims, rng):
+        sites = patch_sites(o, dims)
+        idx = torch.from_numpy(sites).cuda()
+        Up = np.ascontiguousarray(canon[idx].cpu().numpy().astype(np.float64))
+        if storage == 12:
+            oracle.project12(Up, (PATCH,) * 4)
+        patches.append((sites, Up))
+    full = np.ascontiguousarray(canon.cpu().numpy().astype(np.float64)) if name != "cfg4" else None
+    if full is not None and storage == 12:
+        oracle.project12(full, dims)
+
+    # ---- F, theta before the sweep
+    F0, th0 = fx.measure()
+    if full is not None:
+        Fo, tho = oracle.measure(full, dims, gauge)
+        assert abs(F0 - Fo) <= (1e-13 if prec == "f64" else 2e-7)
+        assert abs(th0 - tho) <= (1e-12 if prec == "f64" else 2e-6) * tho
+        del full
+    assert abs(F0) < 0.01 and 5.0 < th0 < 20.0  # a Haar-random gauge copy: F ~ 0, theta = O(10)
+
+    # ---- one sweep, sampled links
+    fx.ovr_sweep(1, omega)
+    fx.get_links(out=canon)
+    inner = inner_local()
+    worst = 0.0
+    for sites, Up in patches:
+        oracle.sweeps(Up, (PATCH,) * 4, gauge, omega, n=1, storage=storage)
+        got = canon[torch.from_numpy(sites[inner]).cuda()].cpu().numpy().astype(np.float64)
+        worst = max(worst, np.abs(got - Up[inner]).max())
+    assert worst <= TOL_LINK[prec], worst
+
+    # ---- properties that hold at any size: links still SU(3); F rose; every link was rewritten
+    sample = torch.from_numpy(rng.integers(0, V, size=4096)).cuda()
+    Us = np.ascontiguousarray(canon[sample].cpu().numpy().astype(np.float64))
+    a, b = oracle.unitarity(Us, (4096, 1, 1, 1))
+    assert max(a, b) <= (1e-13 if prec == "f64" else 5e-6)
+    F1, th1 = fx.measure()
+    assert F1 > F0 + 0.1  # (theta may rise in the first overrelaxed sweep: omega > 1 overshoots the local maximum)
+    assert np.isfinite(th1) and 0.0 < th1 < 3 * th0
+    fx.close()

@@ -1,0 +1,213 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json north_star's: after one sweep max |dU_ij| <= 1e-12 (FP64) / 2e-5
+(FP32); F relative 1e-10 / 1e-5; theta within a factor 1.5; sweeps-to-convergence within +-2 %.
+
+FP32 runs are compared with the FP64 oracle fed the FP32-rounded input (reading A18); 12-real storage is emulated in
+the oracle by rebuilding row 2 after every link write (reading A13).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import gf_inputs as gi
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+# lattices: several 32-site blocks, a ragged tail (V/2 not a multiple of 32), minimal extents, unequal extents
+SHAPES = [(8, 8, 8, 8), (6, 4, 2, 2), (2, 2, 2, 2), (4, 6, 10, 2), (10, 6, 4, 4), (16, 4, 4, 6)]
+TOL_LINK = {"f64": 1e-12, "f32": 2e-5}
+TOL_F = {"f64": 1e-10, "f32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def gf():
+    import paper_1412_1498_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+def host_input(dims, roughness, seed, prec, storage):
+    """(what the GPU gets, what the FP64 oracle gets) for one field."""
+    dt = np.float32 if prec == "f32" else np.float64
+    U = gi.make_links(dims, roughness, seed, dtype=dt)
+    Uo = np.ascontiguousarray(U.astype(np.float64))
+    if storage == 12:
+        oracle.project12(Uo, dims)
+    return U, Uo
+
+
+def gpu_fixer(gf, torch, dims, gauge, prec, storage, U):
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=storage)
+    fx.set_links(torch.from_numpy(U).cuda())
+    return fx
+
+
+@pytest.mark.parametrize("dims", SHAPES)
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_set_get_roundtrip(gf, torch, dims, prec, storage):
+    U, Uo = host_input(dims, 0.5, 11, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, "landau", prec, storage, U)
+    back = fx.get_links().cpu().numpy()
+    if storage == 18:
+        assert np.array_equal(back, U)  # bit-identical
+    else:
+        assert np.array_equal(back[:, :, :2], U[:, :, :2])  # stored rows bit-identical
+        tol = 1e-15 if prec == "f64" else 5e-7
+        assert np.abs(back.astype(np.float64) - Uo).max() <= tol  # row 2 = conj(row0 x row1)
+    fx.close()
+
+
+@pytest.mark.parametrize("dims", SHAPES)
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_measure_matches_oracle(gf, torch, dims, gauge, prec, storage):
+    U, Uo = host_input(dims, 0.5, 12, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
+    F, th = fx.measure()
+    Fo, tho = oracle.measure(Uo, dims, gauge)
+    # F is O(1e-2) on a random gauge copy while the summands are O(1): compare on the scale of the summands
+    atol = 1e-13 if prec == "f64" else 2e-7
+    assert abs(F - Fo) <= atol
+    assert abs(th - tho) <= (1e-12 if prec == "f64" else 2e-6) * tho
+    fx.close()
+
+
+@pytest.mark.parametrize("dims", SHAPES)
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_one_sweep_links_match_oracle(gf, torch, dims, gauge, prec, storage):
+    omega = 1.7
+    U, Uo = host_input(dims, 0.5, 13, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
+    fx.ovr_sweep(1, omega)
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
+    assert np.abs(got - Uo).max() <= TOL_LINK[prec]
+    F, th = fx.measure()
+    Fo, tho = oracle.measure(Uo, dims, gauge)
+    assert abs(F - Fo) <= TOL_F[prec] * abs(Fo)
+    assert tho / 1.5 <= th <= tho * 1.5
+    fx.close()
+
+
+# The one-sweep bar is 1e-12.  Over several sweeps on a still-random field the map itself amplifies rounding: where a
+# subgroup's g is close to -1 (phi near pi) the rotation axis a_vec/|a_vec| is ill-conditioned (error x 1/|a_vec|), and
+# the closer omega is to 2 the less the sweep contracts.  The bounds below are 5 sweeps x that amplification.
+@pytest.mark.parametrize("omega,tol", [(1.0, 5e-12), (1.5, 5e-12), (1.99, 2e-9)])
+def test_several_sweeps_and_omegas(gf, torch, omega, tol):
+    dims = (6, 6, 4, 8)
+    U, Uo = host_input(dims, 0.3, 14, "f64", 18)
+    fx = gpu_fixer(gf, torch, dims, "landau", "f64", 18, U)
+    fx.ovr_sweep(5, omega)
+    got = fx.get_links().cpu().numpy()
+    oracle.sweeps(Uo, dims, "landau", omega, n=5)
+    assert np.abs(got - Uo).max() <= tol
+    fx.close()
+
+
+def test_degenerate_inputs_unit_and_converged(gf, torch):
+    # unit links: every r_vec = 0 exactly (reading A7 branch), F = 1, theta = 0, and the sweep is the identity
+    dims = (4, 4, 4, 4)
+    V = gi.volume(dims)
+    U = np.zeros((V, 4, 3, 3, 2))
+    for i in range(3):
+        U[:, :, i, i, 0] = 1.0
+    for prec, storage in [("f64", 18), ("f32", 12)]:
+        Ui = U.astype(np.float32 if prec == "f32" else np.float64)
+        fx = gpu_fixer(gf, torch, dims, "landau", prec, storage, Ui)
+        assert fx.measure() == (1.0, 0.0)
+        fx.ovr_sweep(2, 1.8)
+        assert np.array_equal(fx.get_links().cpu().numpy(), Ui)
+        assert fx.measure() == (1.0, 0.0)
+        fx.close()
+    # all links = -1 on the (0,1) block: a0 < 0 with s = 0 (phi = pi, axis undefined -> g = 1 on both sides)
+    Um = U.copy()
+    Um[:, :, 0, 0, 0] = -1.0
+    Um[:, :, 1, 1, 0] = -1.0
+    Uo = Um.copy()
+    fx = gpu_fixer(gf, torch, dims, "landau", "f64", 18, Um)
+    fx.ovr_sweep(1, 1.5)
+    oracle.sweeps(Uo, dims, "landau", 1.5, n=1)
+    got = fx.get_links().cpu().numpy()
+    assert np.isfinite(got).all() and np.abs(got - Uo).max() <= 1e-12
+    fx.close()
+
+
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_reunitarize_matches_oracle(gf, torch, prec, storage):
+    dims = (6, 4, 2, 2)
+    U, _ = host_input(dims, 0.5, 15, prec, storage)
+    rng = np.random.default_rng(3)
+    U = (U * (1 + 1e-3 * rng.standard_normal(U.shape))).astype(U.dtype)  # knock the links off SU(3)
+    Uo = np.ascontiguousarray(U.astype(np.float64))
+    if storage == 12:
+        oracle.project12(Uo, dims)
+    fx = gpu_fixer(gf, torch, dims, "landau", prec, storage, U)
+    fx.reunitarize()
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    oracle.reunitarize(Uo, dims)
+    assert np.abs(got - Uo).max() <= (1e-14 if prec == "f64" else 1e-6)
+    a, b = oracle.unitarity(np.ascontiguousarray(got), dims)
+    assert max(a, b) <= (1e-14 if prec == "f64" else 1e-6)
+    fx.close()
+
+
+def test_reunit_cadence_inside_sweeps(gf, torch):
+    dims = (4, 4, 4, 4)
+    U, Uo = host_input(dims, 0.4, 16, "f32", 12)
+    fx = gpu_fixer(gf, torch, dims, "landau", "f32", 12, U)
+    fx.set_reunit_every(3)
+    fx.ovr_sweep(4, 1.75)
+    fx.ovr_sweep(4, 1.75)  # global sweeps 3 and 6 reunitarise, across the two calls
+    n_launch = fx.kernel_launches()
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    oracle.sweeps(Uo, dims, "landau", 1.75, n=8, storage=12, reunit_every=3)
+    assert np.abs(got - Uo).max() <= 8 * 2e-5
+    assert n_launch == 1 + 16 + 2  # set_links + 16 half-sweeps + 2 reunitarisations
+    fx.close()
+
+
+def test_host_set_get(gf, torch):
+    dims = (8, 8, 8, 8)
+    U, _ = host_input(dims, 0.5, 17, "f64", 18)
+    fx = gf.GaugeFixer(dims)
+    pinned = torch.from_numpy(U).pin_memory()
+    fx.set_links_host(pinned)
+    out = torch.empty_like(pinned).pin_memory()
+    fx.get_links_host(out)
+    assert np.array_equal(out.numpy(), U)
+    fx.set_links_host(U)  # pageable numpy works too
+    assert np.array_equal(fx.get_links().cpu().numpy(), U)
+    fx.close()
+
+
+def test_argument_errors(gf, torch):
+    fx = gf.GaugeFixer((4, 4, 4, 4))
+    assert gf.gf_ovr_sweep(fx.ctx, 1, 2.0) == gf.GF_EINVAL      # omega in [1,2[
+    assert gf.gf_ovr_sweep(fx.ctx, 1, 0.99) == gf.GF_EINVAL
+    assert gf.gf_ovr_sweep(fx.ctx, -1, 1.5) == gf.GF_EINVAL
+    assert gf.gf_ovr_sweep(fx.ctx, 0, 1.5) == gf.GF_OK
+    assert gf.gf_fix(fx.ctx, 1.5, 1e-10, 10, 0)[0] == gf.GF_EINVAL
+    assert gf.gf_fix(fx.ctx, 1.5, -1.0, 10, 1)[0] == gf.GF_EINVAL
+    assert gf.gf_set_links(fx.ctx, 0) == gf.GF_EINVAL
+    assert gf.gf_set_reunit_every(fx.ctx, -1) == gf.GF_EINVAL
+    assert gf.gf_set_option(fx.ctx, 99, 0) == gf.GF_EINVAL
+    assert "omega" in gf.gf_last_error(fx.ctx) or gf.gf_last_error(fx.ctx)
+    # NaN links -> GF_ENUMERIC from measure
+    U = np.full((256, 4, 3, 3, 2), np.nan)
+    fx.set_links(torch.from_numpy(U).cuda())
+    assert gf.gf_measure(fx.ctx)[0] == gf.GF_ENUMERIC
+    fx.close()
+    with pytest.raises(gf.GFError):
+        gf.GaugeFixer((4, 4, 3, 4))

@@ -1,0 +1,84 @@
+"""GPU parity over whole Algorithm 1 runs: gf_fix on BASELINE.json configs 0 and 1 against the stored
+oracle trajectories (tests/golden/*_trajectory.json, written by tests/golden/make_golden.py from oracle/ only), and on a
+small lattice against the oracle run live.  Bars (north_star): F relative 1e-10 (FP64) / 1e-5 (FP32), theta within a
+factor 1.5, sweeps-to-convergence within +-2 %."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import gf_inputs as gi
+import oracle
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def run_gpu(cfg, dims=None):
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    dims = dims or cfg["dims"]
+    dt = np.float32 if cfg["prec"] == "f32" else np.float64
+    U = gi.make_links(dims, cfg["roughness"], cfg["seed"], dtype=dt)
+    fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=cfg["prec"], storage=cfg["storage"])
+    fx.set_links(torch.from_numpy(U).cuda())
+    fx.set_reunit_every(cfg["reunit_every"])
+    done = fx.fix(cfg["omega"], cfg["eps"], cfg["max_sweeps"], cfg["check_every"])
+    hist = fx.history()
+    links = fx.get_links().cpu().numpy()
+    fx.close()
+    return done, hist, links, U
+
+
+def compare_histories(hist, gold, tolF, converged):
+    """hist, gold: [(sweep, F, theta)].  F at every common checkpoint, theta within x1.5 wherever it is above the
+    rounding floor, and the final values."""
+    n = min(len(hist), len(gold))
+    for (s, F, th), (so, Fo, tho) in zip(hist[:n], gold[:n]):
+        assert s == so
+        assert abs(F - Fo) <= tolF * abs(Fo), (s, F, Fo)
+        if tho > 1e-9 or not converged:
+            assert tho / 1.5 <= th <= tho * 1.5, (s, th, tho)
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1"])
+def test_fix_matches_stored_oracle_trajectory(name):
+    cfg = next(c for c in gi.CONFIGS if c["name"] == name)
+    gold = json.load(open(os.path.join(HERE, "golden", f"{name}_trajectory.json")))
+    ghist = [(int(s), float(F), float(th)) for s, F, th in gold["history"]]
+    done, hist, links, _ = run_gpu(cfg)
+    converged = ghist[-1][2] < cfg["eps"]
+    assert abs(done - gold["sweeps_done"]) <= 0.02 * gold["sweeps_done"]
+    compare_histories(hist, ghist, 1e-10, converged)
+    Ff, thf = hist[-1][1], hist[-1][2]
+    assert abs(Ff - ghist[-1][1]) <= 1e-10 * abs(ghist[-1][1])
+    if converged:
+        assert thf < cfg["eps"]
+    else:
+        assert ghist[-1][2] / 1.5 <= thf <= ghist[-1][2] * 1.5
+    a, b = oracle.unitarity(np.ascontiguousarray(links.astype(np.float64)), cfg["dims"])
+    assert max(a, b) <= 1e-12  # still SU(3) after hundreds / thousands of sweeps without reunitarisation
+
+
+@pytest.mark.parametrize("name,dims", [("cfg2", (8, 8, 8, 8)), ("cfg3", (6, 6, 6, 12)), ("cfg4", (8, 8, 8, 16)),
+                                       ("cfg1", (8, 8, 8, 4))])
+def test_fix_small_lattice_live_oracle(name, dims):
+    """The run parameters of each config (precision, storage, gauge, omega, cadence, reunitarisation) on a lattice the
+    oracle finishes in seconds."""
+    cfg = dict(next(c for c in gi.CONFIGS if c["name"] == name))
+    cfg["max_sweeps"] = min(cfg["max_sweeps"], 400)
+    done, hist, links, U = run_gpu(cfg, dims)
+    Uo = np.ascontiguousarray(U.astype(np.float64))
+    if cfg["storage"] == 12:
+        oracle.project12(Uo, dims)
+    odone, ohist = oracle.fix(Uo, dims, cfg["gauge"], cfg["omega"], cfg["eps"], cfg["max_sweeps"], cfg["check_every"],
+                              cfg["reunit_every"], cfg["storage"])
+    tolF = 1e-10 if cfg["prec"] == "f64" else 1e-5
+    assert abs(done - odone) <= max(0.02 * odone, 0)
+    converged = ohist[-1][2] < cfg["eps"]
+    compare_histories(hist, [tuple(h) for h in ohist], tolF, converged)
+    if cfg["prec"] == "f64":
+        assert np.abs(links - Uo).max() <= 1e-8  # hundreds of sweeps: rounding grows in the early, random phase only
