@@ -102,8 +102,14 @@ int gf_set_reunit_every(gf_ctx* ctx, int k);
 
 /* Tuning knobs for benchmarking kernel variants; the defaults are the fastest measured.  GF_EINVAL on unknown keys. */
 enum {
-  GF_OPT_SWEEP_VARIANT = 1, /* which half-sweep kernel: 0 = default for this (prec, storage) */
-  GF_OPT_BLOCK_THREADS = 2  /* threads per block of the half-sweep kernel (multiple of 32; 0 = default) */
+  GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (= 3); 1 = two-pass; 2 = two-pass + L2 bulk prefetch;
+                               3 = staged through shared memory with cp.async; see DESIGN.md.  All variants give
+                               bit-identical links. */
+  GF_OPT_BLOCK_THREADS = 2, /* threads per block of the half-sweep kernel (0 = default; a value the chosen variant
+                               has no instantiation for makes the next sweep fail with GF_ECUDA) */
+  GF_OPT_FUSE_MEASURE = 3   /* 1 (default): the last odd half-sweep of every gf_ovr_sweep call also leaves the odd
+                               sites' terms of theta, so a gf_measure that follows directly visits the even sites only
+                               and reads every link once; 0: gf_measure always visits all sites */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 

@@ -17,7 +17,7 @@ constexpr size_t STAGING_BYTES = 64u << 20;  // each of the two staging buffers 
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Sizes {
-  size_t links, partials, result, staging, total;
+  size_t links, partials, qpartials, result, staging, total;
 };
 
 bool valid_lattice(int nx, int ny, int nz, int nt, int* err) {
@@ -46,9 +46,10 @@ Sizes sizes_of(const Geo& g, int prec, int storage) {
   const size_t csize = prec == GF_FP64 ? 16 : 8;
   s.links = align_up((size_t)2 * g.nblk * 4 * (storage / 2) * 32 * csize);
   s.partials = align_up((size_t)measure_num_partials(g) * sizeof(double2));
+  s.qpartials = align_up((size_t)halfsweep_max_qblocks(g) * sizeof(double));
   s.result = align_up(2 * sizeof(double));
   s.staging = align_up(STAGING_BYTES);
-  s.total = s.links + s.partials + s.result + 2 * s.staging;
+  s.total = s.links + s.partials + s.qpartials + s.result + 2 * s.staging;
   return s;
 }
 }  // namespace
@@ -60,6 +61,8 @@ struct gf_ctx {
   cudaEvent_t staging_free[2];
   double* host_result;  // pinned, 2 doubles
   int reunit_every;
+  int fuse_measure;  // GF_OPT_FUSE_MEASURE
+  int qblocks;       // > 0: k.qpartials[0..qblocks) hold the odd sites' theta terms of the links as they stand
   long long sweeps_total;  // sweeps since the last gf_set_links (reunitarisation cadence)
   long long launches;
   std::vector<double> history;
@@ -113,9 +116,11 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   char* base = (char*)dev_workspace;
   c->k.links = base;
   c->k.partials = base + sz.links;
-  c->k.result = base + sz.links + sz.partials;
-  c->staging[0] = base + sz.links + sz.partials + sz.result;
+  c->k.qpartials = base + sz.links + sz.partials;
+  c->k.result = base + sz.links + sz.partials + sz.qpartials;
+  c->staging[0] = base + sz.links + sz.partials + sz.qpartials + sz.result;
   c->staging[1] = c->staging[0] + sz.staging;
+  c->fuse_measure = 1; c->qblocks = 0;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
   c->host_result = nullptr;
@@ -148,6 +153,7 @@ int gf_set_links(gf_ctx* c, const void* dev_links) {
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links");
   c->launches += 1;
   c->sweeps_total = 0;
+  c->qblocks = 0;
   return GF_OK;
 }
 
@@ -191,6 +197,7 @@ int gf_set_links_host(gf_ctx* c, const void* host_links) {
   if (!c) return GF_EINVAL;
   if (!host_links) return fail(c, GF_EINVAL, "gf_set_links_host: null links");
   c->sweeps_total = 0;
+  c->qblocks = 0;
   return links_host(c, const_cast<void*>(host_links), true);
 }
 
@@ -202,6 +209,7 @@ int gf_get_links_host(gf_ctx* c, void* host_links_out) {
 
 int gf_reunitarize(gf_ctx* c) {
   if (!c) return GF_EINVAL;
+  c->qblocks = 0;
   cudaError_t e = launch_reunit(c->k);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_reunitarize");
   c->launches += 1;
@@ -219,8 +227,12 @@ int gf_set_option(gf_ctx* c, int key, int value) {
   if (!c) return GF_EINVAL;
   switch (key) {
     case GF_OPT_SWEEP_VARIANT:
-      if (value < 0) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
+      if (value < 0 || value > 3) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
       c->k.variant = value;
+      return GF_OK;
+    case GF_OPT_FUSE_MEASURE:
+      c->fuse_measure = value != 0;
+      if (!c->fuse_measure) c->qblocks = 0;
       return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
@@ -235,11 +247,16 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
   if (!c) return GF_EINVAL;
   if (n < 0) return fail(c, GF_EINVAL, "gf_ovr_sweep: n < 0");
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
+  if (n > 0) c->qblocks = 0;
   for (int i = 0; i < n; ++i) {
     for (int parity = 0; parity < 2; ++parity) {  // even first
-      cudaError_t e = launch_halfsweep(c->k, parity, omega);
+      // the last odd half-sweep of the call also leaves the odd sites' theta terms for a gf_measure that may follow
+      const bool fuse = c->fuse_measure && parity == 1 && i == n - 1 && halfsweep_can_fuse_theta(c->k);
+      int qblocks = 0;
+      cudaError_t e = launch_halfsweep(c->k, parity, omega, fuse, &qblocks);
       if (e != cudaSuccess) return fail_cuda(c, e, "gf_ovr_sweep");
       c->launches += 1;
+      c->qblocks = qblocks;
     }
     c->sweeps_total += 1;
     if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) {
@@ -253,7 +270,7 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
 int gf_measure(gf_ctx* c, double* F, double* theta) {
   if (!c) return GF_EINVAL;
   if (!F || !theta) return fail(c, GF_EINVAL, "gf_measure: null out-param");
-  cudaError_t e = launch_measure(c->k);
+  cudaError_t e = launch_measure(c->k, c->qblocks);
   if (e == cudaSuccess)
     e = cudaMemcpyAsync(c->host_result, c->k.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->k.stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);

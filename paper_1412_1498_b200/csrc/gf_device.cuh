@@ -169,13 +169,14 @@ __device__ __forceinline__ void su2_step(C (&K)[9], C (&G)[9], T omega) {
 }
 
 // G = g3 g2 g1 for one site from its K (Algorithm 1 l.5-6; subgroup order (0,1),(1,2),(0,2), reading A4; A8)
-template <class T, class C>
+// FINAL_K: also carry K through the last step, so that on return K = G K_in (= K(x) of the updated links).
+template <class T, bool FINAL_K = false, class C>
 __device__ __forceinline__ void site_gauge_rotation(C (&K)[9], C (&G)[9], T omega) {
 #pragma unroll
   for (int e = 0; e < 9; ++e) G[e] = mk<T>((e % 4 == 0) ? T(1) : T(0), T(0));
   su2_step<0, 1, true>(K, G, omega);
   su2_step<1, 2, true>(K, G, omega);
-  su2_step<0, 2, false>(K, G, omega);
+  su2_step<0, 2, FINAL_K>(K, G, omega);
 }
 
 // rows 0..NROW-1 of G.U

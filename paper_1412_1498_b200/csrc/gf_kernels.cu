@@ -70,22 +70,103 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
 }
 
 // ======================================================================================================================
-// overrelaxation half-sweep, variant 0: one thread per site, two passes over the site's eight links
+// deterministic block sums (warp shuffles, then one shared-memory hop between warps; FP64 in both precisions)
 // ======================================================================================================================
-// Pass 1 streams the 2*ND links that enter K(x) (eq. 1.5) and sums them in registers; the three SU(2) steps give
-// G(x); pass 2 re-reads each of the eight links (L1/L2 hit: same thread, same addresses, nothing written between),
-// multiplies and stores in place.  Same-parity sites touch disjoint links, so there is no inter-thread hazard.
-template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS>
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum of (f, q) over the THREADS threads of the block; valid in thread 0.  Every thread of the block must call it.
+template <int THREADS>
+__device__ __forceinline__ void block_sum2(double& f, double& q) {
+  static_assert(THREADS % 32 == 0 && THREADS <= 1024, "whole warps");
+  constexpr int NW = THREADS / 32;
+  f = warp_sum(f);
+  q = warp_sum(q);
+  if (NW == 1) return;
+  __shared__ double sf[NW], sq[NW];
+  if ((threadIdx.x & 31) == 0) { sf[threadIdx.x >> 5] = f; sq[threadIdx.x >> 5] = q; }
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    f = threadIdx.x < NW ? sf[threadIdx.x] : 0.0;
+    q = threadIdx.x < NW ? sq[threadIdx.x] : 0.0;
+    f = warp_sum(f);
+    q = warp_sum(q);
+  }
+}
+
+// sum_ij |Delta_ij|^2 for Delta = (A - A^dag) - (1/3) Tr(A - A^dag)  (eqs. 1.2-1.3, reading A2).  The sign of A drops
+// out, so A may be sum_nu [U_nu(x-nu) - U_nu(x)] or K(x) of eq. 1.5 (A - A^dag = -(K - K^dag)).
+template <class T, class C>
+__device__ __forceinline__ T delta_norm2(const C (&A)[9]) {
+  // D = A - A^dag: D_ii = 2i Im A_ii; D_ij = A_ij - conj(A_ji);  traceless part: D_ii -= (1/3) sum_k D_kk
+  const T d0 = T(2) * A[0].y, d1 = T(2) * A[4].y, d2 = T(2) * A[8].y;
+  const T m = (d0 + d1 + d2) / T(3);
+  T acc = (d0 - m) * (d0 - m) + (d1 - m) * (d1 - m) + (d2 - m) * (d2 - m);
+  // off-diagonal: |D_ij|^2 = |D_ji|^2, so count each pair twice
+  const T ax = A[1].x - A[3].x, ay = A[1].y + A[3].y; acc += T(2) * (ax * ax + ay * ay);
+  const T bx = A[2].x - A[6].x, by = A[2].y + A[6].y; acc += T(2) * (bx * bx + by * by);
+  const T cx = A[5].x - A[7].x, cy = A[5].y + A[7].y; acc += T(2) * (cx * cx + cy * cy);
+  return acc;
+}
+
+// ======================================================================================================================
+// overrelaxation half-sweep
+// ======================================================================================================================
+// One thread per site in every variant; same-parity sites touch disjoint links, so there is no
+// inter-thread hazard and no block-level synchronisation.
+//
+//  "two-pass": pass 1 streams the 2*ND links that enter K(x) (eq. 1.5) and sums them in registers; the
+//      three SU(2) steps give G(x); pass 2 re-reads each of the eight links (L1/L2 hit: same thread, same addresses,
+//      nothing written between), multiplies and stores in place.
+//  "two-pass + L2 bulk prefetch": the same, but each warp first asks the TMA unit to pull its whole
+//      working set (the contiguous 4-direction forward chunk and the backward tiles) into L2 with
+//      cp.async.bulk.prefetch.L2, so the bytes in flight per SM do not depend on how many loads the register budget
+//      lets the compiler hoist.
+//  "staged" (the default): every thread copies its eight links global -> shared with cp.async (LDGSTS; no registers
+//      tied up, all 8*L bytes of the site in flight at once), waits for its own copies, then works out of shared
+//      memory in a single pass: each link crosses L2 -> SM once.  Shared slots are thread-private: no barrier.
+template <class T, int NELEM, class C>
+__device__ __forceinline__ void site_pointers(C* __restrict__ links, const Geo& g, int parity, int cb, C*& fwd,
+                                              C* (&bwd)[4]) {
+  const Site s = site_of(g, parity, cb);
+  fwd = links + link_offset<NELEM>(g, parity, cb, 0);  // + mu*NELEM*32 for direction mu
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) bwd[mu] = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
+}
+
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool PREFETCH>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) {
   using C = cplx_t<T>;
-  const int cb = blockIdx.x * THREADS + threadIdx.x;
-  if (cb >= g.vh) return;
-  const Site s = site_of(g, parity, cb);
-  C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);  // + mu*NELEM*32 for direction mu
+  int cb = blockIdx.x * THREADS + threadIdx.x;
+  const bool live = cb < g.vh;
+  if (!PREFETCH && !live) return;
+  if (!live) cb = g.vh - 1;  // keep the warp converged for the shuffles below; the lane does no loads or stores
+  C* fwd;
   C* bwd[4];
+  site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
+
+  if (PREFETCH) {
+    const unsigned lane = threadIdx.x & 31;
+    constexpr unsigned TILE = NELEM * 32 * sizeof(C);  // one (block, mu) tile
+    // forward links of the warp's 32 sites: one contiguous 4-tile chunk
+    if (lane == 0) prefetch_l2_bulk(links + link_offset<NELEM>(g, parity, cb & ~31, 0), 4 * TILE);
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) bwd[mu] = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
+    for (int mu = 0; mu < 4; ++mu) {
+      // tile (32-site block of the other parity) holding this lane's backward neighbour; one request per distinct tile
+      const unsigned long long tile = (unsigned long long)(bwd[mu] - links) / (NELEM * 32);
+      const unsigned long long prev = __shfl_up_sync(0xffffffffu, tile, 1);
+      if (lane == 0 || tile != prev) prefetch_l2_bulk(links + tile * (NELEM * 32), TILE);
+    }
+    if (!live) return;
+  }
 
   C K[9];
 #pragma unroll
@@ -118,44 +199,181 @@ ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) 
   }
 }
 
-template <class T, int NELEM, int ND>
-static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega) {
-  constexpr int THREADS = 128;
+// ---- staged through shared memory with cp.async ---------------------------------------------------------
+template <class T> constexpr int staged_threads() { return sizeof(T) == 8 ? 64 : 128; }
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (BYTES == 16)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+  else
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+// keeps the compiler from hoisting every shared-memory load of the site to the top (which spills)
+__device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// shared slot of (link l, element e) of this thread: [l][e][THREADS] complex numbers, lane-contiguous (no bank conflicts)
+template <int NELEM, int THREADS, bool FULL, class C>
+__device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
+#pragma unroll
+  for (int e = 0; e < NELEM; ++e) u[e] = sm[(l * NELEM + e) * THREADS];
+  if (NELEM == 6 && FULL) rebuild_row2(u);
+}
+
+// MEASURE: the launch also leaves, per block, the sum over its sites of sum_ij |Delta_ij(x)|^2 AFTER the update, taken
+// from K_final(x) = G(x) K(x), which is K(x) of the updated links (the site's own update is the last one to touch
+// them in this half-sweep).  After the odd half-sweep these are the odd sites' terms of theta of the finished sweep.
+template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE>
+__global__ void __launch_bounds__(THREADS, MINBLOCKS)
+ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
+  using C = cplx_t<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C* sm = reinterpret_cast<C*>(smem_raw) + threadIdx.x;
+  const int cb = blockIdx.x * THREADS + threadIdx.x;
+  const bool live = cb < g.vh;
+  if (!MEASURE && !live) return;
+  double q = 0.0;
+  if (live) {
+    C* fwd;
+    C* bwd[4];
+    site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
+
+    // links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu)
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+#pragma unroll
+      for (int e = 0; e < NELEM; ++e) {
+        cp_async<sizeof(C)>(sm + ((2 * mu) * NELEM + e) * THREADS, fwd + (mu * NELEM + e) * 32);
+        cp_async<sizeof(C)>(sm + ((2 * mu + 1) * NELEM + e) * THREADS, bwd[mu] + e * 32);
+      }
+    }
+    cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
+
+    C K[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) K[e] = mk<T>(T(0), T(0));
+#pragma unroll
+    for (int mu = 0; mu < ND; ++mu) {
+      C u[9];
+      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
+#pragma unroll
+      for (int e = 0; e < 9; ++e) { K[e].x += u[e].x; K[e].y += u[e].y; }
+      sched_fence();
+      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu + 1, u);
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) { K[i * 3 + j].x += u[j * 3 + i].x; K[i * 3 + j].y -= u[j * 3 + i].y; }
+      sched_fence();
+    }
+
+    C G[9];
+    site_gauge_rotation<T, MEASURE>(K, G, omega);
+    if (MEASURE) q = (double)delta_norm2<T>(K);
+
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      C u[9], w[9];
+      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
+      mul_left<NELEM / 3>(G, u, w);                       // U_mu(x) <- G U_mu(x)
+      store_link<NELEM>(fwd + mu * NELEM * 32, w);
+      sched_fence();
+      load_link_smem<NELEM, THREADS, false>(sm, 2 * mu + 1, u);
+      mul_right_adj<NELEM / 3>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+      store_link<NELEM>(bwd[mu], w);
+      sched_fence();
+    }
+  }
+  if (MEASURE) {
+    double f = 0.0;
+    block_sum2<THREADS>(f, q);
+    if (threadIdx.x == 0) qpartials[blockIdx.x] = q;
+  }
+}
+
+template <class T, int NELEM, int ND, int THREADS, bool MEASURE>
+static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double omega) {
+  using C = cplx_t<T>;
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, 1, MEASURE>;
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1><<<blocks, THREADS, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, parity,
-                                                                                  (T)omega);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials);
   return cudaGetLastError();
 }
 
-cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega) {
-  const bool coul = a.gauge == 1;
-  if (a.prec == 0) {
-    if (a.storage == 18) return coul ? halfsweep_T<double, 9, 3>(a, parity, omega) : halfsweep_T<double, 9, 4>(a, parity, omega);
-    return coul ? halfsweep_T<double, 6, 3>(a, parity, omega) : halfsweep_T<double, 6, 4>(a, parity, omega);
+// Variant numbering of GF_OPT_SWEEP_VARIANT: 0 = library default (staged), 1 = two-pass, 2 = two-pass + L2 bulk prefetch,
+// 3 = staged.  Measured on B200 (profiles/): staged 6.8 TB/s on cfg4 and cfg3 against 6.3 / 5.7 TB/s two-pass.
+template <class T, int NELEM, int ND>
+static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
+  using C = cplx_t<T>;
+  *qblocks = 0;
+  if (a.variant == 0 || a.variant == 3) {
+    // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
+    constexpr int THREADS = staged_threads<T>();
+    if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
+    if (fuse_theta) {
+      *qblocks = (a.geo.vh + THREADS - 1) / THREADS;
+      return halfsweep_staged_T<T, NELEM, ND, THREADS, true>(a, parity, omega);
+    }
+    return halfsweep_staged_T<T, NELEM, ND, THREADS, false>(a, parity, omega);
   }
-  if (a.storage == 18) return coul ? halfsweep_T<float, 9, 3>(a, parity, omega) : halfsweep_T<float, 9, 4>(a, parity, omega);
-  return coul ? halfsweep_T<float, 6, 3>(a, parity, omega) : halfsweep_T<float, 6, 4>(a, parity, omega);
+  constexpr int THREADS = 128;
+  if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
+  const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
+  if (a.variant == 2)
+    ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1, true><<<blocks, THREADS, 0, a.stream>>>((C*)a.links, a.geo, parity,
+                                                                                          (T)omega);
+  else if (a.variant == 1)
+    ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1, false><<<blocks, THREADS, 0, a.stream>>>((C*)a.links, a.geo, parity,
+                                                                                           (T)omega);
+  else
+    return cudaErrorInvalidValue;
+  return cudaGetLastError();
 }
+
+#define GF_DISPATCH(FN, ...)                                                                              \
+  do {                                                                                                    \
+    const bool coul = a.gauge == 1;                                                                       \
+    if (a.prec == 0) {                                                                                    \
+      if (a.storage == 18) return coul ? FN<double, 9, 3>(__VA_ARGS__) : FN<double, 9, 4>(__VA_ARGS__);   \
+      return coul ? FN<double, 6, 3>(__VA_ARGS__) : FN<double, 6, 4>(__VA_ARGS__);                        \
+    }                                                                                                     \
+    if (a.storage == 18) return coul ? FN<float, 9, 3>(__VA_ARGS__) : FN<float, 9, 4>(__VA_ARGS__);       \
+    return coul ? FN<float, 6, 3>(__VA_ARGS__) : FN<float, 6, 4>(__VA_ARGS__);                            \
+  } while (0)
+
+cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
+  GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
+}
+
+bool halfsweep_can_fuse_theta(const KernelArgs& a) { return a.variant == 0 || a.variant == 3; }
+int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
 // ======================================================================================================================
 // F and theta
 // ======================================================================================================================
-// One thread per site (both parities).  Per site: f = sum_{mu<ND} Re Tr U_mu(x);  A = sum_{nu<ND} [U_nu(x-nu) - U_nu(x)];
-// Delta = (A - A^dag) - (1/3) Tr(A - A^dag);  q = sum_ij |Delta_ij|^2   (eqs. 1.1-1.3, readings A1, A2).
+// One thread per site.  Per site: f = sum_{nu<ND} Re Tr [U_nu(x) + U_nu(x-nu)] (= Re Tr K(x));
+// A = sum_{nu<ND} [U_nu(x-nu) - U_nu(x)];  Delta = (A - A^dag) - (1/3) Tr(A - A^dag);  q = sum_ij |Delta_ij|^2
+// (eqs. 1.1-1.3, readings A1, A2).  Every link touches exactly one site of each parity, so the sum of f over the sites
+// of ONE parity is the sum of Re Tr U over all links: F needs the even sites only, and a pass over the sites of one
+// parity reads every link exactly once.
+// Grid: blocks_per_parity * nparity blocks; the first blocks_per_parity blocks take parity `parity0`, the rest the other.
 // Block partials by warp shuffles (FP64), one double2 per block; a single-block second stage adds them in index order.
 constexpr int MEASURE_THREADS = 256;
 
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
 template <class T, int NELEM, int ND>
 __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const cplx_t<T>* __restrict__ links, Geo g,
+                                                                          int blocks_per_parity,
                                                                           double2* __restrict__ partials) {
   using C = cplx_t<T>;
-  const int blocks_per_parity = gridDim.x >> 1;
   const int parity = blockIdx.x >= blocks_per_parity;
   const int cb = (blockIdx.x - parity * blocks_per_parity) * MEASURE_THREADS + threadIdx.x;
   double f = 0.0, q = 0.0;
@@ -172,79 +390,54 @@ __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const 
       load_link<NELEM, true>(links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu), u);
 #pragma unroll
       for (int e = 0; e < 9; ++e) { A[e].x += u[e].x; A[e].y += u[e].y; }
+      tr += u[0].x + u[4].x + u[8].x;
       load_link<NELEM, true>(fwd + nu * NELEM * 32, u);
 #pragma unroll
       for (int e = 0; e < 9; ++e) { A[e].x -= u[e].x; A[e].y -= u[e].y; }
       tr += u[0].x + u[4].x + u[8].x;
     }
     f = (double)tr;
-    // D = A - A^dag: D_ii = 2i Im A_ii; D_ij = A_ij - conj(A_ji);  traceless part: D_ii -= (1/3) sum_k D_kk
-    const T d0 = T(2) * A[0].y, d1 = T(2) * A[4].y, d2 = T(2) * A[8].y;
-    const T m = (d0 + d1 + d2) / T(3);
-    T acc = (d0 - m) * (d0 - m) + (d1 - m) * (d1 - m) + (d2 - m) * (d2 - m);
-    // off-diagonal: |D_ij|^2 = |D_ji|^2, so count each pair twice
-    {
-      const T ax = A[1].x - A[3].x, ay = A[1].y + A[3].y; acc += T(2) * (ax * ax + ay * ay);
-      const T bx = A[2].x - A[6].x, by = A[2].y + A[6].y; acc += T(2) * (bx * bx + by * by);
-      const T cx = A[5].x - A[7].x, cy = A[5].y + A[7].y; acc += T(2) * (cx * cx + cy * cy);
-    }
-    q = (double)acc;
+    q = (double)delta_norm2<T>(A);
   }
-  __shared__ double sf[MEASURE_THREADS / 32], sq[MEASURE_THREADS / 32];
-  f = warp_sum(f);
-  q = warp_sum(q);
-  if ((threadIdx.x & 31) == 0) { sf[threadIdx.x >> 5] = f; sq[threadIdx.x >> 5] = q; }
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    f = threadIdx.x < MEASURE_THREADS / 32 ? sf[threadIdx.x] : 0.0;
-    q = threadIdx.x < MEASURE_THREADS / 32 ? sq[threadIdx.x] : 0.0;
-    f = warp_sum(f);
-    q = warp_sum(q);
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(f, q);
-  }
+  block_sum2<MEASURE_THREADS>(f, q);
+  if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(f, q);
 }
 
-// second stage: one block of 1024 threads; thread i adds partials i, i+1024, ... in order; fixed tree afterwards
-__global__ void __launch_bounds__(1024) measure_final_kernel(const double2* __restrict__ partials, int n, double norm_f,
-                                                             double norm_q, double* __restrict__ result) {
+// second stage: one block of 1024 threads; thread i adds partials i, i+1024, ... in order; fixed tree afterwards.
+// f is summed over the first nf entries of `partials` only (the even sites), q over all n of them plus the nq entries
+// of `qpartials` (the odd sites' terms left by the last odd half-sweep, when they are valid).
+__global__ void __launch_bounds__(1024) measure_final_kernel(const double2* __restrict__ partials, int n, int nf,
+                                                             const double* __restrict__ qpartials, int nq,
+                                                             double norm_f, double norm_q, double* __restrict__ result) {
   double f = 0.0, q = 0.0;
-  for (int i = threadIdx.x; i < n; i += 1024) { f += partials[i].x; q += partials[i].y; }
-  __shared__ double sf[32], sq[32];
-  f = warp_sum(f);
-  q = warp_sum(q);
-  if ((threadIdx.x & 31) == 0) { sf[threadIdx.x >> 5] = f; sq[threadIdx.x >> 5] = q; }
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    f = warp_sum(sf[threadIdx.x]);
-    q = warp_sum(sq[threadIdx.x]);
-    if (threadIdx.x == 0) { result[0] = f * norm_f; result[1] = q * norm_q; }
+  for (int i = threadIdx.x; i < n; i += 1024) {
+    const double2 p = partials[i];
+    if (i < nf) f += p.x;
+    q += p.y;
   }
+  for (int i = threadIdx.x; i < nq; i += 1024) q += qpartials[i];
+  block_sum2<1024>(f, q);
+  if (threadIdx.x == 0) { result[0] = f * norm_f; result[1] = q * norm_q; }
 }
 
 int measure_num_partials(const Geo& g) { return 2 * ((g.vh + MEASURE_THREADS - 1) / MEASURE_THREADS); }
 
+// nq > 0: the odd sites' theta terms are already in a.qpartials[0..nq): visit the even sites only.
 template <class T, int NELEM, int ND>
-static cudaError_t measure_T(const KernelArgs& a) {
-  const int nblk = measure_num_partials(a.geo);
-  measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo,
+static cudaError_t measure_T(const KernelArgs& a, int nq) {
+  const int bpp = measure_num_partials(a.geo) / 2;
+  const int nblk = nq > 0 ? bpp : 2 * bpp;
+  measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo, bpp,
                                                                               (double2*)a.partials);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   const double V = 2.0 * (double)a.geo.vh;
-  measure_final_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, 1.0 / (ND * 3.0 * V),
-                                                 1.0 / (3.0 * V), (double*)a.result);
+  measure_final_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, bpp, (const double*)a.qpartials, nq,
+                                                 1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V), (double*)a.result);
   return cudaGetLastError();
 }
 
-cudaError_t launch_measure(const KernelArgs& a) {
-  const bool coul = a.gauge == 1;
-  if (a.prec == 0) {
-    if (a.storage == 18) return coul ? measure_T<double, 9, 3>(a) : measure_T<double, 9, 4>(a);
-    return coul ? measure_T<double, 6, 3>(a) : measure_T<double, 6, 4>(a);
-  }
-  if (a.storage == 18) return coul ? measure_T<float, 9, 3>(a) : measure_T<float, 9, 4>(a);
-  return coul ? measure_T<float, 6, 3>(a) : measure_T<float, 6, 4>(a);
-}
+cudaError_t launch_measure(const KernelArgs& a, int nq) { GF_DISPATCH(measure_T, a, nq); }
 
 // ======================================================================================================================
 // reunitarisation

@@ -203,6 +203,7 @@ def test_argument_errors(gf, torch):
     assert gf.gf_set_links(fx.ctx, 0) == gf.GF_EINVAL
     assert gf.gf_set_reunit_every(fx.ctx, -1) == gf.GF_EINVAL
     assert gf.gf_set_option(fx.ctx, 99, 0) == gf.GF_EINVAL
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_SWEEP_VARIANT, 7) == gf.GF_EINVAL
     assert "omega" in gf.gf_last_error(fx.ctx) or gf.gf_last_error(fx.ctx)
     # NaN links -> GF_ENUMERIC from measure
     U = np.full((256, 4, 3, 3, 2), np.nan)
@@ -211,3 +212,74 @@ def test_argument_errors(gf, torch):
     fx.close()
     with pytest.raises(gf.GFError):
         gf.GaugeFixer((4, 4, 3, 4))
+
+
+# ---- kernel variants and the fused theta terms ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4), (2, 2, 2, 2)])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_halfsweep_variants_agree_bit_for_bit_and_match_oracle(gf, torch, dims, gauge, prec, storage):
+    """GF_OPT_SWEEP_VARIANT 1 (two-pass), 2 (two-pass + L2 bulk prefetch), 3 (staged, the default): same arithmetic per
+    site in the same order, so the links must be bit-identical; each is also held to the one-sweep oracle bar."""
+    omega = 1.7
+    U, Uo = host_input(dims, 0.5, 13, prec, storage)  # the input of test_one_sweep_links_match_oracle
+    oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
+    ref = None
+    for variant in (0, 1, 2, 3):
+        fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
+        fx.set_option(gf.GF_OPT_SWEEP_VARIANT, variant)
+        fx.ovr_sweep(1, omega)
+        got = fx.get_links().cpu().numpy()
+        assert np.abs(got.astype(np.float64) - Uo).max() <= TOL_LINK[prec]
+        fx.ovr_sweep(2, omega)
+        got = fx.get_links().cpu().numpy()
+        if ref is None:
+            ref = got
+        assert np.array_equal(got, ref), f"variant {variant} differs from the default"
+        fx.close()
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4)])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_fused_theta_terms_match_full_measure_and_oracle(gf, torch, dims, gauge, prec, storage):
+    """After gf_ovr_sweep the odd sites' theta terms come from K_final = G K inside the odd half-sweep and gf_measure
+    visits the even sites only; with GF_OPT_FUSE_MEASURE = 0 it visits all sites.  Both against the oracle."""
+    omega = 1.7
+    U, Uo = host_input(dims, 0.4, 22, prec, storage)
+    oracle.sweeps(Uo, dims, gauge, omega, n=3, storage=storage)
+    Fo, tho = oracle.measure(Uo, dims, gauge)
+    res = {}
+    for fuse in (1, 0):
+        fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
+        fx.set_option(gf.GF_OPT_FUSE_MEASURE, fuse)
+        fx.ovr_sweep(3, omega)
+        n0 = fx.kernel_launches()
+        res[fuse] = fx.measure()
+        assert fx.kernel_launches() - n0 == 2
+        again = fx.measure()  # the fused terms stay valid until the links change
+        assert again == res[fuse]
+        fx.reunitarize()  # changes the links: the next measure must visit all sites again
+        F2, th2 = fx.measure()
+        fx.close()
+    rtol_th = 1e-9 if prec == "f64" else 2e-4
+    assert res[1][0] == res[0][0]  # F is summed over the even sites in both modes
+    assert abs(res[1][1] - res[0][1]) <= rtol_th * res[0][1]
+    for F, th in res.values():
+        assert abs(F - Fo) <= TOL_F[prec] * abs(Fo)
+        assert abs(th - tho) <= (1e-8 if prec == "f64" else 1e-3) * tho
+
+
+def test_fused_theta_terms_near_convergence(gf, torch):
+    """theta ~ 1e-13: the fused terms are differences of O(1) entries of G K; they must still track the oracle."""
+    dims = (4, 4, 4, 4)
+    U, Uo = host_input(dims, 0.2, 23, "f64", 18)
+    fx = gpu_fixer(gf, torch, dims, "landau", "f64", 18, U)
+    done = fx.fix(1.6, 1e-13, 2000, 10)
+    hist = fx.history()
+    do, ho = oracle.fix(Uo, dims, "landau", 1.6, 1e-13, 2000, 10)
+    assert done == do and len(hist) == len(ho)
+    for (s, F, th), (so, Fo, tho) in zip(hist, ho):
+        assert s == so and abs(F - Fo) <= 1e-10 * abs(Fo)
+        assert tho / 1.5 <= th <= tho * 1.5 or max(th, tho) < 1e-25
+    fx.close()
