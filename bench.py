@@ -185,6 +185,23 @@ def run_reference(args):
     return 0
 
 
+# ---- replicas: the only cross-rank traffic is the barrier and this MAX -------------------------------------
+def max_over_ranks(ms_local, dist, device):
+    """Elapsed time of the slowest replica.  dist = None (one process) or an initialised torch.distributed module."""
+    if dist is None:
+        return float(ms_local)
+    import torch
+
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, sites, sweeps, ms):
+    """Whole-job site-updates/s of `world` replicas that each did `sweeps` sweeps of `sites` sites in `ms` (max)."""
+    return world * sites * sweeps / (ms * 1e-3)
+
+
 # ---- the CUDA path -----------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
@@ -263,11 +280,8 @@ def run_ours(args):
     ms_measure = sum(b.elapsed_time(c) for _, b, c in timers)
     n_reunit = 0 if not cfg["reunit_every"] else sum(
         1 for s in range((args.warmup) * n_sw + 1, (args.warmup + args.steps) * n_sw + 1) if s % cfg["reunit_every"] == 0)
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * V * n_sw * args.steps / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
+    value = aggregate_value(world, V, n_sw * args.steps, ms_total)
 
     # ---- roofline of the dominant kernel (half-sweep): 2*n_sw launches per step, back to back on the stream
     peak, peak_src = load_peaks()
@@ -312,12 +326,9 @@ def run_ours(args):
         barrier()
         wall = time.perf_counter() - w0
         ms_e2e = max(e0.elapsed_time(e1), wall * 1e3)  # host-side copies of pageable chunks would not show in events
-        if dist is not None:
-            t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
+        ms_e2e = max_over_ranks(ms_e2e, dist, "cuda")
         nbytes = V * 72 * (8 if prec == "f64" else 4)
-        e2e = {"value": world * V * n_sw * n_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": aggregate_value(world, V, n_sw * n_e2e, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 16, "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e,
                "what": "gf_set_links_host (pinned) + %d sweeps + gf_measure + gf_get_links_host (pinned)" % n_sw}
         del host
