@@ -107,11 +107,36 @@ enum {
                                bit-identical links. */
   GF_OPT_BLOCK_THREADS = 2, /* threads per block of the half-sweep kernel (0 = default; a value the chosen variant
                                has no instantiation for makes the next sweep fail with GF_ECUDA) */
-  GF_OPT_FUSE_MEASURE = 3   /* 1 (default): the last odd half-sweep of every gf_ovr_sweep call also leaves the odd
+  GF_OPT_FUSE_MEASURE = 3,  /* 1 (default): the last odd half-sweep of every gf_ovr_sweep call also leaves the odd
                                sites' terms of theta, so a gf_measure that follows directly visits the even sites only
                                and reads every link once; 0: gf_measure always visits all sites */
+  GF_OPT_FFT_ACCELERATE = 4 /* 1 (default): gf_fft_step / gf_fix_fft use the Fourier factor of eq. 1.8; 0: the naive
+                               steepest descent of eq. 1.7 (no transforms) */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
+
+/* ---- Algorithm 2: steepest descent with Fourier acceleration (eqs. 1.7-1.9) ----------
+ * One iteration: Delta(x) of eq. 1.3 at every site; each of its independent components is Fourier transformed over
+ * the d gauge-fixing directions (4-D for Landau; the 3-D transform of every time slice for Coulomb), multiplied by
+ * (alpha/2) p^2_max/p^2 with p^2 = sum_mu 4 sin^2(pi k_mu/n_mu) (0 at p = 0) and transformed back (normalised);
+ * g(x) = reunitarise(1 + w(x)) (first-order exponential; Gram-Schmidt as gf_reunitarize);
+ * U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all four mu.  Readings B1-B6 in DESIGN.md.  The transforms are cuFFT
+ * calls; cuFFT's own allocation is switched off, its work area lives in the caller's workspace.
+ *
+ * gf_fft_workspace_bytes: *bytes = size of the SECOND device workspace these calls need (the packed Delta/w fields,
+ *   4 complex numbers per site; the momentum table; cuFFT's work area).  Creates the cuFFT plans (needs a device).
+ * gf_fft_attach: hands that workspace over (caller-owned, 256-byte aligned, valid until gf_destroy).  Async.
+ * gf_fft_step: n iterations with step size alpha > 0 (the paper's value is 0.08).  The reunitarisation cadence of
+ *   gf_set_reunit_every counts iterations like sweeps.  Async.
+ * gf_fix_fft: Algorithm 2 with a measurement cadence: Delta, F, theta; while theta >= eps and iterations <
+ *   max_iters: min(check_every, remaining) iterations (each ends with the Delta/F/theta pass that feeds the next),
+ *   read F, theta.  History as for gf_fix (gf_get_history).  Synchronises at every read.
+ * Errors: GF_EINVAL (null pointer, n < 0, alpha <= 0, no workspace attached), GF_ENOMEM, GF_ECUDA (CUDA or cuFFT
+ * failure, text via gf_last_error), GF_ENUMERIC. */
+int gf_fft_workspace_bytes(gf_ctx* ctx, size_t* bytes);
+int gf_fft_attach(gf_ctx* ctx, void* dev_workspace, size_t workspace_bytes);
+int gf_fft_step(gf_ctx* ctx, int n, double alpha);
+int gf_fix_fft(gf_ctx* ctx, double alpha, double eps, int max_iters, int check_every, int* iters_done);
 
 /* Number of kernels this context has launched since gf_create (for benchmark bookkeeping). */
 long long gf_kernel_launches(const gf_ctx* ctx);

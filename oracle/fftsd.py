@@ -138,16 +138,25 @@ def step(U, dims, gauge, alpha, storage=18, accelerate=True):
     apply_rotation(U, dims, g, storage)
 
 
-def fix(U, dims, gauge, alpha, eps, max_iters, check_every=1, storage=18, accelerate=True):
+def reunitarize_links(U, dims):
+    """Project every link back onto SU(3) (reading A12), in place."""
+    W = _view(U, dims)
+    W[...] = reunitarize_rows(W)
+
+
+def fix(U, dims, gauge, alpha, eps, max_iters, check_every=1, storage=18, accelerate=True, reunit_every=0):
     """Algorithm 2 with a measurement cadence: measure; while theta >= eps: `check_every` iterations; measure.
+    After iteration s the links are reunitarised if reunit_every > 0 and s % reunit_every == 0.
     Returns (iterations_done, history[(iteration, F, theta), ...])."""
     done = 0
     F, th = measure(U, dims, gauge)
     hist = [(0, F, th)]
     while not (th < eps) and done < max_iters:
         n = min(check_every, max_iters - done)
-        for _ in range(n):
+        for i in range(n):
             step(U, dims, gauge, alpha, storage, accelerate)
+            if reunit_every > 0 and (done + i + 1) % reunit_every == 0:
+                reunitarize_links(U, dims)
         done += n
         F, th = measure(U, dims, gauge)
         hist.append((done, F, th))

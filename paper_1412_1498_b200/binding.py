@@ -15,11 +15,12 @@ from . import build as _build
 GF_LANDAU, GF_COULOMB = 0, 1
 GF_FP64, GF_FP32 = 0, 1
 GF_OK, GF_EINVAL, GF_EODD, GF_EUNSUPPORTED, GF_ENOMEM, GF_ECUDA, GF_ENUMERIC = 0, -1, -2, -3, -4, -5, -6
-GF_OPT_SWEEP_VARIANT, GF_OPT_BLOCK_THREADS, GF_OPT_FUSE_MEASURE = 1, 2, 3
+GF_OPT_SWEEP_VARIANT, GF_OPT_BLOCK_THREADS, GF_OPT_FUSE_MEASURE, GF_OPT_FFT_ACCELERATE = 1, 2, 3, 4
 
 SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "gf_set_links_host",
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
-           "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error"]
+           "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error",
+           "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft"]
 
 
 def _load() -> ctypes.CDLL:
@@ -45,6 +46,14 @@ def _load() -> ctypes.CDLL:
     lib.gf_set_reunit_every.argtypes = [c_void_p, c_int]
     lib.gf_set_option.restype = c_int
     lib.gf_set_option.argtypes = [c_void_p, c_int, c_int]
+    lib.gf_fft_workspace_bytes.restype = c_int
+    lib.gf_fft_workspace_bytes.argtypes = [c_void_p, POINTER(c_size_t)]
+    lib.gf_fft_attach.restype = c_int
+    lib.gf_fft_attach.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.gf_fft_step.restype = c_int
+    lib.gf_fft_step.argtypes = [c_void_p, c_int, c_double]
+    lib.gf_fix_fft.restype = c_int
+    lib.gf_fix_fft.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int)]
     lib.gf_kernel_launches.restype = c_longlong
     lib.gf_kernel_launches.argtypes = [c_void_p]
     lib.gf_destroy.restype = None
@@ -132,6 +141,28 @@ def gf_set_reunit_every(ctx, k: int) -> int:
 
 def gf_set_option(ctx, key: int, value: int) -> int:
     return lib.gf_set_option(ctx, key, value)
+
+
+def gf_fft_workspace_bytes(ctx):
+    """Returns (rc, bytes)."""
+    n = c_size_t()
+    rc = lib.gf_fft_workspace_bytes(ctx, byref(n))
+    return rc, int(n.value)
+
+
+def gf_fft_attach(ctx, dev_workspace: int, workspace_bytes: int) -> int:
+    return lib.gf_fft_attach(ctx, c_void_p(dev_workspace), workspace_bytes)
+
+
+def gf_fft_step(ctx, n: int, alpha: float) -> int:
+    return lib.gf_fft_step(ctx, n, alpha)
+
+
+def gf_fix_fft(ctx, alpha: float, eps: float, max_iters: int, check_every: int):
+    """Returns (rc, iterations_done)."""
+    done = c_int()
+    rc = lib.gf_fix_fft(ctx, alpha, eps, max_iters, check_every, byref(done))
+    return rc, done.value
 
 
 def gf_kernel_launches(ctx) -> int:
@@ -238,6 +269,26 @@ class GaugeFixer:
     def set_option(self, key, value):
         self._check(gf_set_option(self.ctx, int(key), int(value)))
 
+    def fft_attach(self):
+        """Allocate (torch) and hand over the second workspace Algorithm 2 needs.  Idempotent."""
+        if getattr(self, "fft_workspace", None) is not None:
+            return
+        rc, nbytes = gf_fft_workspace_bytes(self.ctx)
+        self._check(rc)
+        with self.torch.cuda.device(self.device):
+            self.fft_workspace = self.torch.empty(max(nbytes, 256), dtype=self.torch.uint8, device=self.device)
+        self._check(gf_fft_attach(self.ctx, self.fft_workspace.data_ptr(), nbytes))
+
+    def fft_step(self, n, alpha):
+        self.fft_attach()
+        self._check(gf_fft_step(self.ctx, int(n), float(alpha)))
+
+    def fix_fft(self, alpha, eps, max_iters, check_every=1):
+        self.fft_attach()
+        rc, done = gf_fix_fft(self.ctx, float(alpha), float(eps), int(max_iters), int(check_every))
+        self._check(rc)
+        return done
+
     def kernel_launches(self):
         return gf_kernel_launches(self.ctx)
 
@@ -246,6 +297,7 @@ class GaugeFixer:
             gf_destroy(self.ctx)
             self.ctx = None
             self.workspace = None
+            self.fft_workspace = None
 
     def __del__(self):
         try:

@@ -67,6 +67,12 @@ struct gf_ctx {
   long long launches;
   std::vector<double> history;
   long long history_n;
+  // Algorithm 2 (gf_fft_*): plans, and the caller's second workspace once attached
+  FftPlans* fft;
+  size_t fft_w_bytes, fft_table_bytes, fft_work_bytes;
+  char* fft_w;        // four packed complex fields of V entries
+  double* fft_table;  // 4 sin^2(pi k/n) per direction
+  int fft_accelerate; // GF_OPT_FFT_ACCELERATE
   char err[256];
 };
 
@@ -123,6 +129,8 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->fuse_measure = 1; c->qblocks = 0;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
+  c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1;
+  c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
   c->host_result = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
   cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocDefault);
@@ -141,6 +149,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
 void gf_destroy(gf_ctx* c) {
   if (!c) return;
   if (c->host_result) cudaFreeHost(c->host_result);
+  fft_plans_destroy(c->fft);
   for (int i = 0; i < 2; ++i)
     if (c->staging_free[i]) cudaEventDestroy(c->staging_free[i]);
   delete c;
@@ -234,6 +243,9 @@ int gf_set_option(gf_ctx* c, int key, int value) {
       c->fuse_measure = value != 0;
       if (!c->fuse_measure) c->qblocks = 0;
       return GF_OK;
+    case GF_OPT_FFT_ACCELERATE:
+      c->fft_accelerate = value != 0;
+      return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
       c->k.block_threads = value;
@@ -321,6 +333,137 @@ int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
   *n = (int)c->history_n;
   const long long m = c->history_n < cap ? c->history_n : cap;
   if (m > 0) memcpy(hist, c->history.data(), (size_t)m * 3 * sizeof(double));
+  return GF_OK;
+}
+
+// ---- Algorithm 2: steepest descent with Fourier acceleration -------------------------------------
+static int fft_plan(gf_ctx* c) {
+  if (c->fft) return GF_OK;
+  size_t work = 0;
+  const char* msg = fft_plans_create(&c->fft, c->k.geo, c->k.prec, c->k.gauge, c->k.stream, &work);
+  if (msg) return fail(c, GF_ECUDA, msg);
+  const size_t csize = c->k.prec == GF_FP64 ? 16 : 8;
+  c->fft_w_bytes = align_up((size_t)4 * volume(c) * csize);
+  c->fft_table_bytes = align_up(sd_table_entries(c->k.geo) * sizeof(double));
+  c->fft_work_bytes = align_up(work);
+  return GF_OK;
+}
+
+int gf_fft_workspace_bytes(gf_ctx* c, size_t* bytes) {
+  if (!c) return GF_EINVAL;
+  if (!bytes) return fail(c, GF_EINVAL, "gf_fft_workspace_bytes: null out-param");
+  int rc = fft_plan(c);
+  if (rc != GF_OK) return rc;
+  *bytes = c->fft_w_bytes + c->fft_table_bytes + c->fft_work_bytes;
+  return GF_OK;
+}
+
+int gf_fft_attach(gf_ctx* c, void* dev_workspace, size_t workspace_bytes) {
+  if (!c) return GF_EINVAL;
+  if (!dev_workspace) return fail(c, GF_EINVAL, "gf_fft_attach: null workspace");
+  int rc = fft_plan(c);
+  if (rc != GF_OK) return rc;
+  if (workspace_bytes < c->fft_w_bytes + c->fft_table_bytes + c->fft_work_bytes || ((uintptr_t)dev_workspace % ALIGN))
+    return fail(c, GF_ENOMEM, "gf_fft_attach: workspace too small or misaligned");
+  c->fft_w = (char*)dev_workspace;
+  c->fft_table = (double*)(c->fft_w + c->fft_w_bytes);
+  const char* msg = fft_plans_set_work(c->fft, c->fft_w + c->fft_w_bytes + c->fft_table_bytes);
+  if (msg) { c->fft_w = nullptr; return fail(c, GF_ECUDA, msg); }
+  cudaError_t e = launch_sd_table(c->k, c->fft_table);
+  if (e != cudaSuccess) { c->fft_w = nullptr; return fail_cuda(c, e, "gf_fft_attach"); }
+  c->launches += 1;
+  return GF_OK;
+}
+
+// Alg. 2 l.3-16 given Delta(x) already in fft_w: transform, factor, transform back, rotate the links.
+static int fft_update(gf_ctx* c, double alpha) {
+  int n = 0;
+  const char* msg = nullptr;
+  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, true, &n);
+  if (msg) return fail(c, GF_ECUDA, msg);
+  cudaError_t e = launch_sd_filter(c->k, c->fft_w, c->fft_table, alpha, c->fft_accelerate != 0);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (factor)");
+  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, false, &n);
+  if (msg) return fail(c, GF_ECUDA, msg);
+  e = launch_sd_rotate(c->k, c->fft_w);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (rotate)");
+  c->launches += n + 2;
+  c->qblocks = 0;
+  c->sweeps_total += 1;
+  if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) return gf_reunitarize(c);
+  return GF_OK;
+}
+
+static int fft_delta(gf_ctx* c) {
+  cudaError_t e = launch_sd_delta(c->k, c->fft_w);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (Delta)");
+  c->launches += 1;
+  return GF_OK;
+}
+
+// F, theta from the partials of the last fft_delta; synchronises
+static int fft_read_result(gf_ctx* c, double* F, double* theta) {
+  cudaError_t e = launch_sd_final(c->k);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(c->host_result, c->k.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->k.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_fix_fft (F, theta)");
+  c->launches += 1;
+  *F = c->host_result[0];
+  *theta = c->host_result[1];
+  if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_fix_fft: non-finite F or theta");
+  return GF_OK;
+}
+
+int gf_fft_step(gf_ctx* c, int n, double alpha) {
+  if (!c) return GF_EINVAL;
+  if (n < 0) return fail(c, GF_EINVAL, "gf_fft_step: n < 0");
+  if (!(alpha > 0.0) || !std::isfinite(alpha)) return fail(c, GF_EINVAL, "gf_fft_step: alpha must be positive");
+  if (!c->fft_w) return fail(c, GF_EINVAL, "gf_fft_step: no workspace attached (gf_fft_attach)");
+  for (int i = 0; i < n; ++i) {
+    int rc = fft_delta(c);
+    if (rc == GF_OK) rc = fft_update(c, alpha);
+    if (rc != GF_OK) return rc;
+  }
+  return GF_OK;
+}
+
+int gf_fix_fft(gf_ctx* c, double alpha, double eps, int max_iters, int check_every, int* iters_done) {
+  if (!c) return GF_EINVAL;
+  if (!iters_done) return fail(c, GF_EINVAL, "gf_fix_fft: null iters_done");
+  if (check_every < 1 || max_iters < 0 || !(eps >= 0.0))
+    return fail(c, GF_EINVAL, "gf_fix_fft: need check_every >= 1, max_iters >= 0, eps >= 0");
+  if (!(alpha > 0.0) || !std::isfinite(alpha)) return fail(c, GF_EINVAL, "gf_fix_fft: alpha must be positive");
+  if (!c->fft_w) return fail(c, GF_EINVAL, "gf_fix_fft: no workspace attached (gf_fft_attach)");
+  c->history.clear();
+  c->history_n = 0;
+  *iters_done = 0;
+  int done = 0;
+  double F, th;
+  // Alg. 2 l.1: Delta(x), F and theta in one pass; the same Delta(x) feeds the first iteration
+  int rc = fft_delta(c);
+  if (rc == GF_OK) rc = fft_read_result(c, &F, &th);
+  if (rc != GF_OK) return rc;
+  auto record = [&]() {
+    c->history.push_back((double)done);
+    c->history.push_back(F);
+    c->history.push_back(th);
+    c->history_n += 1;
+  };
+  record();
+  while (!(th < eps) && done < max_iters) {  // l.2
+    const int n = check_every < max_iters - done ? check_every : max_iters - done;
+    for (int i = 0; i < n; ++i) {
+      rc = fft_update(c, alpha);              // l.3-16
+      if (rc == GF_OK) rc = fft_delta(c);     // l.17 (its F, theta are read back only at the cadence)
+      if (rc != GF_OK) return rc;
+    }
+    done += n;
+    *iters_done = done;
+    rc = fft_read_result(c, &F, &th);
+    if (rc != GF_OK) return rc;
+    record();
+  }
   return GF_OK;
 }
 

@@ -35,4 +35,21 @@ cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);
 int measure_num_partials(const Geo& g);
 
+// ---- Algorithm 2 (gf_fftsd.cu): steepest descent with Fourier acceleration ------------------------------------------------
+struct FftPlans;  // the cuFFT plans of one context
+// Plans are created with cuFFT's own allocation switched off; *work = bytes of work area they need.  These return
+// nullptr on success or a static error text.
+const char* fft_plans_create(FftPlans** out, const Geo& g, int prec, int gauge, cudaStream_t stream, size_t* work);
+const char* fft_plans_set_work(FftPlans* p, void* work);
+void fft_plans_destroy(FftPlans* p);
+// in-place forward / backward (unnormalised) transform of the four packed fields at w; *launches += cuFFT executions
+const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward, int* launches);
+size_t sd_table_entries(const Geo& g);  // doubles in the 4 sin^2(pi k/n) table
+int sd_num_partials(const Geo& g);      // <= measure_num_partials(g): a.partials is shared
+cudaError_t launch_sd_table(const KernelArgs& a, double* table);
+cudaError_t launch_sd_delta(const KernelArgs& a, void* w);  // packed Delta(x) -> w, F/theta block partials -> a.partials
+cudaError_t launch_sd_final(const KernelArgs& a);           // a.partials -> a.result (F, theta)
+cudaError_t launch_sd_filter(const KernelArgs& a, void* w, const double* table, double alpha, bool accelerate);
+cudaError_t launch_sd_rotate(const KernelArgs& a, const void* w);
+
 }  // namespace gf

@@ -1,0 +1,128 @@
+"""GPU parity of Algorithm 2 (steepest descent with Fourier acceleration) against the numpy
+oracle oracle/fftsd.py, through the C ABI (gf_fft_step, gf_fix_fft).  Bars as for Algorithm 1 (north_star): links after
+one iteration within 1e-12 (FP64) / 2e-5 (FP32, against the FP64 oracle on the rounded input, reading A18); F relative
+1e-10 / 1e-5, theta within x1.5, iterations to convergence within +-2 %."""
+import numpy as np
+import pytest
+
+import gf_inputs as gi
+import oracle
+from oracle import fftsd
+
+pytestmark = pytest.mark.gpu
+TOL_LINK = {"f64": 1e-12, "f32": 2e-5}
+TOL_F = {"f64": 1e-10, "f32": 1e-5}
+
+
+def make(dims, r, seed, prec, storage):
+    U = gi.make_links(dims, r, seed, dtype=np.float32 if prec == "f32" else np.float64)
+    Uo = np.ascontiguousarray(U.astype(np.float64))
+    if storage == 12:
+        oracle.project12(Uo, dims)
+    return U, Uo
+
+
+def fixer(dims, gauge, prec, storage, U):
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=storage)
+    fx.set_links(torch.from_numpy(U).cuda())
+    return fx, gf
+
+
+# several tiles of 128 sites plus a ragged tail; extents that differ per direction; the smallest lattice
+LATTICES = [(6, 6, 6, 10), (4, 6, 8, 10), (8, 8, 8, 8), (2, 2, 2, 2), (16, 4, 6, 2)]
+
+
+@pytest.mark.parametrize("dims", LATTICES)
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_iterations_elementwise(dims, gauge, prec, storage):
+    U, Uo = make(dims, 0.5, 31, prec, storage)
+    fx, _ = fixer(dims, gauge, prec, storage, U)
+    for it in range(1, 4):
+        fx.fft_step(1, 0.08)
+        fftsd.step(Uo, dims, gauge, 0.08, storage=storage)
+        got = fx.get_links().cpu().numpy().astype(np.float64)
+        assert np.abs(got - Uo).max() <= TOL_LINK[prec] * it, it
+    F, th = fx.measure()
+    Fo, tho = fftsd.measure(Uo, dims, gauge)
+    assert abs(F - Fo) <= TOL_F[prec] * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
+    fx.close()
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_plain_steepest_descent_option(gauge):
+    dims = (6, 4, 6, 8)
+    U, Uo = make(dims, 0.5, 32, "f64", 18)
+    fx, gf = fixer(dims, gauge, "f64", 18, U)
+    fx.set_option(gf.GF_OPT_FFT_ACCELERATE, 0)
+    fx.fft_step(2, 0.08)
+    for _ in range(2):
+        fftsd.step(Uo, dims, gauge, 0.08, accelerate=False)
+    assert np.abs(fx.get_links().cpu().numpy() - Uo).max() <= 1e-12
+    fx.close()
+
+
+def compare(hist, ohist, tolF, eps):
+    assert len(hist) == len(ohist)
+    for (s, F, th), (so, Fo, tho) in zip(hist, ohist):
+        assert s == so
+        assert abs(F - Fo) <= tolF * abs(Fo), (s, F, Fo)
+        if tho > 1e-3 * max(eps, 1e-20) and tho > 1e-22:
+            assert tho / 1.5 <= th <= tho * 1.5, (s, th, tho)
+
+
+@pytest.mark.parametrize("dims,gauge,prec,storage,eps,reunit", [
+    ((8, 8, 8, 8), "landau", "f64", 18, 1e-12, 0),
+    ((8, 8, 8, 4), "coulomb", "f64", 12, 1e-12, 0),
+    ((8, 8, 8, 8), "landau", "f32", 12, 1e-7, 20),
+])
+def test_fix_fft_trajectory(dims, gauge, prec, storage, eps, reunit):
+    U, Uo = make(dims, 0.4, 33, prec, storage)
+    fx, _ = fixer(dims, gauge, prec, storage, U)
+    fx.set_reunit_every(reunit)
+    done = fx.fix_fft(0.08, eps, 600, 5)
+    hist = fx.history()
+    odone, ohist = fftsd.fix(Uo, dims, gauge, 0.08, eps, 600, 5, storage=storage, reunit_every=reunit)
+    assert abs(done - odone) <= 0.02 * odone + (5 if prec == "f32" else 0)
+    if done == odone:
+        compare(hist, ohist, TOL_F[prec], eps)
+    assert hist[-1][2] < eps and ohist[-1][2] < eps
+    assert abs(hist[-1][1] - ohist[-1][1]) <= TOL_F[prec] * abs(ohist[-1][1])
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    a, b = oracle.unitarity(np.ascontiguousarray(got), dims)
+    assert max(a, b) <= (1e-12 if prec == "f64" else 1e-5)
+    fx.close()
+
+
+def test_fix_fft_every_iteration_and_initial_values():
+    dims = (4, 4, 4, 8)
+    U, Uo = make(dims, 0.3, 34, "f64", 18)
+    fx, _ = fixer(dims, "landau", "f64", 18, U)
+    F0, th0 = fftsd.measure(Uo, dims, "landau")
+    done = fx.fix_fft(0.08, 0.0, 7, 1)
+    hist = fx.history()
+    assert done == 7 and [h[0] for h in hist] == list(range(8))
+    assert abs(hist[0][1] - F0) <= 1e-13 and abs(hist[0][2] - th0) <= 1e-12 * th0
+    _, ohist = fftsd.fix(Uo, dims, "landau", 0.08, 0.0, 7, 1)
+    compare(hist, ohist, 1e-12, 0.0)
+    fx.close()
+
+
+def test_errors():
+    import paper_1412_1498_b200 as gf
+
+    dims = (4, 4, 4, 4)
+    U, _ = make(dims, 0.3, 35, "f64", 18)
+    fx, _ = fixer(dims, "landau", "f64", 18, U)
+    assert gf.gf_fft_step(fx.ctx, 1, 0.08) == gf.GF_EINVAL  # nothing attached yet
+    fx.fft_attach()
+    assert gf.gf_fft_step(fx.ctx, -1, 0.08) == gf.GF_EINVAL
+    assert gf.gf_fft_step(fx.ctx, 1, 0.0) == gf.GF_EINVAL
+    assert gf.gf_fix_fft(fx.ctx, 0.08, 1e-10, 10, 0)[0] == gf.GF_EINVAL
+    assert gf.gf_fft_attach(fx.ctx, fx.fft_workspace.data_ptr(), 16) == gf.GF_ENOMEM
+    assert gf.gf_fft_step(fx.ctx, 0, 0.08) == gf.GF_OK
+    fx.close()
