@@ -1,5 +1,5 @@
-"""GPU parity over whole Algorithm 1 runs: gf_fix on BASELINE.json configs 0 and 1 against the stored
-oracle trajectories (tests/golden/*_trajectory.json, written by tests/golden/make_golden.py from oracle/ only), and on a
+"""GPU parity over whole Algorithm 1 runs: gf_fix on all five BASELINE.json configs at full size against
+the stored oracle trajectories (tests/golden/*_trajectory.json, written by tests/golden/make_golden.py from oracle/ only), and on a
 small lattice against the oracle run live.  Bars (north_star): F relative 1e-10 (FP64) / 1e-5 (FP32), theta within a
 factor 1.5, sweeps-to-convergence within +-2 %."""
 import json
@@ -24,7 +24,10 @@ def run_gpu(cfg, dims=None):
     dt = np.float32 if cfg["prec"] == "f32" else np.float64
     U = gi.make_links(dims, cfg["roughness"], cfg["seed"], dtype=dt)
     fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=cfg["prec"], storage=cfg["storage"])
-    fx.set_links(torch.from_numpy(U).cuda())
+    dev = torch.from_numpy(U).cuda()
+    fx.set_links(dev)
+    torch.cuda.synchronize()
+    del dev
     fx.set_reunit_every(cfg["reunit_every"])
     done = fx.fix(cfg["omega"], cfg["eps"], cfg["max_sweeps"], cfg["check_every"])
     hist = fx.history()
@@ -33,34 +36,44 @@ def run_gpu(cfg, dims=None):
     return done, hist, links, U
 
 
-def compare_histories(hist, gold, tolF, converged):
+def compare_histories(hist, gold, tolF, converged, floor=1e-9):
     """hist, gold: [(sweep, F, theta)].  F at every common checkpoint, theta within x1.5 wherever it is above the
     rounding floor, and the final values."""
     n = min(len(hist), len(gold))
     for (s, F, th), (so, Fo, tho) in zip(hist[:n], gold[:n]):
         assert s == so
         assert abs(F - Fo) <= tolF * abs(Fo), (s, F, Fo)
-        if tho > 1e-9 or not converged:
+        if tho > floor or not converged:
             assert tho / 1.5 <= th <= tho * 1.5, (s, th, tho)
 
 
-@pytest.mark.parametrize("name", ["cfg0", "cfg1"])
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
 def test_fix_matches_stored_oracle_trajectory(name):
+    """The whole contract run of every BASELINE.json config, full size, against the oracle's stored (sweep, F, theta)
+    history.  The input comes from the HOST build of the generator, the one the golden script fed the oracle."""
     cfg = next(c for c in gi.CONFIGS if c["name"] == name)
-    gold = json.load(open(os.path.join(HERE, "golden", f"{name}_trajectory.json")))
+    path = os.path.join(HERE, "golden", f"{name}_trajectory.json")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not written yet (tests/golden/make_golden.py {name})")
+    gold = json.load(open(path))
     ghist = [(int(s), float(F), float(th)) for s, F, th in gold["history"]]
-    done, hist, links, _ = run_gpu(cfg)
+    f64 = cfg["prec"] == "f64"
+    tolF = 1e-10 if f64 else 1e-5
+    done, hist, links, U = run_gpu(cfg)
+    del U
     converged = ghist[-1][2] < cfg["eps"]
     assert abs(done - gold["sweeps_done"]) <= 0.02 * gold["sweeps_done"]
-    compare_histories(hist, ghist, 1e-10, converged)
+    compare_histories(hist, ghist, tolF, converged, 1e-9 if f64 else 1e-6)
     Ff, thf = hist[-1][1], hist[-1][2]
-    assert abs(Ff - ghist[-1][1]) <= 1e-10 * abs(ghist[-1][1])
+    assert abs(Ff - ghist[-1][1]) <= tolF * abs(ghist[-1][1])
     if converged:
         assert thf < cfg["eps"]
     else:
         assert ghist[-1][2] / 1.5 <= thf <= ghist[-1][2] * 1.5
-    a, b = oracle.unitarity(np.ascontiguousarray(links.astype(np.float64)), cfg["dims"])
-    assert max(a, b) <= 1e-12  # still SU(3) after hundreds / thousands of sweeps without reunitarisation
+    a, b = oracle.unitarity(np.ascontiguousarray(links, dtype=np.float64), cfg["dims"])
+    # still SU(3) after hundreds / thousands of sweeps (FP64: without any reunitarisation; FP32: up to 49 sweeps
+    # since the last one: ~100 roundings of 6e-8 per element, maximum over 75 M elements)
+    assert max(a, b) <= (1e-12 if f64 else 1e-4)
 
 
 @pytest.mark.parametrize("name,dims", [("cfg2", (8, 8, 8, 8)), ("cfg3", (6, 6, 6, 12)), ("cfg4", (8, 8, 8, 16)),
