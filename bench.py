@@ -362,6 +362,63 @@ def run_ours(args):
     return 0
 
 
+def run_fftsd(args):
+    """--algo fftsd: Algorithm 2 (steepest descent with Fourier acceleration) on the same workload.
+    A step = `check_every` iterations (Delta+F/theta pass, cuFFT forward, factor, cuFFT backward, rotation) + one read
+    of F/theta.  Secondary line: metric fftsd_site_iterations_per_s, not the headline."""
+    import torch
+
+    import gf_inputs as gi
+    import paper_1412_1498_b200 as gf
+
+    cfg = get_cfg(args.config)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    V = gi.volume(dims)
+    L = LINK_BYTES[(prec, storage)]
+    n_it = cfg["check_every"]
+    fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage)
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], prec,
+                         torch.cuda.current_stream().cuda_stream)
+    fx.set_links(canon)
+    del canon
+    fx.fft_attach()
+    torch.cuda.synchronize()
+    for _ in range(args.warmup):
+        fx.fft_step(n_it, 0.08)
+        fx.measure()
+    torch.cuda.synchronize()
+    l0 = fx.kernel_launches()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        fx.fft_step(n_it, 0.08)
+        F, th = fx.measure()
+    t1.record()
+    torch.cuda.synchronize()
+    ms = t0.elapsed_time(t1)
+    peak, peak_src = load_peaks()
+    csize = 16 if prec == "f64" else 8
+    # algorithmic bytes per iteration: Delta pass reads 4VL, writes 4 fields; rotation reads+writes 4VL and reads the
+    # fields; each transform pass and the factor read+write the 4 fields (3-D: 1 pass, +1 for t in Landau gauge)
+    passes = 2 * (2 if cfg["gauge"] == "landau" else 1) + 1
+    bytes_it = 12 * V * L + 4 * V * csize * (2 + 2 * passes)
+    gbs = bytes_it * n_it * args.steps / (ms * 1e-3) / 1e9
+    line = {"metric": "fftsd_site_iterations_per_s", "value": V * n_it * args.steps / (ms * 1e-3),
+            "unit": "site-iterations/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": prec, "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "algorithm": "Algorithm 2, alpha=0.08",
+                       "step": f"{n_it} iterations + 1 F/theta measurement", "final_F": F, "final_theta": th},
+            "roofline": {"bound": "hbm", "kernel": "whole iteration (sd_delta, cuFFT x2, sd_filter, sd_rotate)",
+                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "peak_source": peak_src, "algorithmic_bytes_per_iteration": bytes_it},
+            "gpu_launches": int(fx.kernel_launches() - l0)}
+    fx.close()
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -374,9 +431,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.algo == "fftsd":
+        return run_fftsd(args)
     return run_ours(args)
 
 

@@ -54,6 +54,31 @@ __device__ __forceinline__ int lex_up(const Geo& g, const Site& s, int lex, int 
 // f = sum over the parity-0 sites of Re Tr [U_nu(x) + U_nu(x-nu)] (= every link once);  q = sum_ij |Delta_ij|^2.
 constexpr int SD_THREADS = 128;
 
+// Block order.  A site's t-neighbours are one time slice away in cb order (151 MB of links on 64^3 x 128: more than
+// L2), so in launch order the temporal links would come from HBM twice.  When a time slice is a whole number of
+// blocks, blocks are renumbered so that a chunk of 1/16 slice runs through all t before the next chunk starts: the
+// reuse distance in t drops to two chunks (a few MB) and the second use hits L2.
+struct BlockOrder {
+  int per_slice;  // blocks per time slice (0: identity order)
+  int chunk;      // blocks per chunk
+  int nt;
+};
+__device__ __forceinline__ int ordered_block(const BlockOrder& o, int b) {
+  if (o.per_slice == 0) return b;
+  const int span = o.nt * o.chunk;
+  const int c = b / span, r = b - c * span;
+  const int t = r / o.chunk, k = r - t * o.chunk;
+  return t * o.per_slice + c * o.chunk + k;
+}
+static BlockOrder make_block_order(const Geo& g) {
+  BlockOrder o{0, 0, g.n[3]};
+  const int slice_cb = g.vh / g.n[3];
+  if (slice_cb % SD_THREADS) return o;
+  o.per_slice = slice_cb / SD_THREADS;
+  o.chunk = o.per_slice % 16 == 0 ? o.per_slice / 16 : o.per_slice;
+  return o;
+}
+
 template <class T, int NELEM, int ND, class C>
 __device__ __forceinline__ void site_delta(const C* __restrict__ links, const Geo& g, int parity, int cb, C (&d)[4],
                                            T& tr, T& q) {
@@ -89,9 +114,11 @@ __device__ __forceinline__ void site_delta(const C* __restrict__ links, const Ge
 
 template <class T, int NELEM, int ND>
 __global__ void __launch_bounds__(SD_THREADS) sd_delta_kernel(const cplx_t<T>* __restrict__ links, Geo g,
-                                                              cplx_t<T>* __restrict__ w, double2* __restrict__ partials) {
+                                                              cplx_t<T>* __restrict__ w, double2* __restrict__ partials,
+                                                              BlockOrder order) {
   using C = cplx_t<T>;
-  const int cb = blockIdx.x * SD_THREADS + threadIdx.x;
+  const int blk = ordered_block(order, blockIdx.x);
+  const int cb = blk * SD_THREADS + threadIdx.x;
   double f = 0.0, q = 0.0;
   if (cb < g.vh) {
     const size_t V = 2 * (size_t)g.vh;
@@ -119,7 +146,7 @@ __global__ void __launch_bounds__(SD_THREADS) sd_delta_kernel(const cplx_t<T>* _
     double F = 0.0, Q = 0.0;
 #pragma unroll
     for (int i = 0; i < SD_THREADS / 32; ++i) { F += sf[i]; Q += sq[i]; }
-    partials[blockIdx.x] = make_double2(F, Q);
+    partials[blk] = make_double2(F, Q);
   }
 }
 
@@ -209,10 +236,11 @@ __device__ __forceinline__ void rotation_from_packed(const C* __restrict__ w, si
 // blocks_per_parity blocks take parity 0, the rest parity 1.
 template <class T, int NELEM>
 __global__ void __launch_bounds__(SD_THREADS) sd_rotate_kernel(cplx_t<T>* __restrict__ links, Geo g,
-                                                               const cplx_t<T>* __restrict__ w, int blocks_per_parity) {
+                                                               const cplx_t<T>* __restrict__ w, int blocks_per_parity,
+                                                               BlockOrder order) {
   using C = cplx_t<T>;
   const int parity = blockIdx.x >= blocks_per_parity;
-  const int cb = (blockIdx.x - parity * blocks_per_parity) * SD_THREADS + threadIdx.x;
+  const int cb = ordered_block(order, blockIdx.x - parity * blocks_per_parity) * SD_THREADS + threadIdx.x;
   if (cb >= g.vh) return;
   const size_t V = 2 * (size_t)g.vh;
   const Site s = site_of(g, parity, cb);
@@ -335,7 +363,7 @@ cudaError_t launch_sd_table(const KernelArgs& a, double* table) {
 template <class T, int NELEM, int ND>
 static cudaError_t sd_delta_T(const KernelArgs& a, void* w) {
   sd_delta_kernel<T, NELEM, ND><<<sd_num_partials(a.geo), SD_THREADS, 0, a.stream>>>(
-      (const cplx_t<T>*)a.links, a.geo, (cplx_t<T>*)w, (double2*)a.partials);
+      (const cplx_t<T>*)a.links, a.geo, (cplx_t<T>*)w, (double2*)a.partials, make_block_order(a.geo));
   return cudaGetLastError();
 }
 
@@ -384,7 +412,8 @@ cudaError_t launch_sd_filter(const KernelArgs& a, void* w, const double* table, 
 template <class T, int NELEM>
 static cudaError_t sd_rotate_T(const KernelArgs& a, const void* w) {
   const int bpp = sd_num_partials(a.geo);
-  sd_rotate_kernel<T, NELEM><<<2 * bpp, SD_THREADS, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, (const cplx_t<T>*)w, bpp);
+  sd_rotate_kernel<T, NELEM><<<2 * bpp, SD_THREADS, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, (const cplx_t<T>*)w, bpp,
+                                                                   make_block_order(a.geo));
   return cudaGetLastError();
 }
 

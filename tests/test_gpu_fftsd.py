@@ -33,7 +33,7 @@ def fixer(dims, gauge, prec, storage, U):
 
 
 # several tiles of 128 sites plus a ragged tail; extents that differ per direction; the smallest lattice
-LATTICES = [(6, 6, 6, 10), (4, 6, 8, 10), (8, 8, 8, 8), (2, 2, 2, 2), (16, 4, 6, 2)]
+LATTICES = [(6, 6, 6, 10), (4, 6, 8, 10), (8, 8, 8, 8), (2, 2, 2, 2), (16, 4, 6, 2), (16, 16, 16, 4), (32, 16, 16, 6)]
 
 
 @pytest.mark.parametrize("dims", LATTICES)
