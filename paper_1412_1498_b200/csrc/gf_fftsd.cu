@@ -79,39 +79,40 @@ static BlockOrder make_block_order(const Geo& g) {
   return o;
 }
 
-template <class T, int NELEM, int ND, class C>
-__device__ __forceinline__ void site_delta(const C* __restrict__ links, const Geo& g, int parity, int cb, C (&d)[4],
-                                           T& tr, T& q) {
-  const Site s = site_of(g, parity, cb);
-  const C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
-  C A[9];
-#pragma unroll
-  for (int e = 0; e < 9; ++e) A[e] = mk<T>(T(0), T(0));
-  tr = T(0);
-#pragma unroll
-  for (int nu = 0; nu < ND; ++nu) {
-    C u[9];
-    load_link<NELEM, true>(links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu), u);
-#pragma unroll
-    for (int e = 0; e < 9; ++e) { A[e].x += u[e].x; A[e].y += u[e].y; }
-    tr += u[0].x + u[4].x + u[8].x;
-    load_link<NELEM, true>(fwd + nu * NELEM * 32, u);
-#pragma unroll
-    for (int e = 0; e < 9; ++e) { A[e].x -= u[e].x; A[e].y -= u[e].y; }
+// The anti-Hermitian part of A is all Delta needs: 3 imaginary diagonal parts and 3 complex upper off-diagonals
+// (9 reals per site instead of the 18 of A), plus Re Tr for F.
+template <class T, class C>
+struct AntiHerm {
+  T d0, d1, d2, tr;
+  C o01, o02, o12;
+  __device__ __forceinline__ void clear() {
+    d0 = d1 = d2 = tr = T(0);
+    o01 = o02 = o12 = mk<T>(T(0), T(0));
+  }
+  // += sign * (u - u^dag) / (diagonal: Im u_ii; the factor 2 is applied at the end), tr += Re Tr u
+  template <int SIGN>
+  __device__ __forceinline__ void add(const C (&u)[9]) {
+    const T s = T(SIGN);
+    d0 += s * u[0].y; d1 += s * u[4].y; d2 += s * u[8].y;
+    o01.x += s * (u[1].x - u[3].x); o01.y += s * (u[1].y + u[3].y);
+    o02.x += s * (u[2].x - u[6].x); o02.y += s * (u[2].y + u[6].y);
+    o12.x += s * (u[5].x - u[7].x); o12.y += s * (u[5].y + u[7].y);
     tr += u[0].x + u[4].x + u[8].x;
   }
-  // D = A - A^dag: D_ii = 2i Im A_ii, D_ij = A_ij - conj(A_ji); traceless part
-  T d0 = T(2) * A[0].y, d1 = T(2) * A[4].y, d2 = T(2) * A[8].y;
-  const T m = (d0 + d1 + d2) / T(3);
-  d0 -= m; d1 -= m; d2 -= m;
-  d[0] = mk<T>(A[1].x - A[3].x, A[1].y + A[3].y);
-  d[1] = mk<T>(A[2].x - A[6].x, A[2].y + A[6].y);
-  d[2] = mk<T>(A[5].x - A[7].x, A[5].y + A[7].y);
-  d[3] = mk<T>(d0, d1);
-  q = d0 * d0 + d1 * d1 + d2 * d2 +
-      T(2) * (d[0].x * d[0].x + d[0].y * d[0].y + d[1].x * d[1].x + d[1].y * d[1].y + d[2].x * d[2].x + d[2].y * d[2].y);
-}
+  // packed Delta and sum_ij |Delta_ij|^2
+  __device__ __forceinline__ T finish(C (&d)[4]) const {
+    T a0 = T(2) * d0, a1 = T(2) * d1, a2 = T(2) * d2;
+    const T m = (a0 + a1 + a2) / T(3);
+    a0 -= m; a1 -= m; a2 -= m;
+    d[0] = o01; d[1] = o02; d[2] = o12; d[3] = mk<T>(a0, a1);
+    return a0 * a0 + a1 * a1 + a2 * a2 +
+           T(2) * (o01.x * o01.x + o01.y * o01.y + o02.x * o02.x + o02.y * o02.y + o12.x * o12.x + o12.y * o12.y);
+  }
+};
 
+// Both sites of a pair are advanced direction by direction, so that the two uses of a link (as U_nu(x) of one site
+// and as U_nu(x'-nu) of its neighbour x' = x+nu) fall at the same point of the program in neighbouring threads and
+// the second one finds the line in L2.
 template <class T, int NELEM, int ND>
 __global__ void __launch_bounds__(SD_THREADS) sd_delta_kernel(const cplx_t<T>* __restrict__ links, Geo g,
                                                               cplx_t<T>* __restrict__ w, double2* __restrict__ partials,
@@ -122,13 +123,28 @@ __global__ void __launch_bounds__(SD_THREADS) sd_delta_kernel(const cplx_t<T>* _
   double f = 0.0, q = 0.0;
   if (cb < g.vh) {
     const size_t V = 2 * (size_t)g.vh;
-    const Site s0 = site_of(g, 0, cb);
+    const Site s0 = site_of(g, 0, cb), s1 = site_of(g, 1, cb);
     const int first = s0.x & 1;  // parity-0 site sits at lex = 2 cb + first, the parity-1 site at the other one
+    const C* fwd0 = links + link_offset<NELEM>(g, 0, cb, 0);
+    const C* fwd1 = links + link_offset<NELEM>(g, 1, cb, 0);
+    AntiHerm<T, C> a0, a1;
+    a0.clear();
+    a1.clear();
+#pragma unroll
+    for (int nu = 0; nu < ND; ++nu) {
+      C u[9];
+      load_link<NELEM, true>(fwd0 + nu * NELEM * 32, u);
+      a0.template add<-1>(u);
+      load_link<NELEM, true>(fwd1 + nu * NELEM * 32, u);
+      a1.template add<-1>(u);
+      load_link<NELEM, true>(links + link_offset<NELEM>(g, 1, cb_down(g, s0, cb, nu), nu), u);
+      a0.template add<1>(u);
+      load_link<NELEM, true>(links + link_offset<NELEM>(g, 0, cb_down(g, s1, cb, nu), nu), u);
+      a1.template add<1>(u);
+    }
     C de[4], dodd[4];
-    T tr, q0, q1, tr1;
-    site_delta<T, NELEM, ND>(links, g, 0, cb, de, tr, q0);
-    site_delta<T, NELEM, ND>(links, g, 1, cb, dodd, tr1, q1);
-    f = (double)tr;
+    const T q0 = a0.finish(de), q1 = a1.finish(dodd);
+    f = (double)a0.tr;
     q = (double)q0 + (double)q1;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
