@@ -283,3 +283,39 @@ def test_fused_theta_terms_near_convergence(gf, torch):
         assert s == so and abs(F - Fo) <= 1e-10 * abs(Fo)
         assert tho / 1.5 <= th <= tho * 1.5 or max(th, tho) < 1e-25
     fx.close()
+
+
+def test_two_contexts_on_their_own_streams(gf, torch):
+    """Work is ordered on the stream handed to gf_create (include/gf.h): two contexts on two non-default streams,
+    launched interleaved, each reproduce the oracle; Algorithm 1 on one, Algorithm 2 on the other."""
+    from oracle import fftsd
+
+    dims = (8, 6, 4, 6)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    U1, O1 = host_input(dims, 0.4, 41, "f64", 18)
+    U2, O2 = host_input(dims, 0.5, 42, "f64", 12)
+    d1, d2 = torch.from_numpy(U1).cuda(), torch.from_numpy(U2).cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s1):
+        f1 = gf.GaugeFixer(dims, gauge="landau", prec="f64", storage=18, stream=s1)
+        f1.set_links(d1)
+    with torch.cuda.stream(s2):
+        f2 = gf.GaugeFixer(dims, gauge="coulomb", prec="f64", storage=12, stream=s2)
+        f2.set_links(d2)
+        f2.fft_attach()
+    for _ in range(3):
+        f1.ovr_sweep(1, 1.6)
+        f2.fft_step(1, 0.08)
+    with torch.cuda.stream(s1):
+        g1 = f1.get_links()
+    with torch.cuda.stream(s2):
+        g2 = f2.get_links()
+    s1.synchronize()
+    s2.synchronize()
+    oracle.sweeps(O1, dims, "landau", 1.6, n=3)
+    for _ in range(3):
+        fftsd.step(O2, dims, "coulomb", 0.08, storage=12)
+    assert np.abs(g1.cpu().numpy() - O1).max() <= 3e-12
+    assert np.abs(g2.cpu().numpy() - O2).max() <= 3e-12
+    f1.close()
+    f2.close()
