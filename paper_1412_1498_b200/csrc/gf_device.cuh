@@ -144,36 +144,44 @@ __device__ __forceinline__ void su2_overrelax(T r0, T r1, T r2, T r3, T omega, T
 }
 
 // One subgroup step on rows/cols (I,J): K <- gK, G <- gG with g = [[c+i q3, q2+i q1], [-q2+i q1, c-i q3]] embedded.
-template <int I, int J, bool UPDATE_K, class T, class C>
-__device__ __forceinline__ void su2_step(C (&K)[9], C (&G)[9], T omega) {
+// K (and g) are in precision T; G may be kept in a lower precision TG (g is rounded once per step).
+template <int I, int J, bool UPDATE_K, class T, class C, class CG>
+__device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega) {
+  using TG = decltype(G[0].x);
   const T r0 = K[I * 3 + I].x + K[J * 3 + J].x;
   const T r1 = -(K[I * 3 + J].y + K[J * 3 + I].y);
   const T r2 = K[J * 3 + I].x - K[I * 3 + J].x;
   const T r3 = -(K[I * 3 + I].y - K[J * 3 + J].y);
   T c, q1, q2, q3;
   su2_overrelax(r0, r1, r2, r3, omega, c, q1, q2, q3);
-  const C g00 = mk<T>(c, q3), g01 = mk<T>(q2, q1), g10 = mk<T>(-q2, q1), g11 = mk<T>(c, -q3);
+  if (UPDATE_K) {
+    const C g00 = mk<T>(c, q3), g01 = mk<T>(q2, q1), g10 = mk<T>(-q2, q1), g11 = mk<T>(c, -q3);
 #pragma unroll
-  for (int col = 0; col < 3; ++col) {
-    if (UPDATE_K) {
+    for (int col = 0; col < 3; ++col) {
       const C ki = K[I * 3 + col], kj = K[J * 3 + col];
       C a = cmul(g00, ki); cfma(a, g01, kj);
       C b = cmul(g10, ki); cfma(b, g11, kj);
       K[I * 3 + col] = a; K[J * 3 + col] = b;
     }
-    const C gi = G[I * 3 + col], gj = G[J * 3 + col];
-    C a = cmul(g00, gi); cfma(a, g01, gj);
-    C b = cmul(g10, gi); cfma(b, g11, gj);
+  }
+  const TG cg = (TG)c, p1 = (TG)q1, p2 = (TG)q2, p3 = (TG)q3;
+  const CG h00 = mk<TG>(cg, p3), h01 = mk<TG>(p2, p1), h10 = mk<TG>(-p2, p1), h11 = mk<TG>(cg, -p3);
+#pragma unroll
+  for (int col = 0; col < 3; ++col) {
+    const CG gi = G[I * 3 + col], gj = G[J * 3 + col];
+    CG a = cmul(h00, gi); cfma(a, h01, gj);
+    CG b = cmul(h10, gi); cfma(b, h11, gj);
     G[I * 3 + col] = a; G[J * 3 + col] = b;
   }
 }
 
 // G = g3 g2 g1 for one site from its K (Algorithm 1 l.5-6; subgroup order (0,1),(1,2),(0,2), reading A4; A8)
 // FINAL_K: also carry K through the last step, so that on return K = G K_in (= K(x) of the updated links).
-template <class T, bool FINAL_K = false, class C>
-__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], C (&G)[9], T omega) {
+template <class T, bool FINAL_K = false, class C, class CG>
+__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], CG (&G)[9], T omega) {
+  using TG = decltype(G[0].x);
 #pragma unroll
-  for (int e = 0; e < 9; ++e) G[e] = mk<T>((e % 4 == 0) ? T(1) : T(0), T(0));
+  for (int e = 0; e < 9; ++e) G[e] = mk<TG>((e % 4 == 0) ? TG(1) : TG(0), TG(0));
   su2_step<0, 1, true>(K, G, omega);
   su2_step<1, 2, true>(K, G, omega);
   su2_step<0, 2, FINAL_K>(K, G, omega);

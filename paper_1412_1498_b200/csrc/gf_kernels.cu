@@ -128,6 +128,32 @@ __device__ __forceinline__ T delta_norm2(const C (&A)[9]) {
 //  "staged" (the default): every thread copies its eight links global -> shared with cp.async (LDGSTS; no registers
 //      tied up, all 8*L bytes of the site in flight at once), waits for its own copies, then works out of shared
 //      memory in a single pass: each link crosses L2 -> SM once.  Shared slots are thread-private: no barrier.
+// Precision of K(x), the three SU(2) steps and G(x) in BOTH storage precisions.  In FP32 the direction r/|r| of a
+// subgroup step is ill-conditioned wherever |r| << |K| (cancellation in the sum of eight links): with FP32 arithmetic
+// 63 of the 1,048,576 sites of config 2 miss the 2e-5 one-sweep bound against the FP64 oracle (max 1.4e-4; the
+// oracle's own float instantiation does the same).  The links are FP32 inputs, so their sum in FP64 is exact, and
+// each g is rounded to FP32 once; G = g3 g2 g1, loads, stores and the eight 3x3 products stay in the storage precision.
+using RotationType = double;
+
+// Accumulator of K(x) in RotationType: every real of the 2*ND links is converted and added in FP64 (exact for FP32
+// inputs).  Measured alternative for FP32 storage (config 2, ncu): carrying the sum as an unevaluated FP32 pair with
+// TwoSum and converting once (36 conversions per site instead of 144) takes the XU pipe from 31 % to 11 % busy but
+// lengthens the dependent chain: 86.8 us per half-sweep against 74.8 us for the plain conversions kept here
+// (all-FP32 arithmetic, which misses the parity bound: 64.6 us).
+template <class T>
+struct KSum {
+  double2 k[9];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int e = 0; e < 9; ++e) k[e] = make_double2(0.0, 0.0);
+  }
+  __device__ __forceinline__ void add(int e, T x, T y) { k[e].x += (double)x; k[e].y += (double)y; }
+  __device__ __forceinline__ void finish(double2 (&K)[9]) const {
+#pragma unroll
+    for (int e = 0; e < 9; ++e) K[e] = k[e];
+  }
+};
+
 template <class T, int NELEM, class C>
 __device__ __forceinline__ void site_pointers(C* __restrict__ links, const Geo& g, int parity, int cb, C*& fwd,
                                               C* (&bwd)[4]) {
@@ -145,6 +171,8 @@ template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool PREFETCH>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) {
   using C = cplx_t<T>;
+  using TK = RotationType;  // K(x), the SU(2) steps and G(x) are always FP64 (see RotationType)
+  using CK = cplx_t<TK>;
   int cb = blockIdx.x * THREADS + threadIdx.x;
   const bool live = cb < g.vh;
   if (!PREFETCH && !live) return;
@@ -168,24 +196,25 @@ ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) 
     if (!live) return;
   }
 
-  C K[9];
-#pragma unroll
-  for (int e = 0; e < 9; ++e) K[e] = mk<T>(T(0), T(0));
+  KSum<T> ks;
+  ks.clear();
 #pragma unroll
   for (int mu = 0; mu < ND; ++mu) {
     C u[9];
     load_link<NELEM, true>(fwd + mu * NELEM * 32, u);
 #pragma unroll
-    for (int e = 0; e < 9; ++e) { K[e].x += u[e].x; K[e].y += u[e].y; }
+    for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
     load_link<NELEM, true>(bwd[mu], u);
 #pragma unroll
     for (int i = 0; i < 3; ++i)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) { K[i * 3 + j].x += u[j * 3 + i].x; K[i * 3 + j].y -= u[j * 3 + i].y; }
+      for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
   }
+  CK K[9];
+  ks.finish(K);
 
   C G[9];
-  site_gauge_rotation<T>(K, G, omega);
+  site_gauge_rotation<TK>(K, G, (TK)omega);
 
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
@@ -201,6 +230,8 @@ ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) 
 
 // ---- staged through shared memory with cp.async ---------------------------------------------------------
 template <class T> constexpr int staged_threads() { return sizeof(T) == 8 ? 64 : 128; }
+// FP32 storage: 4 blocks of 128 threads per SM (shared memory allows 4), i.e. at most 128 registers for the FP64 rotation
+template <class T> constexpr int staged_minblocks() { return sizeof(T) == 8 ? 1 : 4; }
 
 template <int BYTES>
 __device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
@@ -229,6 +260,8 @@ template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
   using C = cplx_t<T>;
+  using TK = RotationType;
+  using CK = cplx_t<TK>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C* sm = reinterpret_cast<C*>(smem_raw) + threadIdx.x;
   const int cb = blockIdx.x * THREADS + threadIdx.x;
@@ -251,27 +284,28 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     }
     cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
 
-    C K[9];
-#pragma unroll
-    for (int e = 0; e < 9; ++e) K[e] = mk<T>(T(0), T(0));
+    KSum<T> ks;
+    ks.clear();
 #pragma unroll
     for (int mu = 0; mu < ND; ++mu) {
       C u[9];
       load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
 #pragma unroll
-      for (int e = 0; e < 9; ++e) { K[e].x += u[e].x; K[e].y += u[e].y; }
+      for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
       sched_fence();
       load_link_smem<NELEM, THREADS, true>(sm, 2 * mu + 1, u);
 #pragma unroll
       for (int i = 0; i < 3; ++i)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) { K[i * 3 + j].x += u[j * 3 + i].x; K[i * 3 + j].y -= u[j * 3 + i].y; }
+        for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
       sched_fence();
     }
+    CK K[9];
+    ks.finish(K);
 
     C G[9];
-    site_gauge_rotation<T, MEASURE>(K, G, omega);
-    if (MEASURE) q = (double)delta_norm2<T>(K);
+    site_gauge_rotation<TK, MEASURE>(K, G, (TK)omega);
+    if (MEASURE) q = (double)delta_norm2<TK>(K);
 
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
@@ -297,7 +331,7 @@ template <class T, int NELEM, int ND, int THREADS, bool MEASURE>
 static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
-  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, 1, MEASURE>;
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE>;
   static bool attr_set = false;  // per instantiation
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
