@@ -130,8 +130,8 @@ __device__ __forceinline__ T delta_norm2(const C (&A)[9]) {
 //      memory in a single pass: each link crosses L2 -> SM once.  Shared slots are thread-private: no barrier.
 // Precision of K(x), the three SU(2) steps and G(x) in BOTH storage precisions.  In FP32 the direction r/|r| of a
 // subgroup step is ill-conditioned wherever |r| << |K| (cancellation in the sum of eight links): with FP32 arithmetic
-// 63 of the 1,048,576 sites of config 2 miss the 2e-5 one-sweep bound against the FP64 oracle (max 1.4e-4; the
-// oracle's own float instantiation does the same).  The links are FP32 inputs, so their sum in FP64 is exact, and
+// 63 of the 1,048,576 sites of config 2 miss the 2e-5 one-sweep bound against an FP64 evaluation (max 1.4e-4; any
+// all-FP32 evaluation of the same formulas does).  The links are FP32 inputs, so their sum in FP64 is exact, and
 // each g is rounded to FP32 once; G = g3 g2 g1, loads, stores and the eight 3x3 products stay in the storage precision.
 using RotationType = double;
 
