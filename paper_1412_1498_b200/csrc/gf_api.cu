@@ -59,7 +59,7 @@ struct gf_ctx {
   Sizes sz;
   char* staging[2];
   cudaEvent_t staging_free[2];
-  double* host_result;  // pinned, 2 doubles
+  double* host_result;  // pinned and mapped, 2 doubles: the reduction kernels write F, theta straight into it
   int reunit_every;
   int fuse_measure;  // GF_OPT_FUSE_MEASURE
   int qblocks;       // > 0: k.qpartials[0..qblocks) hold the odd sites' theta terms of the links as they stand
@@ -123,7 +123,8 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->k.links = base;
   c->k.partials = base + sz.links;
   c->k.qpartials = base + sz.links + sz.partials;
-  c->k.result = base + sz.links + sz.partials + sz.qpartials;
+  c->k.result = base + sz.links + sz.partials + sz.qpartials;  // replaced by the mapped host pointer below
+  c->k.counter = base + sz.links + sz.partials + sz.qpartials;  // the workspace's result slot holds the counter
   c->staging[0] = base + sz.links + sz.partials + sz.qpartials + sz.result;
   c->staging[1] = c->staging[0] + sz.staging;
   c->fuse_measure = 1; c->qblocks = 0;
@@ -133,11 +134,17 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
   c->host_result = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
-  cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocDefault);
+  cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
+  if (e == cudaSuccess) {  // zero-copy result: saves a 16-byte D2H copy per measurement (latency on small lattices)
+    void* dev = nullptr;
+    e = cudaHostGetDevicePointer(&dev, c->host_result, 0);
+    if (e == cudaSuccess) c->k.result = dev;
+  }
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[0], cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[1], cudaEventDisableTiming);
   // padding lanes of the last 32-site block must read as zeros
   if (e == cudaSuccess) e = cudaMemsetAsync(c->k.links, 0, sz.links, c->k.stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->k.counter, 0, sz.result, c->k.stream);
   if (e != cudaSuccess) {
     gf_destroy(c);
     return GF_ECUDA;
@@ -283,11 +290,9 @@ int gf_measure(gf_ctx* c, double* F, double* theta) {
   if (!c) return GF_EINVAL;
   if (!F || !theta) return fail(c, GF_EINVAL, "gf_measure: null out-param");
   cudaError_t e = launch_measure(c->k, c->qblocks);
-  if (e == cudaSuccess)
-    e = cudaMemcpyAsync(c->host_result, c->k.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->k.stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_measure");
-  c->launches += 2;
+  c->launches += 1;
   *F = c->host_result[0];
   *theta = c->host_result[1];
   if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_measure: non-finite F or theta");
@@ -404,8 +409,6 @@ static int fft_delta(gf_ctx* c) {
 // F, theta from the partials of the last fft_delta; synchronises
 static int fft_read_result(gf_ctx* c, double* F, double* theta) {
   cudaError_t e = launch_sd_final(c->k);
-  if (e == cudaSuccess)
-    e = cudaMemcpyAsync(c->host_result, c->k.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->k.stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_fix_fft (F, theta)");
   c->launches += 1;

@@ -10,7 +10,8 @@ struct KernelArgs {
   void* links;     // internal-layout link field (device)
   void* partials;  // double2 per measure block (device)
   void* qpartials; // double per half-sweep block: theta terms left by a fused odd half-sweep (device)
-  void* result;    // 2 doubles: F, theta (device)
+  void* result;    // 2 doubles: F, theta (device pointer of mapped pinned host memory)
+  void* counter;   // one unsigned, zero between launches: block-completion count of the measure kernel (device)
   Geo geo;
   cudaStream_t stream;
   int prec;     // 0 = FP64, 1 = FP32
@@ -29,7 +30,7 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks);
 bool halfsweep_can_fuse_theta(const KernelArgs& a);
 int halfsweep_max_qblocks(const Geo& g);
-// 2 kernel launches.  nq > 0: a.qpartials[0..nq) hold the odd sites' theta terms of the links as they stand, so only
+// 1 kernel launch (the last block to finish does the second stage).  nq > 0: a.qpartials[0..nq) hold the odd sites' theta terms of the links as they stand, so only
 // the even sites are visited (every link read once); nq = 0: all sites are visited.
 cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);

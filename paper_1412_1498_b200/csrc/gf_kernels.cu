@@ -403,10 +403,20 @@ int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 // Block partials by warp shuffles (FP64), one double2 per block; a single-block second stage adds them in index order.
 constexpr int MEASURE_THREADS = 256;
 
+// what the last block of measure_partial_kernel needs to finish the reduction
+struct MeasureTail {
+  unsigned* counter;        // zero before the launch; left at zero
+  int nf;                   // f is summed over the first nf partials only (the even sites: every link once)
+  const double* qpartials;  // nq theta terms left by the last odd half-sweep (may be 0)
+  int nq;
+  double norm_f, norm_q;
+  double* result;           // F, theta
+};
+
 template <class T, int NELEM, int ND>
 __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const cplx_t<T>* __restrict__ links, Geo g,
                                                                           int blocks_per_parity,
-                                                                          double2* __restrict__ partials) {
+                                                                          double2* __restrict__ partials, MeasureTail tail) {
   using C = cplx_t<T>;
   const int parity = blockIdx.x >= blocks_per_parity;
   const int cb = (blockIdx.x - parity * blocks_per_parity) * MEASURE_THREADS + threadIdx.x;
@@ -434,24 +444,31 @@ __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const 
     q = (double)delta_norm2<T>(A);
   }
   block_sum2<MEASURE_THREADS>(f, q);
-  if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(f, q);
-}
-
-// second stage: one block of 1024 threads; thread i adds partials i, i+1024, ... in order; fixed tree afterwards.
-// f is summed over the first nf entries of `partials` only (the even sites), q over all n of them plus the nq entries
-// of `qpartials` (the odd sites' terms left by the last odd half-sweep, when they are valid).
-__global__ void __launch_bounds__(1024) measure_final_kernel(const double2* __restrict__ partials, int n, int nf,
-                                                             const double* __restrict__ qpartials, int nq,
-                                                             double norm_f, double norm_q, double* __restrict__ result) {
-  double f = 0.0, q = 0.0;
-  for (int i = threadIdx.x; i < n; i += 1024) {
-    const double2 p = partials[i];
-    if (i < nf) f += p.x;
+  // Second stage in the same launch: the block that finishes last adds the partials in index order (thread i takes
+  // i, i+256, ...; fixed tree afterwards), so the result does not depend on which block that is.
+  __shared__ bool last;
+  if (threadIdx.x == 0) {
+    partials[blockIdx.x] = make_double2(f, q);
+    __threadfence();
+    last = atomicAdd(tail.counter, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  f = 0.0; q = 0.0;
+  for (int i = threadIdx.x; i < (int)gridDim.x; i += MEASURE_THREADS) {
+    const double2 p = __ldcg(partials + i);
+    if (i < tail.nf) f += p.x;
     q += p.y;
   }
-  for (int i = threadIdx.x; i < nq; i += 1024) q += qpartials[i];
-  block_sum2<1024>(f, q);
-  if (threadIdx.x == 0) { result[0] = f * norm_f; result[1] = q * norm_q; }
+  for (int i = threadIdx.x; i < tail.nq; i += MEASURE_THREADS) q += __ldcg(tail.qpartials + i);
+  __syncthreads();  // block_sum2's shared scratch is reused
+  block_sum2<MEASURE_THREADS>(f, q);
+  if (threadIdx.x == 0) {
+    tail.result[0] = f * tail.norm_f;
+    tail.result[1] = q * tail.norm_q;
+    *tail.counter = 0u;  // ready for the next launch on this stream
+  }
 }
 
 int measure_num_partials(const Geo& g) { return 2 * ((g.vh + MEASURE_THREADS - 1) / MEASURE_THREADS); }
@@ -461,13 +478,11 @@ template <class T, int NELEM, int ND>
 static cudaError_t measure_T(const KernelArgs& a, int nq) {
   const int bpp = measure_num_partials(a.geo) / 2;
   const int nblk = nq > 0 ? bpp : 2 * bpp;
-  measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo, bpp,
-                                                                              (double2*)a.partials);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
   const double V = 2.0 * (double)a.geo.vh;
-  measure_final_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, bpp, (const double*)a.qpartials, nq,
-                                                 1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V), (double*)a.result);
+  const MeasureTail tail{(unsigned*)a.counter, bpp, (const double*)a.qpartials, nq, 1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V),
+                         (double*)a.result};
+  measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo, bpp,
+                                                                              (double2*)a.partials, tail);
   return cudaGetLastError();
 }
 

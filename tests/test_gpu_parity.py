@@ -256,7 +256,7 @@ def test_fused_theta_terms_match_full_measure_and_oracle(gf, torch, dims, gauge,
         fx.ovr_sweep(3, omega)
         n0 = fx.kernel_launches()
         res[fuse] = fx.measure()
-        assert fx.kernel_launches() - n0 == 2
+        assert fx.kernel_launches() - n0 == 1  # one launch: the last block to finish does the second stage
         again = fx.measure()  # the fused terms stay valid until the links change
         assert again == res[fuse]
         fx.reunitarize()  # changes the links: the next measure must visit all sites again
