@@ -299,6 +299,24 @@ def run_ours(args):
                 "whole_step_gbs": (16 * V * L * n_sw + 4 * V * L) / (ms_total / args.steps * 1e-3) / 1e9}
     roofline["whole_step_frac"] = roofline["whole_step_gbs"] / peak
 
+    # ---- the config's whole contract run (gf_fix from fresh links with the config's eps / sweep cap / cadence):
+    # config 4's "fixed 200 sweeps with F/theta every 20 sweeps, run as a sustained-throughput test"
+    contract = None
+    if not args.no_contract:
+        fx.set_links(canon)
+        torch.cuda.synchronize()
+        c0, c1 = ev(), ev()
+        c0.record()
+        done = fx.fix(omega, cfg["eps"], cfg["max_sweeps"], n_sw)
+        c1.record()
+        torch.cuda.synchronize()
+        ms_c = max_over_ranks(c0.elapsed_time(c1), dist, "cuda")
+        hist = fx.history()
+        contract = {"what": f"gf_fix(omega={omega}, eps={cfg['eps']}, max_sweeps={cfg['max_sweeps']}, check_every={n_sw})",
+                    "sweeps_done": done, "measurements": len(hist), "ms": ms_c,
+                    "value": aggregate_value(world, V, done, ms_c), "unit": UNIT,
+                    "final_F": hist[-1][1], "final_theta": hist[-1][2]}
+
     # ---- end to end through the host entry points (pinned host memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -354,7 +372,7 @@ def run_ours(args):
                    "sites": V, "l2": "inputs exceed L2 (field %.2f GB vs 126 MB)" % (4 * V * L / 1e9)
                    if 4 * V * L > 4 * 126e6 else "field fits L2: not an HBM measurement", "parallelism": "replicas only",
                    "final_F": F, "final_theta": th},
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": roofline, "contract_run": contract, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -415,6 +433,21 @@ def run_fftsd(args):
                          "peak_source": peak_src, "algorithmic_bytes_per_iteration": bytes_it},
             "gpu_launches": int(fx.kernel_launches() - l0)}
     fx.close()
+    if not args.no_cpu:  # the numpy oracle of Algorithm 2 as it stands, on a slab of the same lattice
+        import numpy as np
+
+        from oracle import fftsd
+
+        sd = oracle_sample_dims(cfg)
+        Uo = np.ascontiguousarray(gi.make_links(sd, cfg["roughness"], cfg["seed"]))
+        w0 = time.perf_counter()
+        fftsd.step(Uo, sd, cfg["gauge"], 0.08, storage=storage)
+        F, th = fftsd.measure(Uo, sd, cfg["gauge"])
+        dt = time.perf_counter() - w0
+        line["cpu_baseline"] = {"value": gi.volume(sd) / dt, "unit": "site-iterations/s", "cores": os.cpu_count(),
+                                "kind": "oracle", "seconds": dt,
+                                "sample": f"oracle/fftsd.py (numpy, FP64), 1 iteration + 1 F/theta on a "
+                                          f"{sd[0]}x{sd[1]}x{sd[2]}x{sd[3]} slab of the workload lattice"}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -431,6 +464,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-contract", action="store_true", help="skip the timed whole-config gf_fix run")
     ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
     args = ap.parse_args()
     if args.impl == "reference":
