@@ -39,7 +39,9 @@ UNIT = "site-updates/s"
 LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48}
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the committed ncu --set full capture
 # (profiles/): filled per config once a capture exists, else null.
-NCU_TRAFFIC_BYTES = {"cfg4": 19.329357e9 + 19.270288e9}  # profiles/r1b_halfsweep_cfg4_ncu.txt
+NCU_TRAFFIC_BYTES = {"cfg4": 19.327848e9 + 19.269022e9,  # profiles/r1f_halfsweep_cfg4_ncu.txt
+                     "cfg3": 4.076932e9 + 4.017487e9,    # profiles/r1c_halfsweep_cfg3_ncu.txt
+                     "cfg2": 201.386e6 + 142.245e6}      # profiles/r1f_halfsweep_cfg2_ncu.txt (partly L2-resident)
 
 
 def log(*a):

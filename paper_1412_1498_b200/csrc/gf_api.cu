@@ -292,7 +292,7 @@ int gf_measure(gf_ctx* c, double* F, double* theta) {
   cudaError_t e = launch_measure(c->k, c->qblocks);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_measure");
-  c->launches += 1;
+  c->launches += measure_launches(c->k.geo, c->qblocks);
   *F = c->host_result[0];
   *theta = c->host_result[1];
   if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_measure: non-finite F or theta");

@@ -30,11 +30,12 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks);
 bool halfsweep_can_fuse_theta(const KernelArgs& a);
 int halfsweep_max_qblocks(const Geo& g);
-// 1 kernel launch (the last block to finish does the second stage).  nq > 0: a.qpartials[0..nq) hold the odd sites' theta terms of the links as they stand, so only
+// 1 kernel launch on small grids (the last block to finish does the second stage), else 2.  nq > 0: a.qpartials[0..nq) hold the odd sites' theta terms of the links as they stand, so only
 // the even sites are visited (every link read once); nq = 0: all sites are visited.
 cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);
 int measure_num_partials(const Geo& g);
+int measure_launches(const Geo& g, int nq);  // kernels launch_measure issues: 1 (small grids) or 2
 
 // ---- Algorithm 2 (gf_fftsd.cu): steepest descent with Fourier acceleration ------------------------------------------------
 struct FftPlans;  // the cuFFT plans of one context

@@ -402,6 +402,7 @@ int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 // Grid: blocks_per_parity * nparity blocks; the first blocks_per_parity blocks take parity `parity0`, the rest the other.
 // Block partials by warp shuffles (FP64), one double2 per block; a single-block second stage adds them in index order.
 constexpr int MEASURE_THREADS = 256;
+constexpr int MEASURE_SINGLE_LAUNCH_MAX_BLOCKS = 4096;
 
 // what the last block of measure_partial_kernel needs to finish the reduction
 struct MeasureTail {
@@ -412,6 +413,24 @@ struct MeasureTail {
   double norm_f, norm_q;
   double* result;           // F, theta
 };
+
+// thread i adds partials i, i+THREADS, ... in order; fixed tree afterwards (deterministic).  One block of THREADS.
+template <int THREADS>
+__device__ __forceinline__ void measure_tail(const double2* __restrict__ partials, int n, const MeasureTail& tail) {
+  double f = 0.0, q = 0.0;
+  for (int i = threadIdx.x; i < n; i += THREADS) {
+    const double2 p = __ldcg(partials + i);
+    if (i < tail.nf) f += p.x;
+    q += p.y;
+  }
+  for (int i = threadIdx.x; i < tail.nq; i += THREADS) q += __ldcg(tail.qpartials + i);
+  __syncthreads();  // block_sum2's shared scratch may still be in use by the caller's first stage
+  block_sum2<THREADS>(f, q);
+  if (threadIdx.x == 0) {
+    tail.result[0] = f * tail.norm_f;
+    tail.result[1] = q * tail.norm_q;
+  }
+}
 
 template <class T, int NELEM, int ND>
 __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const cplx_t<T>* __restrict__ links, Geo g,
@@ -444,8 +463,12 @@ __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const 
     q = (double)delta_norm2<T>(A);
   }
   block_sum2<MEASURE_THREADS>(f, q);
-  // Second stage in the same launch: the block that finishes last adds the partials in index order (thread i takes
-  // i, i+256, ...; fixed tree afterwards), so the result does not depend on which block that is.
+  if (tail.counter == nullptr) {  // large grids: the second stage is its own small launch (see measure_T)
+    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(f, q);
+    return;
+  }
+  // Second stage in the same launch: the block that finishes last adds the partials in index order, so the result
+  // does not depend on which block that is.
   __shared__ bool last;
   if (threadIdx.x == 0) {
     partials[blockIdx.x] = make_double2(f, q);
@@ -455,22 +478,18 @@ __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const 
   __syncthreads();
   if (!last) return;
   __threadfence();
-  f = 0.0; q = 0.0;
-  for (int i = threadIdx.x; i < (int)gridDim.x; i += MEASURE_THREADS) {
-    const double2 p = __ldcg(partials + i);
-    if (i < tail.nf) f += p.x;
-    q += p.y;
-  }
-  for (int i = threadIdx.x; i < tail.nq; i += MEASURE_THREADS) q += __ldcg(tail.qpartials + i);
-  __syncthreads();  // block_sum2's shared scratch is reused
-  block_sum2<MEASURE_THREADS>(f, q);
-  if (threadIdx.x == 0) {
-    tail.result[0] = f * tail.norm_f;
-    tail.result[1] = q * tail.norm_q;
-    *tail.counter = 0u;  // ready for the next launch on this stream
-  }
+  measure_tail<MEASURE_THREADS>(partials, (int)gridDim.x, tail);
+  if (threadIdx.x == 0) *tail.counter = 0u;  // ready for the next launch on this stream
 }
 
+__global__ void __launch_bounds__(1024) measure_tail_kernel(const double2* __restrict__ partials, int n, MeasureTail tail) {
+  measure_tail<1024>(partials, n, tail);
+}
+
+int measure_launches(const Geo& g, int nq) {
+  const int bpp = ((g.vh + MEASURE_THREADS - 1) / MEASURE_THREADS);
+  return (nq > 0 ? bpp : 2 * bpp) <= MEASURE_SINGLE_LAUNCH_MAX_BLOCKS ? 1 : 2;
+}
 int measure_num_partials(const Geo& g) { return 2 * ((g.vh + MEASURE_THREADS - 1) / MEASURE_THREADS); }
 
 // nq > 0: the odd sites' theta terms are already in a.qpartials[0..nq): visit the even sites only.
@@ -479,10 +498,16 @@ static cudaError_t measure_T(const KernelArgs& a, int nq) {
   const int bpp = measure_num_partials(a.geo) / 2;
   const int nblk = nq > 0 ? bpp : 2 * bpp;
   const double V = 2.0 * (double)a.geo.vh;
-  const MeasureTail tail{(unsigned*)a.counter, bpp, (const double*)a.qpartials, nq, 1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V),
-                         (double*)a.result};
+  // Small lattices are latency bound: one launch, the last block to finish does the second stage.  On large grids
+  // 65536 blocks queueing on one completion counter cost more (cfg4: +0.13 ms) than a second small launch.
+  const bool single = nblk <= MEASURE_SINGLE_LAUNCH_MAX_BLOCKS;
+  const MeasureTail tail{single ? (unsigned*)a.counter : nullptr, bpp, (const double*)a.qpartials, nq,
+                         1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V), (double*)a.result};
   measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo, bpp,
                                                                               (double2*)a.partials, tail);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess || single) return e;
+  measure_tail_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, tail);
   return cudaGetLastError();
 }
 
