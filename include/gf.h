@@ -110,8 +110,11 @@ enum {
   GF_OPT_FUSE_MEASURE = 3,  /* 1 (default): the last odd half-sweep of every gf_ovr_sweep call also leaves the odd
                                sites' terms of theta, so a gf_measure that follows directly visits the even sites only
                                and reads every link once; 0: gf_measure always visits all sites */
-  GF_OPT_FFT_ACCELERATE = 4 /* 1 (default): gf_fft_step / gf_fix_fft use the Fourier factor of eq. 1.8; 0: the naive
+  GF_OPT_FFT_ACCELERATE = 4, /* 1 (default): gf_fft_step / gf_fix_fft use the Fourier factor of eq. 1.8; 0: the naive
                                steepest descent of eq. 1.7 (no transforms) */
+  GF_OPT_FFT_FUSED_T = 5    /* 1: in Landau gauge with n_t a power of two (<= 256) the transform along t, the Fourier
+                               factor and the inverse transform along t are one hand-written pass through shared
+                               memory; 0 (default): cuFFT's strided 1-D transforms and a separate factor kernel */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 

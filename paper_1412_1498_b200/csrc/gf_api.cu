@@ -73,6 +73,7 @@ struct gf_ctx {
   char* fft_w;        // four packed complex fields of V entries
   double* fft_table;  // 4 sin^2(pi k/n) per direction
   int fft_accelerate; // GF_OPT_FFT_ACCELERATE
+  int fft_fused_t;    // GF_OPT_FFT_FUSED_T
   char err[256];
 };
 
@@ -130,7 +131,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->fuse_measure = 1; c->qblocks = 0;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
-  c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1;
+  c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
   c->host_result = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
@@ -252,6 +253,9 @@ int gf_set_option(gf_ctx* c, int key, int value) {
       return GF_OK;
     case GF_OPT_FFT_ACCELERATE:
       c->fft_accelerate = value != 0;
+      return GF_OK;
+    case GF_OPT_FFT_FUSED_T:
+      c->fft_fused_t = value != 0;
       return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
@@ -384,11 +388,15 @@ int gf_fft_attach(gf_ctx* c, void* dev_workspace, size_t workspace_bytes) {
 static int fft_update(gf_ctx* c, double alpha) {
   int n = 0;
   const char* msg = nullptr;
-  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, true, &n);
+  cudaError_t e;
+  // Landau gauge, n_t a power of two: the t direction (transform, factor, inverse transform) is one fused pass
+  const bool fused_t = c->fft_accelerate && c->fft_fused_t && c->k.gauge == GF_LANDAU && sd_tline_supported(c->k.geo);
+  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, true, !fused_t, &n);
   if (msg) return fail(c, GF_ECUDA, msg);
-  cudaError_t e = launch_sd_filter(c->k, c->fft_w, c->fft_table, alpha, c->fft_accelerate != 0);
+  if (fused_t) e = launch_sd_tline(c->k, c->fft_w, c->fft_table, alpha);
+  else e = launch_sd_filter(c->k, c->fft_w, c->fft_table, alpha, c->fft_accelerate != 0);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (factor)");
-  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, false, &n);
+  if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, false, !fused_t, &n);
   if (msg) return fail(c, GF_ECUDA, msg);
   e = launch_sd_rotate(c->k, c->fft_w);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (rotate)");

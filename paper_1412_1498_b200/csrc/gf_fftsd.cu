@@ -230,6 +230,142 @@ __global__ void __launch_bounds__(256) sd_scale_kernel(cplx_t<T>* __restrict__ w
 }
 
 // ======================================================================================================================
+// t direction: forward transform, Fourier factor and inverse transform in ONE pass (Landau gauge, n_t a power of two)
+// ======================================================================================================================
+// The factor is diagonal in 4-D momentum space and the transforms along different axes commute, so after the 3-D
+// transform of every time slice the remaining work per spatial momentum (kx,ky,kz) is: transform the n_t numbers along
+// t, multiply by (alpha/2) p^2_max / p^2 / N, transform back.  A block takes TLINE_XB consecutive x of one field and
+// keeps their t-lines in shared memory: one read and one write of the field instead of three of each (cuFFT's strided
+// 1-D transform, sd_filter, cuFFT's inverse) and one launch instead of nine.
+// Radix-2: decimation in time on a bit-reversed load (natural-order output for the factor), then decimation in
+// frequency for the inverse (bit-reversed output, undone by the store).  Thread (j, b): x offset j, butterfly b < n_t/2.
+constexpr int TLINE_THREADS = 512;
+
+template <class C> __device__ __forceinline__ C cmul_conj(const C a, const C b) {  // a * conj(b)
+  C z; z.x = a.x * b.x + a.y * b.y; z.y = a.y * b.x - a.x * b.y; return z;
+}
+
+// XB consecutive x per block (XB * sizeof(complex) = 256 B contiguous per t);
+// thread (j, b0): x offset j = tid % XB, butterflies b = b0, b0 + TLINE_THREADS/XB, ... < n_t/2.
+template <class T, int XB>
+__global__ void __launch_bounds__(TLINE_THREADS) sd_tline_kernel(cplx_t<T>* __restrict__ w, Geo g, int logn,
+                                                                 const double* __restrict__ table, double scale_p2max) {
+  using C = cplx_t<T>;
+  extern __shared__ __align__(16) unsigned char tline_smem[];
+  constexpr int BT = TLINE_THREADS / XB;
+  const int n = g.n[3], nh = n / 2;
+  C* data = reinterpret_cast<C*>(tline_smem);   // [n][XB]
+  C* tw = data + n * XB;                        // [n/2]: exp(-2 pi i k / n)
+  const int j = threadIdx.x % XB, b0 = threadIdx.x / XB;
+  const size_t V3 = (size_t)g.n[0] * g.n[1] * g.n[2], V = V3 * n;
+  const size_t s = (size_t)blockIdx.x * XB + j;  // spatial momentum index kx + nx (ky + ny kz)
+  C* base = w + (size_t)blockIdx.y * V + s;
+  for (int k = threadIdx.x; k < nh; k += TLINE_THREADS) {
+    double sn, cs;
+    sincospi(-2.0 * (double)k / (double)n, &sn, &cs);
+    tw[k] = mk<T>((T)cs, (T)sn);
+  }
+  // bit-reversed load straight into shared memory (cp.async: every row of the block in flight at once)
+  for (int e = b0; e < n; e += BT) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(data + (int)(__brev((unsigned)e) >> (32 - logn)) * XB + j);
+    if (sizeof(C) == 16)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(base + (size_t)e * V3) : "memory");
+    else
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(base + (size_t)e * V3) : "memory");
+  }
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
+  for (int st = 0; st < logn; ++st) {  // forward, decimation in time
+    const int half = 1 << st;
+    for (int b = b0; b < nh; b += BT) {
+      const int pos = b & (half - 1), i0 = ((b >> st) << (st + 1)) + pos, i1 = i0 + half;
+      const C t = tw[pos << (logn - 1 - st)];
+      const C a = data[i0 * XB + j], c = cmul(data[i1 * XB + j], t);
+      data[i0 * XB + j] = mk<T>(a.x + c.x, a.y + c.y);
+      data[i1 * XB + j] = mk<T>(a.x - c.x, a.y - c.y);
+    }
+    __syncthreads();
+  }
+  {  // factor (readings B2-B4), natural order: entry e is k_t = e
+    unsigned q = (unsigned)s;
+    const int kx = q % (unsigned)g.n[0]; q /= (unsigned)g.n[0];
+    const int ky = q % (unsigned)g.n[1];
+    const int kz = q / (unsigned)g.n[1];
+    const double p3 = table[kx] + table[g.n[0] + ky] + table[g.n[0] + g.n[1] + kz];
+    const double* tt = table + g.n[0] + g.n[1] + g.n[2];
+    for (int e = b0; e < n; e += BT) {
+      const double p2 = p3 + tt[e];
+      const T f = p2 > 0.0 ? (T)(scale_p2max / p2) : T(0);
+      C v = data[e * XB + j];
+      v.x *= f; v.y *= f;
+      data[e * XB + j] = v;
+    }
+  }
+  __syncthreads();
+  for (int st = logn - 1; st >= 0; --st) {  // inverse, decimation in frequency
+    const int half = 1 << st;
+    for (int b = b0; b < nh; b += BT) {
+      const int pos = b & (half - 1), i0 = ((b >> st) << (st + 1)) + pos, i1 = i0 + half;
+      const C t = tw[pos << (logn - 1 - st)];
+      const C a = data[i0 * XB + j], c = data[i1 * XB + j];
+      data[i0 * XB + j] = mk<T>(a.x + c.x, a.y + c.y);
+      data[i1 * XB + j] = cmul_conj(mk<T>(a.x - c.x, a.y - c.y), t);
+    }
+    __syncthreads();
+  }
+#pragma unroll 8
+  for (int e = b0; e < n; e += BT) base[(size_t)(__brev((unsigned)e) >> (32 - logn)) * V3] = data[e * XB + j];
+}
+
+// can the fused t pass be used on this lattice?  (Landau gauge is the caller's business)
+static int tline_xb(const Geo& g, int prec) {
+  const long long V3 = (long long)g.n[0] * g.n[1] * g.n[2];
+  const int want = prec == 0 ? 16 : 32;  // 256 B per t; smaller tiles = more blocks per SM to overlap load / butterfly / store phases
+  for (int xb = want; xb >= 8; xb /= 2)
+    if (V3 % xb == 0) return xb;
+  return 0;
+}
+bool sd_tline_supported(const Geo& g) {
+  const int n = g.n[3];
+  return n >= 2 && n <= 256 && (n & (n - 1)) == 0 && tline_xb(g, 0) != 0;
+}
+
+template <class T, int XB>
+static cudaError_t sd_tline_T(const KernelArgs& a, void* w, const double* table, int logn, double scale_p2max) {
+  using C = cplx_t<T>;
+  const int n = a.geo.n[3];
+  const size_t V3 = (size_t)a.geo.n[0] * a.geo.n[1] * a.geo.n[2];
+  const size_t smem = ((size_t)n * XB + n / 2) * sizeof(C);
+  auto kern = sd_tline_kernel<T, XB>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  kern<<<dim3((unsigned)(V3 / XB), 4), TLINE_THREADS, smem, a.stream>>>((C*)w, a.geo, logn, table, scale_p2max);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_sd_tline(const KernelArgs& a, void* w, const double* table, double alpha) {
+  const int n = a.geo.n[3];
+  int logn = 0;
+  while ((1 << logn) < n) ++logn;
+  const double V = 2.0 * (double)a.geo.vh;
+  const double scale_p2max = 0.5 * alpha / V * 16.0;
+  const int xb = tline_xb(a.geo, a.prec);
+  if (a.prec == 0) {
+    switch (xb) {
+      case 16: return sd_tline_T<double, 16>(a, w, table, logn, scale_p2max);
+      case 8: return sd_tline_T<double, 8>(a, w, table, logn, scale_p2max);
+    }
+  } else {
+    switch (xb) {
+      case 32: return sd_tline_T<float, 32>(a, w, table, logn, scale_p2max);
+      case 16: return sd_tline_T<float, 16>(a, w, table, logn, scale_p2max);
+      case 8: return sd_tline_T<float, 8>(a, w, table, logn, scale_p2max);
+    }
+  }
+  return cudaErrorInvalidValue;
+}
+
+// ======================================================================================================================
 // g(x) and the gauge rotation
 // ======================================================================================================================
 // g = reunitarise(1 + w), w rebuilt from its packed form (reading B5)
@@ -343,14 +479,14 @@ const char* fft_plans_set_work(FftPlans* p, void* work) {
 }
 
 // in-place transform of the four packed fields; *launches += number of cuFFT executions
-const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward, int* launches) {
+const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward, bool with_t, int* launches) {
   const int dir = forward ? CUFFT_FORWARD : CUFFT_INVERSE;
   const size_t V = 2 * (size_t)g.vh;
   cufftResult r;
   if (prec == 0) {
     r = cufftExecZ2Z(p->plan3, (cufftDoubleComplex*)w, (cufftDoubleComplex*)w, dir);
     *launches += 1;
-    for (int k = 0; k < 4 && r == CUFFT_SUCCESS && p->have1; ++k) {
+    for (int k = 0; k < 4 && r == CUFFT_SUCCESS && p->have1 && with_t; ++k) {
       cufftDoubleComplex* f = (cufftDoubleComplex*)w + k * V;
       r = cufftExecZ2Z(p->plan1, f, f, dir);
       *launches += 1;
@@ -358,7 +494,7 @@ const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward,
   } else {
     r = cufftExecC2C(p->plan3, (cufftComplex*)w, (cufftComplex*)w, dir);
     *launches += 1;
-    for (int k = 0; k < 4 && r == CUFFT_SUCCESS && p->have1; ++k) {
+    for (int k = 0; k < 4 && r == CUFFT_SUCCESS && p->have1 && with_t; ++k) {
       cufftComplex* f = (cufftComplex*)w + k * V;
       r = cufftExecC2C(p->plan1, f, f, dir);
       *launches += 1;

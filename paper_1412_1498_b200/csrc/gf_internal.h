@@ -45,7 +45,11 @@ const char* fft_plans_create(FftPlans** out, const Geo& g, int prec, int gauge, 
 const char* fft_plans_set_work(FftPlans* p, void* work);
 void fft_plans_destroy(FftPlans* p);
 // in-place forward / backward (unnormalised) transform of the four packed fields at w; *launches += cuFFT executions
-const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward, int* launches);
+// with_t = false: only the 3-D transform of every time slice (the t direction is done by launch_sd_tline)
+const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward, bool with_t, int* launches);
+bool sd_tline_supported(const Geo& g);
+// forward transform along t, Fourier factor, inverse transform along t in one pass (Landau, n_t a power of two)
+cudaError_t launch_sd_tline(const KernelArgs& a, void* w, const double* table, double alpha);
 size_t sd_table_entries(const Geo& g);  // doubles in the 4 sin^2(pi k/n) table
 int sd_num_partials(const Geo& g);      // <= measure_num_partials(g): a.partials is shared
 cudaError_t launch_sd_table(const KernelArgs& a, double* table);

@@ -126,3 +126,27 @@ def test_errors():
     assert gf.gf_fft_attach(fx.ctx, fx.fft_workspace.data_ptr(), 16) == gf.GF_ENOMEM
     assert gf.gf_fft_step(fx.ctx, 0, 0.08) == gf.GF_OK
     fx.close()
+
+
+@pytest.mark.parametrize("dims,prec", [((8, 8, 8, 16), "f64"), ((8, 8, 8, 16), "f32"), ((16, 4, 6, 2), "f64"),
+                                       ((16, 4, 6, 2), "f32"), ((8, 4, 4, 64), "f64"), ((8, 4, 4, 64), "f32"),
+                                       ((16, 16, 8, 32), "f64"), ((16, 16, 8, 32), "f32"),
+                                       ((4, 4, 4, 256), "f64")])  # n_t = 256 in FP32: p^2_max/p^2 = 26000 amplifies
+def test_fused_t_pass_against_cufft_path_and_oracle(dims, prec):
+    """GF_OPT_FFT_FUSED_T: the hand-written pass (transform along t, Fourier factor, inverse transform along t through
+    shared memory; n_t = 2 ... 256) against cuFFT's strided 1-D transforms + the factor kernel, and both against the
+    oracle."""
+    U, Uo = make(dims, 0.5, 36, prec, 18)
+    res = {}
+    for fused in (1, 0):
+        fx, gf = fixer(dims, "landau", prec, 18, U)
+        fx.set_option(gf.GF_OPT_FFT_FUSED_T, fused)
+        n0 = None
+        fx.fft_step(2, 0.08)
+        res[fused] = fx.get_links().cpu().numpy().astype(np.float64)
+        fx.close()
+    for _ in range(2):
+        fftsd.step(Uo, dims, "landau", 0.08)
+    tol = TOL_LINK[prec]
+    assert np.abs(res[1] - res[0]).max() <= (1e-13 if prec == "f64" else 1e-5)
+    assert np.abs(res[1] - Uo).max() <= 2 * tol and np.abs(res[0] - Uo).max() <= 2 * tol
