@@ -141,6 +141,45 @@ int gf_fft_attach(gf_ctx* ctx, void* dev_workspace, size_t workspace_bytes);
 int gf_fft_step(gf_ctx* ctx, int n, double alpha);
 int gf_fix_fft(gf_ctx* ctx, double alpha, double eps, int max_iters, int check_every, int* iters_done);
 
+/* ---- T-slab sharding of the overrelaxation sweep (PAPER.md:132-134 border / interior split and the exchange of the
+ * top links "and back"; PAPER.md:146 partition T first) ------------------------------------------------------------------
+ * A lattice nx*ny*nz*(R*lt) is cut into R slabs of lt time slices (lt even, so local and global site parity agree).
+ * Each slab is an ordinary context created with gf_create(nx, ny, nz, lt, ...) that becomes a slab once a halo
+ * workspace is attached.  The only links a slab's sites touch that it does not own are U_t(x - t) of its t = 0 sites:
+ * the lower neighbour's top-slice temporal links.  They are kept in a ghost buffer that the half-sweep kernels read
+ * and update in place; the caller (one process per GPU) moves the four messages below between neighbours with its
+ * own transport (device-to-device copies, NCCL send/recv), all device memory, no host staging.
+ *
+ * Halo workspace (caller-owned device memory, 256-byte aligned, valid until gf_destroy), B = gf_slab_halo_bytes:
+ *   [0, B)    ghost[0]: U_t(x) of the parity-0 sites of the lower neighbour's top slice     (kernels read + write)
+ *   [B, 2B)   ghost[1]: the same for its parity-1 sites
+ *   [2B, 3B)  top_out : U_t(x) of one parity of this slab's top slice, packed by gf_slab_pack_top /
+ *                       gf_slab_halfsweep_border, to be delivered into the UPPER neighbour's ghost[parity]
+ *   [3B, 4B)  top_in  : a ghost buffer coming back from the upper neighbour, scattered by gf_slab_unpack_top
+ * Message layout = the internal layout of one parity of one time slice, direction t only:
+ *   [cb3 / 32][element][cb3 % 32] complex numbers, cb3 = (x + nx (y + ny z)) / 2, 9 or 6 elements per link.
+ *
+ * One half-sweep of parity p on every slab (even first, then odd, as gf_ovr_sweep):
+ *   1. gf_slab_halfsweep_border(p, omega): the parity-p sites of slices 0 and lt-1; the t = 0 sites update ghost[1-p];
+ *      then top_out <- U_t of the parity-p sites of the top slice (just updated).
+ *   2. gf_slab_halfsweep_interior(p, omega): slices 1 .. lt-2; touches no link of step 3, so the transport may run
+ *      beside it on another stream.
+ *   3. transport: ghost[1-p] -> lower neighbour's top_in;  top_out -> upper neighbour's ghost[p].
+ *   4. gf_slab_unpack_top(1-p): top_in -> U_t of the parity-(1-p) sites of the top slice.
+ * Before the first half-sweep (after gf_set_links, gf_reunitarize): for q = 0, 1: gf_slab_pack_top(q), transport
+ * top_out -> upper neighbour's ghost[q].
+ * On a slab context gf_measure returns the slab's own F and theta (the global values are the means over the R
+ * equal slabs); gf_ovr_sweep and gf_fix return GF_EINVAL, the gf_fft_* calls GF_EUNSUPPORTED (the paper has no
+ * multi-GPU Algorithm 2 either).  With R = 1 (the slab is its own neighbour) the calls reproduce
+ * gf_ovr_sweep bit for bit.  All Async.  Errors: GF_EINVAL (no halo attached, parity not 0/1, omega), GF_ENOMEM,
+ * GF_ECUDA. */
+size_t gf_slab_halo_bytes(const gf_ctx* ctx);
+int gf_slab_attach(gf_ctx* ctx, void* dev_halo, size_t halo_workspace_bytes);
+int gf_slab_pack_top(gf_ctx* ctx, int parity);
+int gf_slab_unpack_top(gf_ctx* ctx, int parity);
+int gf_slab_halfsweep_border(gf_ctx* ctx, int parity, double omega);
+int gf_slab_halfsweep_interior(gf_ctx* ctx, int parity, double omega);
+
 /* Number of kernels this context has launched since gf_create (for benchmark bookkeeping). */
 long long gf_kernel_launches(const gf_ctx* ctx);
 

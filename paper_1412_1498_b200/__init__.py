@@ -4,3 +4,4 @@ The product is the C-ABI library libgf.so (include/gf.h, csrc/); this package is
 """
 from .binding import *  # noqa: F401,F403
 from .binding import GaugeFixer, GFError, SYMBOLS  # noqa: F401
+from .sharded import GpuSlabEngine, ShardedGaugeFixer  # noqa: F401

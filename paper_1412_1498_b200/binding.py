@@ -20,7 +20,9 @@ GF_OPT_SWEEP_VARIANT, GF_OPT_BLOCK_THREADS, GF_OPT_FUSE_MEASURE, GF_OPT_FFT_ACCE
 SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "gf_set_links_host",
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
            "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error",
-           "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft"]
+           "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
+           "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_pack_top", "gf_slab_unpack_top",
+           "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"]
 
 
 def _load() -> ctypes.CDLL:
@@ -54,6 +56,16 @@ def _load() -> ctypes.CDLL:
     lib.gf_fft_step.argtypes = [c_void_p, c_int, c_double]
     lib.gf_fix_fft.restype = c_int
     lib.gf_fix_fft.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int)]
+    lib.gf_slab_halo_bytes.restype = c_size_t
+    lib.gf_slab_halo_bytes.argtypes = [c_void_p]
+    lib.gf_slab_attach.restype = c_int
+    lib.gf_slab_attach.argtypes = [c_void_p, c_void_p, c_size_t]
+    for name in ("gf_slab_pack_top", "gf_slab_unpack_top"):
+        getattr(lib, name).restype = c_int
+        getattr(lib, name).argtypes = [c_void_p, c_int]
+    for name in ("gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"):
+        getattr(lib, name).restype = c_int
+        getattr(lib, name).argtypes = [c_void_p, c_int, c_double]
     lib.gf_kernel_launches.restype = c_longlong
     lib.gf_kernel_launches.argtypes = [c_void_p]
     lib.gf_destroy.restype = None
@@ -163,6 +175,30 @@ def gf_fix_fft(ctx, alpha: float, eps: float, max_iters: int, check_every: int):
     done = c_int()
     rc = lib.gf_fix_fft(ctx, alpha, eps, max_iters, check_every, byref(done))
     return rc, done.value
+
+
+def gf_slab_halo_bytes(ctx) -> int:
+    return int(lib.gf_slab_halo_bytes(ctx))
+
+
+def gf_slab_attach(ctx, dev_halo: int, halo_workspace_bytes: int) -> int:
+    return lib.gf_slab_attach(ctx, c_void_p(dev_halo), halo_workspace_bytes)
+
+
+def gf_slab_pack_top(ctx, parity: int) -> int:
+    return lib.gf_slab_pack_top(ctx, parity)
+
+
+def gf_slab_unpack_top(ctx, parity: int) -> int:
+    return lib.gf_slab_unpack_top(ctx, parity)
+
+
+def gf_slab_halfsweep_border(ctx, parity: int, omega: float) -> int:
+    return lib.gf_slab_halfsweep_border(ctx, parity, omega)
+
+
+def gf_slab_halfsweep_interior(ctx, parity: int, omega: float) -> int:
+    return lib.gf_slab_halfsweep_interior(ctx, parity, omega)
 
 
 def gf_kernel_launches(ctx) -> int:

@@ -9,8 +9,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgf.so")
 SOURCES = ["gf_kernels.cu", "gf_fftsd.cu", "gf_api.cu"]
 HEADERS = ["gf_device.cuh", "gf_internal.h", os.path.join("..", "..", "include", "gf.h")]
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
-              "-Xcompiler", "-fPIC"]
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def stale() -> bool:
@@ -22,9 +21,20 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        cmd = ["nvcc", *NVCC_FLAGS, *( ["-Xptxas", "-v"] if verbose else []), "-o", LIB,
-               *[os.path.join(CSRC, s) for s in SOURCES], "-lcufft"]
-        subprocess.check_call(cmd)
+        import tempfile
+        from concurrent.futures import ThreadPoolExecutor
+
+        with tempfile.TemporaryDirectory() as tmp:
+            def compile_one(src):  # one nvcc per translation unit, side by side
+                obj = os.path.join(tmp, src + ".o")
+                subprocess.check_call(["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c",
+                                       os.path.join(CSRC, src), "-o", obj])
+                return obj
+
+            with ThreadPoolExecutor(len(SOURCES)) as pool:
+                objs = list(pool.map(compile_one, SOURCES))
+            subprocess.check_call(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs,
+                                   "-lcufft"])
     return LIB
 
 

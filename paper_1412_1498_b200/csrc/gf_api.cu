@@ -74,6 +74,10 @@ struct gf_ctx {
   double* fft_table;  // 4 sin^2(pi k/n) per direction
   int fft_accelerate; // GF_OPT_FFT_ACCELERATE
   int fft_fused_t;    // GF_OPT_FFT_FUSED_T
+  // T-slab sharding (gf_slab_*): the caller's halo workspace once attached
+  size_t halo_bytes;  // one message: U_t of one parity of one time slice
+  char* top_out;      // packed top-slice links on their way to the upper neighbour's ghost buffer
+  char* top_in;       // ghost links coming back from the upper neighbour
   char err[256];
 };
 
@@ -133,6 +137,9 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
+  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0};
+  c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
+  c->top_out = c->top_in = nullptr;
   c->host_result = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
   cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
@@ -270,6 +277,7 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
   if (!c) return GF_EINVAL;
   if (n < 0) return fail(c, GF_EINVAL, "gf_ovr_sweep: n < 0");
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
+  if (c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_ovr_sweep: the context is a slab, use gf_slab_halfsweep_*");
   if (n > 0) c->qblocks = 0;
   for (int i = 0; i < n; ++i) {
     for (int parity = 0; parity < 2; ++parity) {  // even first
@@ -309,6 +317,7 @@ int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every,
   if (check_every < 1 || max_sweeps < 0 || !(eps >= 0.0))
     return fail(c, GF_EINVAL, "gf_fix: need check_every >= 1, max_sweeps >= 0, eps >= 0");
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_fix: omega outside [1,2)");
+  if (c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_fix: the context is a slab, the driver loop belongs to the caller");
   c->history.clear();
   c->history_n = 0;
   *sweeps_done = 0;
@@ -347,6 +356,8 @@ int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
 
 // ---- Algorithm 2: steepest descent with Fourier acceleration -------------------------------------
 static int fft_plan(gf_ctx* c) {
+  if (c->k.slab.ghost)  // no multi-GPU steepest descent (no distributed 4-D transform)
+    return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not available on a slab context");
   if (c->fft) return GF_OK;
   size_t work = 0;
   const char* msg = fft_plans_create(&c->fft, c->k.geo, c->k.prec, c->k.gauge, c->k.stream, &work);
@@ -475,6 +486,81 @@ int gf_fix_fft(gf_ctx* c, double alpha, double eps, int max_iters, int check_eve
     if (rc != GF_OK) return rc;
     record();
   }
+  return GF_OK;
+}
+
+// ---- T-slab sharding --------------------------------------------------------------------------------
+size_t gf_slab_halo_bytes(const gf_ctx* c) { return c ? c->halo_bytes : 0; }
+
+int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
+  if (!c) return GF_EINVAL;
+  if (!dev_halo) return fail(c, GF_EINVAL, "gf_slab_attach: null workspace");
+  if (bytes < 4 * c->halo_bytes || ((uintptr_t)dev_halo % ALIGN))
+    return fail(c, GF_ENOMEM, "gf_slab_attach: workspace too small or misaligned");
+  if (c->fft_w) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: Algorithm 2 is attached to this context");
+  char* base = (char*)dev_halo;
+  c->k.slab.ghost = base;  // ghost[0], ghost[1]
+  c->top_out = base + 2 * c->halo_bytes;
+  c->top_in = base + 3 * c->halo_bytes;
+  c->qblocks = 0;
+  return GF_OK;
+}
+
+static int slab_check(gf_ctx* c, int parity, const char* who) {
+  if (!c) return GF_EINVAL;
+  if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_*: no halo workspace attached (gf_slab_attach)");
+  if (parity != 0 && parity != 1) return fail(c, GF_EINVAL, who);
+  return GF_OK;
+}
+
+int gf_slab_pack_top(gf_ctx* c, int parity) {
+  int rc = slab_check(c, parity, "gf_slab_pack_top: parity must be 0 or 1");
+  if (rc != GF_OK) return rc;
+  cudaError_t e = launch_slab_top(c->k, parity, c->top_out, true);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_pack_top");
+  c->launches += 1;
+  return GF_OK;
+}
+
+int gf_slab_unpack_top(gf_ctx* c, int parity) {
+  int rc = slab_check(c, parity, "gf_slab_unpack_top: parity must be 0 or 1");
+  if (rc != GF_OK) return rc;
+  cudaError_t e = launch_slab_top(c->k, parity, c->top_in, false);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_unpack_top");
+  c->launches += 1;
+  c->qblocks = 0;
+  return GF_OK;
+}
+
+int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
+  int rc = slab_check(c, parity, "gf_slab_halfsweep_border: parity must be 0 or 1");
+  if (rc != GF_OK) return rc;
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_border: omega outside [1,2)");
+  const Geo& g = c->k.geo;
+  cudaError_t e;
+  if (g.n[3] == 2) {  // both slices are border
+    e = launch_halfsweep_slab(c->k, parity, omega, 0, g.vh);
+    c->launches += 1;
+  } else {
+    e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3);
+    if (e == cudaSuccess) e = launch_halfsweep_slab(c->k, parity, omega, g.vh - g.s3, g.vh);
+    c->launches += 2;
+  }
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_border");
+  c->qblocks = 0;
+  return gf_slab_pack_top(c, parity);
+}
+
+int gf_slab_halfsweep_interior(gf_ctx* c, int parity, double omega) {
+  int rc = slab_check(c, parity, "gf_slab_halfsweep_interior: parity must be 0 or 1");
+  if (rc != GF_OK) return rc;
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_interior: omega outside [1,2)");
+  const Geo& g = c->k.geo;
+  if (g.n[3] == 2) return GF_OK;
+  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, g.s3, g.vh - g.s3);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_interior");
+  c->launches += 1;
+  c->qblocks = 0;
   return GF_OK;
 }
 

@@ -6,6 +6,13 @@
 
 namespace gf {
 
+// A context that is one T-slab of a taller lattice (gf_slab_*): see ghost_link in gf_kernels.cu for the buffer layout.
+struct SlabView {
+  void* ghost;           // two parities of nblk3 tiles; nullptr: the lattice is periodic in t (not a slab)
+  int nblk3;             // ceil(s3 / 32): tiles per parity of one time slice
+  int cb_begin, cb_end;  // checkerboard range of a half-sweep launch
+};
+
 struct KernelArgs {
   void* links;     // internal-layout link field (device)
   void* partials;  // double2 per measure block (device)
@@ -19,6 +26,7 @@ struct KernelArgs {
   int gauge;    // 0 = Landau, 1 = Coulomb
   int variant;  // half-sweep kernel variant (GF_OPT_SWEEP_VARIANT)
   int block_threads;
+  SlabView slab;
 };
 
 // canonical <-> internal for the lexicographic site range [lex_begin, lex_end).  If chunk_base is non-null the canonical
@@ -29,6 +37,10 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
 // halfsweep_can_fuse_theta(a) holds; *qblocks = 0 otherwise)
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks);
 bool halfsweep_can_fuse_theta(const KernelArgs& a);
+// T-slab: the sites [cb_begin, cb_end) of `parity` (staged kernel; t = 0 sites use a.slab.ghost)
+cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end);
+// U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
+cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);
 // 1 kernel launch on small grids (the last block to finish does the second stage), else 2.  nq > 0: a.qpartials[0..nq) hold the odd sites' theta terms of the links as they stand, so only
 // the even sites are visited (every link read once); nq = 0: all sites are visited.

@@ -163,6 +163,14 @@ __device__ __forceinline__ void site_pointers(C* __restrict__ links, const Geo& 
   for (int mu = 0; mu < 4; ++mu) bwd[mu] = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
 }
 
+// T-slab sharding (gf_slab_*): the context is one slab of a taller lattice; U_t(x - t) of its t = 0
+// sites belongs to the lower neighbour and lives, for the duration of a half-sweep, in the ghost buffer
+//   ghost[parity of the owning site][cb3 / 32][elem][cb3 % 32],   cb3 = checkerboard index within the time slice.
+template <class T, int NELEM, class C>
+__device__ __forceinline__ C* ghost_link(const SlabView& sv, int owner_parity, int cb3) {
+  return (C*)sv.ghost + (((size_t)owner_parity * sv.nblk3 + (size_t)(cb3 >> 5)) * NELEM) * 32 + (cb3 & 31);
+}
+
 __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
@@ -256,22 +264,26 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
 // MEASURE: the launch also leaves, per block, the sum over its sites of sum_ij |Delta_ij(x)|^2 AFTER the update, taken
 // from K_final(x) = G(x) K(x), which is K(x) of the updated links (the site's own update is the last one to touch
 // them in this half-sweep).  After the odd half-sweep these are the odd sites' terms of theta of the finished sweep.
-template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE>
+// SLAB: the launch covers the checkerboard range [sv.cb_begin, sv.cb_end) of a T-slab; t = 0 sites take U_t(x - t) from
+// (and return it to) the ghost buffer.  The per-site arithmetic is the same instruction sequence in both cases.
+template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
-ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
+ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials,
+                            SlabView sv) {
   using C = cplx_t<T>;
   using TK = RotationType;
   using CK = cplx_t<TK>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C* sm = reinterpret_cast<C*>(smem_raw) + threadIdx.x;
-  const int cb = blockIdx.x * THREADS + threadIdx.x;
-  const bool live = cb < g.vh;
+  const int cb = (SLAB ? sv.cb_begin : 0) + blockIdx.x * THREADS + threadIdx.x;
+  const bool live = cb < (SLAB ? sv.cb_end : g.vh);
   if (!MEASURE && !live) return;
   double q = 0.0;
   if (live) {
     C* fwd;
     C* bwd[4];
     site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
+    if (SLAB && cb < g.s3) bwd[3] = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
 
     // links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu)
 #pragma unroll
@@ -331,7 +343,7 @@ template <class T, int NELEM, int ND, int THREADS, bool MEASURE>
 static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
-  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE>;
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false>;
   static bool attr_set = false;  // per instantiation
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
@@ -339,7 +351,28 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{});
+  return cudaGetLastError();
+}
+
+// the sites [cb_begin, cb_end) of one parity of a T-slab
+template <class T, int NELEM, int ND>
+static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end) {
+  using C = cplx_t<T>;
+  constexpr int THREADS = staged_threads<T>();
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  if (cb_end <= cb_begin) return cudaSuccess;
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  SlabView sv = a.slab;
+  sv.cb_begin = cb_begin; sv.cb_end = cb_end;
+  const unsigned blocks = (unsigned)((cb_end - cb_begin + THREADS - 1) / THREADS);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv);
   return cudaGetLastError();
 }
 
@@ -388,6 +421,41 @@ cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool
   GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
 }
 
+cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end) {
+  GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end);
+}
+
+// ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------
+// One thread per site of the slice: U_t(x) of the `parity` sites of slice n_t - 1, element by element (both sides are
+// 32-lane runs of one element, so reads and writes are full sectors).
+template <class T, int NELEM, bool PACK>
+__global__ void __launch_bounds__(256) slab_top_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity,
+                                                       cplx_t<T>* __restrict__ buf) {
+  using C = cplx_t<T>;
+  const int cb3 = blockIdx.x * 256 + threadIdx.x;
+  if (cb3 >= g.s3) return;
+  C* l = links + link_offset<NELEM>(g, parity, g.s3 * (g.n[3] - 1) + cb3, 3);
+  C* b = buf + ((size_t)(cb3 >> 5) * NELEM) * 32 + (cb3 & 31);
+#pragma unroll
+  for (int e = 0; e < NELEM; ++e) {
+    if (PACK) b[e * 32] = l[e * 32];
+    else l[e * 32] = b[e * 32];
+  }
+}
+
+template <class T, int NELEM>
+static cudaError_t slab_top_T(const KernelArgs& a, int parity, void* buf, bool pack) {
+  const unsigned blocks = (unsigned)((a.geo.s3 + 255) / 256);
+  if (pack) slab_top_kernel<T, NELEM, true><<<blocks, 256, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, parity, (cplx_t<T>*)buf);
+  else slab_top_kernel<T, NELEM, false><<<blocks, 256, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, parity, (cplx_t<T>*)buf);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack) {
+  if (a.prec == 0) return a.storage == 18 ? slab_top_T<double, 9>(a, parity, buf, pack) : slab_top_T<double, 6>(a, parity, buf, pack);
+  return a.storage == 18 ? slab_top_T<float, 9>(a, parity, buf, pack) : slab_top_T<float, 6>(a, parity, buf, pack);
+}
+
 bool halfsweep_can_fuse_theta(const KernelArgs& a) { return a.variant == 0 || a.variant == 3; }
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
@@ -432,10 +500,11 @@ __device__ __forceinline__ void measure_tail(const double2* __restrict__ partial
   }
 }
 
-template <class T, int NELEM, int ND>
+template <class T, int NELEM, int ND, bool SLAB>
 __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const cplx_t<T>* __restrict__ links, Geo g,
                                                                           int blocks_per_parity,
-                                                                          double2* __restrict__ partials, MeasureTail tail) {
+                                                                          double2* __restrict__ partials, MeasureTail tail,
+                                                                          SlabView sv) {
   using C = cplx_t<T>;
   const int parity = blockIdx.x >= blocks_per_parity;
   const int cb = (blockIdx.x - parity * blocks_per_parity) * MEASURE_THREADS + threadIdx.x;
@@ -450,7 +519,9 @@ __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const 
 #pragma unroll
     for (int nu = 0; nu < ND; ++nu) {
       C u[9];
-      load_link<NELEM, true>(links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu), u);
+      const C* down = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu);
+      if (SLAB && nu == 3 && cb < g.s3) down = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
+      load_link<NELEM, true>(down, u);
 #pragma unroll
       for (int e = 0; e < 9; ++e) { A[e].x += u[e].x; A[e].y += u[e].y; }
       tr += u[0].x + u[4].x + u[8].x;
@@ -503,8 +574,12 @@ static cudaError_t measure_T(const KernelArgs& a, int nq) {
   const bool single = nblk <= MEASURE_SINGLE_LAUNCH_MAX_BLOCKS;
   const MeasureTail tail{single ? (unsigned*)a.counter : nullptr, bpp, (const double*)a.qpartials, nq,
                          1.0 / (ND * 3.0 * V), 1.0 / (3.0 * V), (double*)a.result};
-  measure_partial_kernel<T, NELEM, ND><<<nblk, MEASURE_THREADS, 0, a.stream>>>((const cplx_t<T>*)a.links, a.geo, bpp,
-                                                                              (double2*)a.partials, tail);
+  if (a.slab.ghost)
+    measure_partial_kernel<T, NELEM, ND, true><<<nblk, MEASURE_THREADS, 0, a.stream>>>(
+        (const cplx_t<T>*)a.links, a.geo, bpp, (double2*)a.partials, tail, a.slab);
+  else
+    measure_partial_kernel<T, NELEM, ND, false><<<nblk, MEASURE_THREADS, 0, a.stream>>>(
+        (const cplx_t<T>*)a.links, a.geo, bpp, (double2*)a.partials, tail, SlabView{});
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess || single) return e;
   measure_tail_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, tail);

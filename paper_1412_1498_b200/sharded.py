@@ -1,0 +1,311 @@
+"""T-slab sharding of the overrelaxation sweep over several GPUs (include/gf.h "T-slab sharding").
+
+The lattice nx*ny*nz*nt is cut along t into `n_slabs` slabs of lt = nt/n_slabs time slices (lt even).  Every slab is a
+libgf context with a halo workspace attached; all arithmetic (border / interior half-sweeps, packing and scattering of
+the top-slice temporal links, F and theta) runs in libgf's kernels.  This module is the plumbing between them: which
+buffer goes to which neighbour and when, on which stream, over which transport
+
+  * slabs owned by the same process: device-to-device copies,
+  * slabs owned by different processes (one process per GPU): torch.distributed send / recv (NCCL on GPUs),
+
+and the driver loop of Algorithm 1 around it (the one data-path collective: an all-gather of each slab's F and theta).
+
+Per half-sweep of parity p (include/gf.h steps 1-4), for every local slab s with lower neighbour s-1 and upper s+1:
+    border(p)    -> ghost[1-p] updated in place, top_out = top-slice U_t of the parity-p sites
+    interior(p)  -> overlaps with the transport, which runs on its own stream
+    ghost[1-p] --"ret"--> top_in of slab s-1          top_out --"fwd"--> ghost[p] of slab s+1
+    unpack_top(1-p)
+"""
+from __future__ import annotations
+
+import contextlib
+
+from . import binding as _b
+
+
+# ---- one slab on a GPU ------------------------------------------------------------------------------------------------------
+class GpuSlabEngine:
+    """A libgf context on the local lattice (nx, ny, nz, lt) with its halo workspace.  Marshals arguments only."""
+
+    def __init__(self, local_dims, gauge, prec, storage, device, stream=None):
+        import torch
+
+        self.torch = torch
+        self.fx = _b.GaugeFixer(local_dims, gauge=gauge, prec=prec, storage=storage, device=device, stream=stream)
+        self.device = self.fx.device
+        self.stream = self.fx.stream
+        B = _b.gf_slab_halo_bytes(self.fx.ctx)
+        self.halo_bytes = B
+        with torch.cuda.device(self.device):
+            self.halo = torch.zeros(4 * B, dtype=torch.uint8, device=self.device)
+        self.fx._check(_b.gf_slab_attach(self.fx.ctx, self.halo.data_ptr(), 4 * B))
+        self.ghost = [self.halo[0:B], self.halo[B:2 * B]]
+        self.top_out = self.halo[2 * B:3 * B]
+        self.top_in = self.halo[3 * B:4 * B]
+
+    def set_links(self, links):
+        self.fx.set_links(links)
+
+    def get_links(self, out=None):
+        return self.fx.get_links(out)
+
+    def pack_top(self, parity):
+        self.fx._check(_b.gf_slab_pack_top(self.fx.ctx, int(parity)))
+
+    def unpack_top(self, parity):
+        self.fx._check(_b.gf_slab_unpack_top(self.fx.ctx, int(parity)))
+
+    def border(self, parity, omega):
+        self.fx._check(_b.gf_slab_halfsweep_border(self.fx.ctx, int(parity), float(omega)))
+
+    def interior(self, parity, omega):
+        self.fx._check(_b.gf_slab_halfsweep_interior(self.fx.ctx, int(parity), float(omega)))
+
+    def measure(self):
+        return self.fx.measure()
+
+    def reunitarize(self):
+        self.fx.reunitarize()
+
+    def kernel_launches(self):
+        return self.fx.kernel_launches()
+
+    # stream hand-offs between the compute stream of this slab and the process's transport stream
+    def mark(self):
+        ev = self.torch.cuda.Event()
+        ev.record(self.stream)
+        return ev
+
+    def wait(self, event):
+        if event is not None:
+            self.stream.wait_event(event)
+
+    def close(self):
+        self.fx.close()
+
+
+# ---- who owns which slab ---------------------------------------------------------------------------------------------------
+def slab_owner(slab: int, n_slabs: int, world: int) -> int:
+    """Slabs are dealt to the ranks in contiguous runs of n_slabs / world (neighbouring slabs on the same or the next GPU)."""
+    return slab // (n_slabs // world)
+
+
+def local_slabs(rank: int, n_slabs: int, world: int):
+    k = n_slabs // world
+    return list(range(rank * k, (rank + 1) * k))
+
+
+def halo_messages(p: int, slabs, n_slabs: int):
+    """The messages of one half-sweep of parity p that involve the given slabs, as (kind, src_slab, dst_slab):
+    "ret": ghost[1-p] of src -> top_in of dst = src - 1;   "fwd": top_out of src -> ghost[p] of dst = src + 1.
+    (p does not change who talks to whom, only which ghost buffer is meant.)"""
+    out = []
+    for s in slabs:
+        out.append(("ret", s, (s - 1) % n_slabs))
+        out.append(("fwd", s, (s + 1) % n_slabs))
+        out.append(("ret", (s + 1) % n_slabs, s))
+        out.append(("fwd", (s - 1) % n_slabs, s))
+    # One global order (kind, destination) on every rank: between any two ranks the sends are posted in the order the
+    # matching receives are, which is what a tag-less transport (NCCL) matches by.
+    return sorted(set(out), key=lambda m: (m[0], m[2]))
+
+
+def message_tag(kind: str, dst_slab: int) -> int:
+    return 2 * dst_slab + (1 if kind == "fwd" else 0)
+
+
+class ShardedGaugeFixer:
+    """Overrelaxation gauge fixing of one lattice spread over n_slabs T-slabs.
+
+    dims: the GLOBAL lattice (nx, ny, nz, nt).  With torch.distributed initialised every rank constructs the same object
+    and owns n_slabs / world_size consecutive slabs; without it (or with group=False) all slabs live in this process.
+    engine_factory(local_dims, slab_index) builds one slab (default: GpuSlabEngine on `device`).
+    """
+
+    def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
+                 engine_factory=None):
+        import torch
+
+        self.torch = torch
+        self.dims = tuple(int(d) for d in dims)
+        self.n_slabs = int(n_slabs)
+        nx, ny, nz, nt = self.dims
+        if self.n_slabs < 1 or nt % self.n_slabs or (nt // self.n_slabs) % 2 or nt // self.n_slabs < 2:
+            raise ValueError("nt must split into n_slabs slabs of an even number (>= 2) of time slices")
+        self.local_dims = (nx, ny, nz, nt // self.n_slabs)
+        self.local_volume = nx * ny * nz * (nt // self.n_slabs)
+        self.dist = None
+        self.group = None
+        self.rank, self.world = 0, 1
+        if group is not False:
+            import torch.distributed as dist
+
+            if dist.is_available() and dist.is_initialized():
+                self.dist, self.group = dist, group
+                self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        if self.n_slabs % self.world:
+            raise ValueError("n_slabs must be a multiple of the number of ranks")
+        self.slabs = local_slabs(self.rank, self.n_slabs, self.world)
+        self.device = torch.device(device) if device is not None else torch.device("cpu")
+        self.on_gpu = self.device.type == "cuda"
+        if engine_factory is None:
+            def engine_factory(local_dims, slab):
+                return GpuSlabEngine(local_dims, gauge, prec, storage, self.device)
+        self.engines = {s: engine_factory(self.local_dims, s) for s in self.slabs}
+        self.comm_stream = None
+        if self.on_gpu:
+            with torch.cuda.device(self.device):
+                self.comm_stream = torch.cuda.Stream(self.device)
+        self.reunit_every = 0
+        self.sweeps_total = 0
+        self.messages_sent = 0  # remote (torch.distributed) messages posted by this rank
+        self.copies = 0         # local device-to-device copies
+
+    # ---- transport ------------------------------------------------------------------------------------------------------
+    def _buffer(self, kind, end, slab, p):
+        e = self.engines[slab]
+        if kind == "ret":
+            return e.ghost[1 - p] if end == "src" else e.top_in
+        return e.top_out if end == "src" else e.ghost[p]
+
+    def _exchange(self, p, kinds=("ret", "fwd"), after=None):
+        """Move this half-sweep's messages on the transport stream.  `after`: events the transport waits for (default:
+        everything queued so far on the local compute streams).  On return every local compute stream waits for the
+        transport, so neither a source nor a destination buffer is touched by a later kernel before it is done."""
+        torch = self.torch
+        ctx = contextlib.nullcontext()
+        if self.on_gpu:
+            for ev in (after if after is not None else [self.engines[s].mark() for s in self.slabs]):
+                self.comm_stream.wait_event(ev)
+            ctx = torch.cuda.stream(self.comm_stream)
+        with ctx:
+            ops = []
+            for kind, src, dst in halo_messages(p, self.slabs, self.n_slabs):
+                if kind not in kinds:
+                    continue
+                src_local, dst_local = src in self.engines, dst in self.engines
+                if src_local and dst_local:
+                    self._buffer(kind, "dst", dst, p).copy_(self._buffer(kind, "src", src, p), non_blocking=True)
+                    self.copies += 1
+                elif src_local:
+                    peer = self._global_rank(slab_owner(dst, self.n_slabs, self.world))
+                    ops.append(self.dist.P2POp(self.dist.isend, self._buffer(kind, "src", src, p), peer, self.group,
+                                               message_tag(kind, dst)))
+                    self.messages_sent += 1
+                elif dst_local:
+                    peer = self._global_rank(slab_owner(src, self.n_slabs, self.world))
+                    ops.append(self.dist.P2POp(self.dist.irecv, self._buffer(kind, "dst", dst, p), peer, self.group,
+                                               message_tag(kind, dst)))
+            if ops:
+                for req in self.dist.batch_isend_irecv(ops):
+                    req.wait()
+        if self.on_gpu:
+            done = torch.cuda.Event()
+            done.record(self.comm_stream)
+            for s in self.slabs:
+                self.engines[s].wait(done)
+
+    def _global_rank(self, group_rank):
+        if self.group is None:
+            return group_rank
+        return self.dist.get_global_rank(self.group, group_rank)
+
+    def refresh_ghosts(self):
+        """Fill both ghost buffers of every slab from its lower neighbour's top slice (after set_links, reunitarize)."""
+        for q in (0, 1):
+            for s in self.slabs:
+                self.engines[s].pack_top(q)
+            self._exchange(q, kinds=("fwd",))
+
+    # ---- links in / out ---------------------------------------------------------------------------------------------------
+    def set_links(self, links_by_slab):
+        """links_by_slab: {slab: canonical (V_local,4,3,3,2) tensor} for the local slabs."""
+        for s in self.slabs:
+            self.engines[s].set_links(links_by_slab[s])
+        self.sweeps_total = 0
+        self.refresh_ghosts()
+
+    def set_links_global(self, links):
+        """links: the canonical array of the WHOLE lattice (t is the slowest index, so a slab is a contiguous run of sites)."""
+        V = self.local_volume
+        self.set_links({s: links[s * V:(s + 1) * V].contiguous() for s in self.slabs})
+
+    def get_links(self):
+        return {s: self.engines[s].get_links() for s in self.slabs}
+
+    # ---- Algorithm 1 ---------------------------------------------------------------------------------------------------------
+    def half_sweep(self, p, omega):
+        for s in self.slabs:
+            self.engines[s].border(p, omega)
+        # the transport starts as soon as the border kernels are done, beside the interior kernels queued behind them
+        after = [self.engines[s].mark() for s in self.slabs] if self.on_gpu else None
+        for s in self.slabs:
+            self.engines[s].interior(p, omega)
+        self._exchange(p, after=after)
+        for s in self.slabs:
+            self.engines[s].unpack_top(1 - p)
+
+    def reunitarize(self):
+        for s in self.slabs:
+            self.engines[s].reunitarize()
+        self.refresh_ghosts()
+
+    def set_reunit_every(self, k):
+        self.reunit_every = int(k)
+
+    def ovr_sweep(self, n, omega):
+        """n sweeps, even half-sweep first; reunitarisation cadence as gf_ovr_sweep."""
+        if not (1.0 <= omega < 2.0):
+            raise ValueError("omega outside [1,2)")
+        for _ in range(int(n)):
+            self.half_sweep(0, omega)
+            self.half_sweep(1, omega)
+            self.sweeps_total += 1
+            if self.reunit_every > 0 and self.sweeps_total % self.reunit_every == 0:
+                self.reunitarize()
+
+    def measure(self):
+        """Global F and theta: the mean over all slabs (equal volumes) of each slab's gf_measure, added in slab order on
+        every rank, so all ranks take the same stop decision."""
+        torch = self.torch
+        local = torch.tensor([list(self.engines[s].measure()) for s in self.slabs], dtype=torch.float64)
+        if self.world > 1:
+            # gf_measure's results are host numbers; NCCL moves device memory only
+            buf = local.to(self.device) if self.on_gpu else local
+            parts = [torch.empty_like(buf) for _ in range(self.world)]
+            self.dist.all_gather(parts, buf, group=self.group)
+            local = torch.cat(parts).cpu()
+        F = theta = 0.0
+        for row in local.tolist():
+            F += row[0]
+            theta += row[1]
+        return F / self.n_slabs, theta / self.n_slabs
+
+    def fix(self, omega, eps, max_sweeps, check_every):
+        """Algorithm 1 with a measurement cadence (as gf_fix).  Returns (sweeps_done, [(sweep, F, theta), ...])."""
+        if check_every < 1 or max_sweeps < 0 or not eps >= 0.0:
+            raise ValueError("need check_every >= 1, max_sweeps >= 0, eps >= 0")
+        done = 0
+        F, th = self.measure()
+        history = [(0, F, th)]
+        while not th < eps and done < max_sweeps:
+            n = min(check_every, max_sweeps - done)
+            self.ovr_sweep(n, omega)
+            done += n
+            F, th = self.measure()
+            history.append((done, F, th))
+        return done, history
+
+    def kernel_launches(self):
+        return sum(e.kernel_launches() for e in self.engines.values())
+
+    def synchronize(self):
+        if self.on_gpu:
+            for e in self.engines.values():
+                e.stream.synchronize()
+            self.comm_stream.synchronize()
+
+    def close(self):
+        for e in self.engines.values():
+            e.close()
+        self.engines = {}
