@@ -454,6 +454,95 @@ def run_fftsd(args):
     return 0
 
 
+def run_sharded(args):
+    """--sharded K: the overrelaxation sweep over T-slabs (paper_1412_1498_b200.sharded; SURVEY.md §8(f) NEXT-2,
+    PAPER.md:132-134).  Every rank holds the config's lattice as K slabs; the global lattice is world x taller (fixed
+    local volume per GPU, the paper's weak-scaling set-up).  Secondary line: with one rank the halo
+    messages are device-to-device copies and the number is the cost of the border / interior split on one GPU."""
+    import torch
+
+    import gf_inputs as gi
+    import paper_1412_1498_b200 as gf
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = get_cfg(args.config)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    K = args.sharded
+    gdims = (dims[0], dims[1], dims[2], dims[3] * world)
+    n_slabs = K * world
+    V = gi.volume(dims)
+    L = LINK_BYTES[(prec, storage)]
+    n_sw, omega = cfg["check_every"], cfg["omega"]
+    sh = gf.ShardedGaugeFixer(gdims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
+    sh.set_reunit_every(cfg["reunit_every"])
+    links = {}
+    for s in sh.slabs:  # every slab its own seeded field of the config's recipe (rougher across slab boundaries)
+        e = sh.engines[s]
+        buf = e.fx.new_links_buffer()
+        gi.make_links_device(buf.data_ptr(), sh.local_dims, cfg["roughness"], cfg["seed"] + 1000 * s, prec,
+                             torch.cuda.current_stream().cuda_stream)
+        links[s] = buf
+    sh.set_links(links)
+    del links, buf
+    torch.cuda.synchronize()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        sh.ovr_sweep(n_sw, omega)
+        sh.measure()
+    barrier()
+    l0 = sh.kernel_launches()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        sh.ovr_sweep(n_sw, omega)
+        F, th = sh.measure()
+    t1.record()
+    barrier()
+    ms = max_over_ranks(t0.elapsed_time(t1), dist, f"cuda:{local}")
+    clocks = sampler.stop() if sampler else None
+    if rank == 0:
+        peak, peak_src = load_peaks()
+        value = aggregate_value(world, V, n_sw * args.steps, ms)
+        gbs = value / world * 16 * L / 1e9  # per GPU and site-update: 8 links read and written
+        halo = sum(e.halo_bytes for e in sh.engines.values())
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": prec, "data": "synthetic",
+                "config": {"workload": workload_name(cfg) + f" per GPU; global lattice {gdims[0]}x{gdims[1]}x{gdims[2]}x{gdims[3]}",
+                           "step": f"{n_sw} sweeps + 1 F/theta measurement",
+                           "parallelism": f"T-slabs: {n_slabs} slabs over {world} rank(s), {K} per rank",
+                           "halo": f"2 messages of {halo // len(sh.engines)} B per slab and half-sweep "
+                                   f"({'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
+                           "l2": "inputs exceed L2" if 4 * V * L > 126e6 else "field fits L2 in part",
+                           "final_F": F, "final_theta": th},
+                "roofline": {"bound": "hbm", "kernel": "ovr_halfsweep_staged_kernel (border + interior launches)",
+                             "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                             "peak_source": peak_src, "note": "whole step incl. halo traffic and measurement"},
+                "gpu_launches": int(sh.kernel_launches() - l0), "halo_copies": sh.copies,
+                "halo_messages_sent": sh.messages_sent, "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    sh.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -468,9 +557,13 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-contract", action="store_true", help="skip the timed whole-config gf_fix run")
     ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
+    ap.add_argument("--sharded", type=int, default=0, metavar="K",
+                    help="T-slab sharded sweep with K slabs per rank (secondary line; default 0 = single context / replicas)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
     if args.algo == "fftsd":
         return run_fftsd(args)
     return run_ours(args)

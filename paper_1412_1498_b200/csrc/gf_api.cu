@@ -137,7 +137,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
-  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0};
+  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr};
   c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
   c->top_out = c->top_in = nullptr;
   c->host_result = nullptr;
@@ -537,18 +537,12 @@ int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
   if (rc != GF_OK) return rc;
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_border: omega outside [1,2)");
   const Geo& g = c->k.geo;
-  cudaError_t e;
-  if (g.n[3] == 2) {  // both slices are border
-    e = launch_halfsweep_slab(c->k, parity, omega, 0, g.vh);
-    c->launches += 1;
-  } else {
-    e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3);
-    if (e == cudaSuccess) e = launch_halfsweep_slab(c->k, parity, omega, g.vh - g.s3, g.vh);
-    c->launches += 2;
-  }
+  // one launch: bottom slice, top slice; the top-slice sites also write their updated U_t(x) into top_out
+  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3, g.vh - g.s3, g.vh, c->top_out);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_border");
+  c->launches += 1;
   c->qblocks = 0;
-  return gf_slab_pack_top(c, parity);
+  return GF_OK;
 }
 
 int gf_slab_halfsweep_interior(gf_ctx* c, int parity, double omega) {
@@ -557,7 +551,7 @@ int gf_slab_halfsweep_interior(gf_ctx* c, int parity, double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_interior: omega outside [1,2)");
   const Geo& g = c->k.geo;
   if (g.n[3] == 2) return GF_OK;
-  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, g.s3, g.vh - g.s3);
+  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, g.s3, g.vh - g.s3, 0, 0, nullptr);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_interior");
   c->launches += 1;
   c->qblocks = 0;

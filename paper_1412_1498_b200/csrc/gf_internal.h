@@ -10,7 +10,10 @@ namespace gf {
 struct SlabView {
   void* ghost;           // two parities of nblk3 tiles; nullptr: the lattice is periodic in t (not a slab)
   int nblk3;             // ceil(s3 / 32): tiles per parity of one time slice
-  int cb_begin, cb_end;  // checkerboard range of a half-sweep launch
+  int cb_begin, cb_end;  // checkerboard range of a half-sweep launch ...
+  int nblocks0;          // ... covered by the first nblocks0 blocks; the remaining blocks cover
+  int cb2_begin, cb2_end;  //     a second range (border launch: bottom and top slice in one grid)
+  void* top_out;         // non-null: top-slice sites also leave their updated U_t(x) here (message layout)
 };
 
 struct KernelArgs {
@@ -37,8 +40,10 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
 // halfsweep_can_fuse_theta(a) holds; *qblocks = 0 otherwise)
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks);
 bool halfsweep_can_fuse_theta(const KernelArgs& a);
-// T-slab: the sites [cb_begin, cb_end) of `parity` (staged kernel; t = 0 sites use a.slab.ghost)
-cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end);
+// T-slab: the sites [cb_begin, cb_end) and [cb2_begin, cb2_end) of `parity` in one launch (staged kernel; t = 0 sites
+// use a.slab.ghost; with top_out the top-slice sites also write their updated U_t(x) there)
+cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
+                                  int cb2_begin, int cb2_end, void* top_out);
 // U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
 cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);

@@ -275,8 +275,13 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   using CK = cplx_t<TK>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C* sm = reinterpret_cast<C*>(smem_raw) + threadIdx.x;
-  const int cb = (SLAB ? sv.cb_begin : 0) + blockIdx.x * THREADS + threadIdx.x;
-  const bool live = cb < (SLAB ? sv.cb_end : g.vh);
+  int cb = blockIdx.x * THREADS + threadIdx.x;
+  bool live = cb < g.vh;
+  if (SLAB) {
+    const bool second = (int)blockIdx.x >= sv.nblocks0;
+    cb = second ? sv.cb2_begin + (blockIdx.x - sv.nblocks0) * THREADS + threadIdx.x : sv.cb_begin + cb;
+    live = cb < (second ? sv.cb2_end : sv.cb_end);
+  }
   if (!MEASURE && !live) return;
   double q = 0.0;
   if (live) {
@@ -325,6 +330,11 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
       mul_left<NELEM / 3>(G, u, w);                       // U_mu(x) <- G U_mu(x)
       store_link<NELEM>(fwd + mu * NELEM * 32, w);
+      if (SLAB && mu == 3 && sv.top_out && cb >= g.vh - g.s3) {  // top slice: the copy that goes to the upper neighbour
+        SlabView out = sv;
+        out.ghost = sv.top_out;
+        store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb - (g.vh - g.s3)), w);
+      }
       sched_fence();
       load_link_smem<NELEM, THREADS, false>(sm, 2 * mu + 1, u);
       mul_right_adj<NELEM / 3>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
@@ -357,11 +367,12 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
 
 // the sites [cb_begin, cb_end) of one parity of a T-slab
 template <class T, int NELEM, int ND>
-static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end) {
+static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
+                                    int cb2_begin, int cb2_end, void* top_out) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
-  if (cb_end <= cb_begin) return cudaSuccess;
+  if (cb_end <= cb_begin && cb2_end <= cb2_begin) return cudaSuccess;
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
   static bool attr_set = false;  // per instantiation
   if (!attr_set) {
@@ -371,7 +382,10 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   }
   SlabView sv = a.slab;
   sv.cb_begin = cb_begin; sv.cb_end = cb_end;
-  const unsigned blocks = (unsigned)((cb_end - cb_begin + THREADS - 1) / THREADS);
+  sv.cb2_begin = cb2_begin; sv.cb2_end = cb2_end;
+  sv.nblocks0 = cb_end > cb_begin ? (cb_end - cb_begin + THREADS - 1) / THREADS : 0;
+  sv.top_out = top_out;
+  const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv);
   return cudaGetLastError();
 }
@@ -421,8 +435,9 @@ cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool
   GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
 }
 
-cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end) {
-  GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end);
+cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
+                                  int cb2_begin, int cb2_end, void* top_out) {
+  GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end, cb2_begin, cb2_end, top_out);
 }
 
 // ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------
