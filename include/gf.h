@@ -112,9 +112,13 @@ enum {
                                and reads every link once; 0: gf_measure always visits all sites */
   GF_OPT_FFT_ACCELERATE = 4, /* 1 (default): gf_fft_step / gf_fix_fft use the Fourier factor of eq. 1.8; 0: the naive
                                steepest descent of eq. 1.7 (no transforms) */
-  GF_OPT_FFT_FUSED_T = 5    /* 1: in Landau gauge with n_t a power of two (<= 256) the transform along t, the Fourier
+  GF_OPT_FFT_FUSED_T = 5,   /* 1: in Landau gauge with n_t a power of two (<= 256) the transform along t, the Fourier
                                factor and the inverse transform along t are one hand-written pass through shared
                                memory; 0 (default): cuFFT's strided 1-D transforms and a separate factor kernel */
+  GF_OPT_FFT_OWN = 6        /* 1 (default): when every transformed extent is a product of two of {1,2,3,4,6,8,12,16}
+                               (<= 256) and an (x,y) plane fits shared memory, the transforms, the Fourier factor and
+                               the inverse transforms run as hand-written passes (5 over the fields in Landau gauge,
+                               3 in Coulomb gauge), without cuFFT; other lattices, or 0: the cuFFT path */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 

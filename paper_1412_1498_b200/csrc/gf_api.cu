@@ -74,6 +74,8 @@ struct gf_ctx {
   double* fft_table;  // 4 sin^2(pi k/n) per direction
   int fft_accelerate; // GF_OPT_FFT_ACCELERATE
   int fft_fused_t;    // GF_OPT_FFT_FUSED_T
+  int fft_own;        // GF_OPT_FFT_OWN
+  double* own_table;  // tables of the hand-written transforms (behind fft_table in the same workspace slot)
   // T-slab sharding (gf_slab_*): the caller's halo workspace once attached
   size_t halo_bytes;  // one message: U_t of one parity of one time slice
   char* top_out;      // packed top-slice links on their way to the upper neighbour's ghost buffer
@@ -135,7 +137,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->fuse_measure = 1; c->qblocks = 0;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
-  c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0;
+  c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0; c->fft_own = 1; c->own_table = nullptr;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
   c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr};
   c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
@@ -264,6 +266,9 @@ int gf_set_option(gf_ctx* c, int key, int value) {
     case GF_OPT_FFT_FUSED_T:
       c->fft_fused_t = value != 0;
       return GF_OK;
+    case GF_OPT_FFT_OWN:
+      c->fft_own = value != 0;
+      return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
       c->k.block_threads = value;
@@ -364,7 +369,8 @@ static int fft_plan(gf_ctx* c) {
   if (msg) return fail(c, GF_ECUDA, msg);
   const size_t csize = c->k.prec == GF_FP64 ? 16 : 8;
   c->fft_w_bytes = align_up((size_t)4 * volume(c) * csize);
-  c->fft_table_bytes = align_up(sd_table_entries(c->k.geo) * sizeof(double));
+  c->fft_table_bytes = align_up(sd_table_entries(c->k.geo) * sizeof(double)) +
+                       align_up(own_fft_table_entries(c->k.geo) * sizeof(double));
   c->fft_work_bytes = align_up(work);
   return GF_OK;
 }
@@ -389,7 +395,9 @@ int gf_fft_attach(gf_ctx* c, void* dev_workspace, size_t workspace_bytes) {
   c->fft_table = (double*)(c->fft_w + c->fft_w_bytes);
   const char* msg = fft_plans_set_work(c->fft, c->fft_w + c->fft_w_bytes + c->fft_table_bytes);
   if (msg) { c->fft_w = nullptr; return fail(c, GF_ECUDA, msg); }
+  c->own_table = (double*)((char*)c->fft_table + align_up(sd_table_entries(c->k.geo) * sizeof(double)));
   cudaError_t e = launch_sd_table(c->k, c->fft_table);
+  if (e == cudaSuccess && own_fft_supported(c->k.geo, c->k.gauge, c->k.prec)) e = launch_own_fft_tables(c->k, c->own_table);
   if (e != cudaSuccess) { c->fft_w = nullptr; return fail_cuda(c, e, "gf_fft_attach"); }
   c->launches += 1;
   return GF_OK;
@@ -400,6 +408,18 @@ static int fft_update(gf_ctx* c, double alpha) {
   int n = 0;
   const char* msg = nullptr;
   cudaError_t e;
+  if (c->fft_accelerate && c->fft_own && own_fft_supported(c->k.geo, c->k.gauge, c->k.prec)) {
+    // hand-written passes: transform, factor and inverse transform without cuFFT (gf_fft.cu)
+    e = launch_own_fft_update(c->k, c->fft_w, c->own_table, alpha, &n);
+    if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (transforms)");
+    e = launch_sd_rotate(c->k, c->fft_w);
+    if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (rotate)");
+    c->launches += n + 1;
+    c->qblocks = 0;
+    c->sweeps_total += 1;
+    if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) return gf_reunitarize(c);
+    return GF_OK;
+  }
   // Landau gauge, n_t a power of two: the t direction (transform, factor, inverse transform) is one fused pass
   const bool fused_t = c->fft_accelerate && c->fft_fused_t && c->k.gauge == GF_LANDAU && sd_tline_supported(c->k.geo);
   if (c->fft_accelerate) msg = fft_exec(c->fft, c->k.geo, c->k.prec, c->fft_w, true, !fused_t, &n);

@@ -67,6 +67,11 @@ const char* fft_exec(FftPlans* p, const Geo& g, int prec, void* w, bool forward,
 bool sd_tline_supported(const Geo& g);
 // forward transform along t, Fourier factor, inverse transform along t in one pass (Landau, n_t a power of two)
 cudaError_t launch_sd_tline(const KernelArgs& a, void* w, const double* table, double alpha);
+// hand-written transforms (gf_fft.cu): forward, Fourier factor, inverse in 5 (Landau) / 3 (Coulomb) passes
+bool own_fft_supported(const Geo& g, int gauge, int prec);
+size_t own_fft_table_entries(const Geo& g);  // doubles: per axis the position-ordered p^2 and the twiddles
+cudaError_t launch_own_fft_tables(const KernelArgs& a, double* table);
+cudaError_t launch_own_fft_update(const KernelArgs& a, void* w, const double* table, double alpha, int* launches);
 size_t sd_table_entries(const Geo& g);  // doubles in the 4 sin^2(pi k/n) table
 int sd_num_partials(const Geo& g);      // <= measure_num_partials(g): a.partials is shared
 cudaError_t launch_sd_table(const KernelArgs& a, double* table);

@@ -150,3 +150,43 @@ def test_fused_t_pass_against_cufft_path_and_oracle(dims, prec):
     tol = TOL_LINK[prec]
     assert np.abs(res[1] - res[0]).max() <= (1e-13 if prec == "f64" else 1e-5)
     assert np.abs(res[1] - Uo).max() <= 2 * tol and np.abs(res[0] - Uo).max() <= 2 * tol
+
+
+# extents: single radix (2..16), two-step powers of two (32, 64), factors of three (6, 12, 24, 48), unequal splits (24 = 6x4)
+OWN_FFT_LATTICES = [(8, 8, 8, 16), (16, 4, 6, 2), (32, 8, 4, 4), (4, 32, 2, 8), (4, 4, 32, 8), (8, 4, 4, 64), (12, 6, 24, 4),
+                    (48, 4, 2, 6), (2, 2, 2, 2), (24, 12, 6, 32), (4, 2, 48, 2), (64, 64, 2, 2)]
+
+
+@pytest.mark.parametrize("dims", OWN_FFT_LATTICES)
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_hand_written_transforms_against_cufft_path_and_oracle(dims, gauge, prec):
+    """GF_OPT_FFT_OWN: plane (x,y) / line z / line t passes with the factor fused (csrc/gf_fft.cu) against the cuFFT path
+    of the same library and against the oracle, two iterations."""
+    U, Uo = make(dims, 0.5, 37, prec, 18)
+    res = {}
+    for own in (1, 0):
+        fx, gf = fixer(dims, gauge, prec, 18, U)
+        fx.set_option(gf.GF_OPT_FFT_OWN, own)
+        l0 = fx.kernel_launches()
+        fx.fft_step(2, 0.08)
+        res[own] = (fx.get_links().cpu().numpy().astype(np.float64), fx.kernel_launches() - l0)
+        fx.close()
+    for _ in range(2):
+        fftsd.step(Uo, dims, gauge, 0.08)
+    tol = TOL_LINK[prec]
+    # the own path is the one that ran: 1 Delta + 5 (3) passes + 1 rotation per iteration, plus the table kernels
+    assert res[1][1] <= 2 * (7 if gauge == "landau" else 5) + 5
+    assert np.abs(res[1][0] - res[0][0]).max() <= (1e-13 if prec == "f64" else 1e-5)
+    assert np.abs(res[1][0] - Uo).max() <= 2 * tol and np.abs(res[0][0] - Uo).max() <= 2 * tol
+
+
+def test_extents_the_hand_written_transforms_do_not_cover_use_cufft():
+    dims = (10, 6, 4, 4)  # 10 = 2 x 5
+    U, Uo = make(dims, 0.5, 38, "f64", 18)
+    fx, gf = fixer(dims, "landau", "f64", 18, U)
+    fx.fft_step(1, 0.08)
+    got = fx.get_links().cpu().numpy()
+    fx.close()
+    fftsd.step(Uo, dims, "landau", 0.08)
+    assert np.abs(got - Uo).max() <= TOL_LINK["f64"]
