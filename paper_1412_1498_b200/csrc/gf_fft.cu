@@ -116,6 +116,16 @@ __device__ __forceinline__ void fft_step(const C* src, size_t sstride, C* dst, s
   for (int m = 0; m < R; ++m) dst[m * dstride] = v[m];
 }
 
+// scale / p2 for the Fourier factor: FP32 reciprocal seed + two Newton steps (full double accuracy, no FP64 division)
+template <class T> __device__ __forceinline__ T factor_of(double scale_p2max, double p2) {
+  if (!(p2 > 0.0)) return T(0);  // p = 0 (reading B3)
+  if (sizeof(T) == 4) return (T)scale_p2max * __frcp_rn((float)p2);
+  double r = (double)__frcp_rn((float)p2);
+  r = r * (2.0 - p2 * r);
+  r = r * (2.0 - p2 * r);
+  return (T)(scale_p2max * r);
+}
+
 #define GF_R_CASES(R, ...)                                         \
   switch (R) {                                                     \
     case 1: { constexpr int RR = 1; __VA_ARGS__; } break;          \
@@ -215,8 +225,7 @@ _Pragma("unroll")
         Dft<T, RR, false>::run(v);
 _Pragma("unroll")
         for (int m = 0; m < RR; ++m) {
-          const double p2 = p2_other + a.p2_axis[m];
-          const T f = p2 > 0.0 ? (T)(a.scale_p2max / p2) : T(0);
+          const T f = factor_of<T>(a.scale_p2max, p2_other + a.p2_axis[m]);
           v[m].x *= f; v[m].y *= f;
         }
         Dft<T, RR, true>::run(v);
@@ -245,8 +254,7 @@ _Pragma("unroll")
           Dft<T, RR, false>::run(v);
 _Pragma("unroll")
           for (int m = 0; m < RR; ++m) {
-            const double p2 = p2_other + a.p2_axis[R2 * k1 + m];
-            const T f = p2 > 0.0 ? (T)(a.scale_p2max / p2) : T(0);
+            const T f = factor_of<T>(a.scale_p2max, p2_other + a.p2_axis[R2 * k1 + m]);
             v[m].x *= f; v[m].y *= f;
           }
           Dft<T, RR, true>::run(v);
@@ -291,24 +299,32 @@ struct PlaneArgs {
 
 template <bool V> struct DirTag { static constexpr bool value = V; };
 
+// 128 threads per block: three blocks (three 66 KB tiles on a 64 x 64 FP64 plane) share an SM, so one block's load and
+// store phases overlap the others' register steps.
+constexpr int PLANE_THREADS = 128;
+
 template <class T, bool INV>
-__global__ void __launch_bounds__(256) fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
+__global__ void __launch_bounds__(PLANE_THREADS, 3) fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
   using C = cplx_t<T>;
   extern __shared__ __align__(16) unsigned char plane_smem[];
   C* tile = reinterpret_cast<C*>(plane_smem);
   const int nx = a.nx, ny = a.ny, row = a.row;
   C* g = w + (size_t)blockIdx.x * nx * ny;
   const int nthreads = blockDim.x;
-  for (int i = threadIdx.x; i < nx * ny; i += nthreads) {
+  for (int i = threadIdx.x; i < nx * ny; i += nthreads) {  // global -> tile without a register round trip
     const int y = i / nx, x = i - y * nx;
-    tile[y * row + x] = g[i];
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(tile + y * row + x);
+    if (sizeof(C) == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(g + i) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(g + i) : "memory");
   }
+  asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
-  // x lines: line y, elements tile[y*row + pos]; work item -> (y, sub) with sub fastest (neighbouring lanes, neighbouring words)
+  // x lines: line y, elements tile[y*row + pos]; work item -> (sub, y) with y fastest: neighbouring lanes are one row
+  // apart, and the row stride is odd, so they fall on different banks whatever the stride along the line is
   auto x_outer = [&](auto inv_tag) {
     constexpr bool I = decltype(inv_tag)::value;
     for (int it = threadIdx.x; it < ny * a.rx2; it += nthreads) {
-      const int y = it / a.rx2, t2 = it - y * a.rx2;
+      const int t2 = it / ny, y = it - t2 * ny;
       C* p = tile + y * row + t2;
       GF_R_CASES(a.rx1, fft_step<T, RR, I, !I>(p, (size_t)a.rx2, p, (size_t)a.rx2, a.twx, t2));
     }
@@ -316,7 +332,7 @@ __global__ void __launch_bounds__(256) fft_plane_kernel(cplx_t<T>* __restrict__ 
   auto x_inner = [&](auto inv_tag) {
     constexpr bool I = decltype(inv_tag)::value;
     for (int it = threadIdx.x; it < ny * a.rx1; it += nthreads) {
-      const int y = it / a.rx1, k1 = it - y * a.rx1;
+      const int k1 = it / ny, y = it - k1 * ny;
       C* p = tile + y * row + a.rx2 * k1;
       GF_R_CASES(a.rx2, fft_step<T, RR, I, I>(p, (size_t)1, p, (size_t)1, a.twx, k1));
     }
@@ -351,6 +367,7 @@ __global__ void __launch_bounds__(256) fft_plane_kernel(cplx_t<T>* __restrict__ 
     if (a.rx2 > 1) { x_inner(Inv{}); __syncthreads(); }
     x_outer(Inv{}); __syncthreads();
   }
+#pragma unroll 4
   for (int i = threadIdx.x; i < nx * ny; i += nthreads) {
     const int y = i / nx, x = i - y * nx;
     g[i] = tile[y * row + x];
@@ -368,12 +385,13 @@ static bool make_shape(const Geo& g, int gauge, FftShape* s) {
   return true;
 }
 
-static int plane_row(int nx) { return nx % 8 == 0 ? nx + 1 : nx; }  // odd row stride: y lines of neighbouring x, x lines of neighbouring y on different banks
+static int plane_row(int nx) { return nx + 1; }  // odd row stride (extents are even): neighbouring rows on different banks
 
 static int line_xb(size_t inner, int n, int r2, size_t csize) {
-  // as many consecutive inner indices as keep the tile <= 64 KB and the block <= 256 threads; at least 128 B per row when possible
+  // consecutive inner indices per block: rows of up to 256 B (two full lines per row), block <= 256 threads; small
+  // tiles (32 KB at n = 128) so that several blocks share an SM and their load / step / store phases overlap
   int xb = 1;
-  while (xb * 2 <= 256 / r2 && inner % (size_t)(xb * 2) == 0 && (size_t)n * (xb * 2) * csize <= 64 * 1024 && xb * 2 <= 32) xb *= 2;
+  while (xb * 2 <= 256 / r2 && inner % (size_t)(xb * 2) == 0 && (size_t)(xb * 2) * csize <= 256) xb *= 2;
   return xb;
 }
 
@@ -411,7 +429,7 @@ static cudaError_t plane_pass(const KernelArgs& a, const FftShape& s, void* w, c
   int items = p.ny * p.rx2;
   if (p.nx * p.ry2 > items) items = p.nx * p.ry2;
   int threads = 32;
-  while (threads < items && threads < 256) threads *= 2;
+  while (threads < items && threads < PLANE_THREADS) threads *= 2;
   cudaError_t e;
   if (inverse) {
     auto k = fft_plane_kernel<T, true>;
