@@ -126,16 +126,18 @@ template <class T> __device__ __forceinline__ T factor_of(double scale_p2max, do
   return (T)(scale_p2max * r);
 }
 
-#define GF_R_CASES(R, ...)                                         \
-  switch (R) {                                                     \
-    case 1: { constexpr int RR = 1; __VA_ARGS__; } break;          \
-    case 2: { constexpr int RR = 2; __VA_ARGS__; } break;          \
-    case 3: { constexpr int RR = 3; __VA_ARGS__; } break;          \
-    case 4: { constexpr int RR = 4; __VA_ARGS__; } break;          \
-    case 6: { constexpr int RR = 6; __VA_ARGS__; } break;          \
-    case 8: { constexpr int RR = 8; __VA_ARGS__; } break;          \
-    case 12: { constexpr int RR = 12; __VA_ARGS__; } break;        \
-    default: { constexpr int RR = 16; __VA_ARGS__; } break;        \
+// MAXR (a constexpr int in scope): the largest radix the enclosing kernel instantiation is launched with; the cases
+// above it compile to nothing, so a kernel for radices <= 8 does not carry the register budget of a 16-point transform.
+#define GF_R_CASES(R, ...)                                                                      \
+  switch (R) {                                                                                  \
+    case 1: { constexpr int RR = 1; __VA_ARGS__; } break;                                       \
+    case 2: { constexpr int RR = 2; __VA_ARGS__; } break;                                       \
+    case 3: { constexpr int RR = 3; __VA_ARGS__; } break;                                       \
+    case 4: { constexpr int RR = 4; __VA_ARGS__; } break;                                       \
+    case 6: { constexpr int RR = 6; __VA_ARGS__; } break;                                       \
+    case 8: { constexpr int RR = 8; __VA_ARGS__; } break;                                       \
+    case 12: { constexpr int RR = MAXR >= 12 ? 12 : 1; if (MAXR >= 12) { __VA_ARGS__; } } break; \
+    default: { constexpr int RR = MAXR >= 16 ? 16 : 1; if (MAXR >= 16) { __VA_ARGS__; } } break; \
   }
 
 // ---- tables ----------------------------------------------------------------------------------------------------------------
@@ -197,7 +199,7 @@ struct LineArgs {
   double scale_p2max;
 };
 
-template <class T, int MODE>
+template <class T, int MODE, int MAXR>
 __global__ void __launch_bounds__(256) fft_line_kernel(cplx_t<T>* __restrict__ w, LineArgs a) {
   using C = cplx_t<T>;
   extern __shared__ __align__(16) unsigned char line_smem[];
@@ -303,8 +305,9 @@ template <bool V> struct DirTag { static constexpr bool value = V; };
 // store phases overlap the others' register steps.
 constexpr int PLANE_THREADS = 128;
 
-template <class T, bool INV>
-__global__ void __launch_bounds__(PLANE_THREADS, 3) fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
+template <class T, bool INV, int MAXR>
+__global__ void __launch_bounds__(MAXR <= 8 ? 2 * PLANE_THREADS : PLANE_THREADS, 3)
+fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
   using C = cplx_t<T>;
   extern __shared__ __align__(16) unsigned char plane_smem[];
   C* tile = reinterpret_cast<C*>(plane_smem);
@@ -428,21 +431,17 @@ static cudaError_t plane_pass(const KernelArgs& a, const FftShape& s, void* w, c
   // work items per step: ny*rx2 ... nx*ry1; one block of up to 256 threads per plane
   int items = p.ny * p.rx2;
   if (p.nx * p.ry2 > items) items = p.nx * p.ry2;
+  const bool small = p.rx1 <= 8 && p.ry1 <= 8;  // r1 >= r2: the largest radix of the plane
   int threads = 32;
-  while (threads < items && threads < PLANE_THREADS) threads *= 2;
-  cudaError_t e;
-  if (inverse) {
-    auto k = fft_plane_kernel<T, true>;
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OWN_FFT_MAX_SMEM);
+  while (threads < items && threads < (small ? 2 * PLANE_THREADS : PLANE_THREADS)) threads *= 2;
+  auto go = [&](auto k) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OWN_FFT_MAX_SMEM);
     if (e != cudaSuccess) return e;
     k<<<planes, threads, smem, a.stream>>>((C*)w, p);
-  } else {
-    auto k = fft_plane_kernel<T, false>;
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OWN_FFT_MAX_SMEM);
-    if (e != cudaSuccess) return e;
-    k<<<planes, threads, smem, a.stream>>>((C*)w, p);
-  }
-  return cudaGetLastError();
+    return cudaGetLastError();
+  };
+  if (inverse) return small ? go(fft_plane_kernel<T, true, 8>) : go(fft_plane_kernel<T, true, 16>);
+  return small ? go(fft_plane_kernel<T, false, 8>) : go(fft_plane_kernel<T, false, 16>);
 }
 
 template <class T>
@@ -471,15 +470,16 @@ static cudaError_t line_pass(const KernelArgs& a, const FftShape& s, void* w, co
   const size_t smem = l.r2 == 1 ? 0 : (size_t)l.n * l.xb * sizeof(C);
   const dim3 grid((unsigned)(l.es / l.xb), (unsigned)outer);
   const int threads = l.xb * l.ty;
-  if (mode == LINE_FWD) fft_line_kernel<T, LINE_FWD><<<grid, threads, smem, a.stream>>>((C*)w, l);
-  else if (mode == LINE_INV) fft_line_kernel<T, LINE_INV><<<grid, threads, smem, a.stream>>>((C*)w, l);
-  else {
-    auto k = fft_line_kernel<T, LINE_FUSED>;
+  const bool small = l.r1 <= 8;
+  auto go = [&](auto k) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     if (e != cudaSuccess) return e;
     k<<<grid, threads, smem, a.stream>>>((C*)w, l);
-  }
-  return cudaGetLastError();
+    return cudaGetLastError();
+  };
+  if (mode == LINE_FWD) return small ? go(fft_line_kernel<T, LINE_FWD, 8>) : go(fft_line_kernel<T, LINE_FWD, 16>);
+  if (mode == LINE_INV) return small ? go(fft_line_kernel<T, LINE_INV, 8>) : go(fft_line_kernel<T, LINE_INV, 16>);
+  return small ? go(fft_line_kernel<T, LINE_FUSED, 8>) : go(fft_line_kernel<T, LINE_FUSED, 16>);
 }
 
 template <class T>
@@ -490,12 +490,6 @@ static cudaError_t own_update_T(const KernelArgs& a, void* w, const double* tabl
   // (alpha/2) / N * p^2_max with N = the transform's size and p^2_max = 4 per transformed direction (readings B2-B4)
   const double N = (double)a.geo.n[0] * a.geo.n[1] * a.geo.n[2] * (landau ? a.geo.n[3] : 1);
   const double scale_p2max = 0.5 * alpha / N * (landau ? 16.0 : 12.0);
-  for (int m : {LINE_FWD, LINE_INV}) {  // both plain line kernels may need > 48 KB
-    cudaError_t e = m == LINE_FWD
-                        ? cudaFuncSetAttribute(fft_line_kernel<T, LINE_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024)
-                        : cudaFuncSetAttribute(fft_line_kernel<T, LINE_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-    if (e != cudaSuccess) return e;
-  }
   cudaError_t e = plane_pass<T>(a, s, w, table, false);
   if (e != cudaSuccess) return e;
   if (landau) {
