@@ -384,7 +384,7 @@ def run_ours(args):
 
 def run_fftsd(args):
     """--algo fftsd: Algorithm 2 (steepest descent with Fourier acceleration) on the same workload.
-    A step = `check_every` iterations (Delta+F/theta pass, cuFFT forward, factor, cuFFT backward, rotation) + one read
+    A step = `check_every` iterations (Delta+F/theta pass, transforms + factor + inverse transforms, rotation) + one read
     of F/theta.  Secondary line: metric fftsd_site_iterations_per_s, not the headline."""
     import torch
 
@@ -430,7 +430,7 @@ def run_fftsd(args):
             "dtype": prec, "data": "synthetic",
             "config": {"workload": workload_name(cfg), "algorithm": "Algorithm 2, alpha=0.08",
                        "step": f"{n_it} iterations + 1 F/theta measurement", "final_F": F, "final_theta": th},
-            "roofline": {"bound": "hbm", "kernel": "whole iteration (sd_delta, cuFFT x2, sd_filter, sd_rotate)",
+            "roofline": {"bound": "hbm", "kernel": "whole iteration (sd_delta, transform passes with the Fourier factor, sd_rotate)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
                          "peak_source": peak_src, "algorithmic_bytes_per_iteration": bytes_it},
             "gpu_launches": int(fx.kernel_launches() - l0)}

@@ -127,8 +127,9 @@ int gf_set_option(gf_ctx* ctx, int key, int value);
  * the d gauge-fixing directions (4-D for Landau; the 3-D transform of every time slice for Coulomb), multiplied by
  * (alpha/2) p^2_max/p^2 with p^2 = sum_mu 4 sin^2(pi k_mu/n_mu) (0 at p = 0) and transformed back (normalised);
  * g(x) = reunitarise(1 + w(x)) (first-order exponential; Gram-Schmidt as gf_reunitarize);
- * U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all four mu.  Readings B1-B6 in DESIGN.md.  The transforms are cuFFT
- * calls; cuFFT's own allocation is switched off, its work area lives in the caller's workspace.
+ * U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all four mu.  Readings B1-B6 in DESIGN.md.  The transforms are the
+ * library's own passes (GF_OPT_FFT_OWN) where the lattice extents allow it, else cuFFT calls; cuFFT's own allocation
+ * is switched off, its work area lives in the caller's workspace.
  *
  * gf_fft_workspace_bytes: *bytes = size of the SECOND device workspace these calls need (the packed Delta/w fields,
  *   4 complex numbers per site; the momentum table; cuFFT's work area).  Creates the cuFFT plans (needs a device).
