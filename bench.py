@@ -527,7 +527,8 @@ def run_sharded(args):
     V = gi.volume(dims)
     L = LINK_BYTES[(prec, storage)]
     n_sw, omega = cfg["check_every"], cfg["omega"]
-    sh = gf.ShardedGaugeFixer(gdims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
+    sh = gf.ShardedGaugeFixer(gdims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}",
+                              direct=False if args.no_direct else None)
     sh.set_reunit_every(cfg["reunit_every"])
     links = {}
     for s in sh.slabs:  # every slab its own seeded field of the config's recipe (rougher across slab boundaries)
@@ -572,7 +573,7 @@ def run_sharded(args):
                            "step": f"{n_sw} sweeps + 1 F/theta measurement",
                            "parallelism": f"T-slabs: {n_slabs} slabs over {world} rank(s), {K} per rank",
                            "halo": f"2 messages of {halo // len(sh.engines)} B per slab and half-sweep "
-                                   f"({'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
+                                   f"({'stored by the border kernel into the neighbour slab' if sh.direct else 'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
                            "l2": "inputs exceed L2" if 4 * V * L > 126e6 else "field fits L2 in part",
                            "final_F": F, "final_theta": th},
                 "roofline": {"bound": "hbm", "kernel": "ovr_halfsweep_staged_kernel (border + interior launches)",
@@ -605,6 +606,7 @@ def main():
     ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
     ap.add_argument("--sharded", type=int, default=0, metavar="K",
                     help="T-slab sharded sweep with K slabs per rank (secondary line; default 0 = single context / replicas)")
+    ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

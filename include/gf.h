@@ -177,8 +177,19 @@ int gf_fix_fft(gf_ctx* ctx, double alpha, double eps, int max_iters, int check_e
  * equal slabs); gf_ovr_sweep and gf_fix return GF_EINVAL, the gf_fft_* calls GF_EUNSUPPORTED (the paper has no
  * multi-GPU Algorithm 2 either).  With R = 1 (the slab is its own neighbour) the calls reproduce
  * gf_ovr_sweep bit for bit.  All Async.  Errors: GF_EINVAL (no halo attached, parity not 0/1, omega), GF_ENOMEM,
- * GF_ECUDA. */
+ * GF_ECUDA.
+ *
+ * Direct delivery (gf_slab_set_targets): where the neighbours' halo workspaces are addressable from this device (slabs
+ * of the same process; peer-mapped memory of another GPU over NVLink), the border kernel itself stores the two
+ * messages at their destination — the top-slice sites write their new U_t(x) into the upper neighbour's ghost[p]
+ * (instead of top_out), the t = 0 sites write the updated ghost links into the lower neighbour's top_in as well as
+ * into ghost[1-p] — and step 3 disappears; the caller only orders the kernels: a neighbour's border kernel of this
+ * half-sweep must have finished before gf_slab_unpack_top(1-p) and before the next half-sweep's border kernel, and a
+ * slab's unpack before a neighbour's next border kernel.  Pass the three pointers of the neighbours' workspaces (upper:
+ * offset 0 and B, lower: offset 3B), or three nulls to go back to top_out.  gf_slab_pack_top then writes to the upper
+ * neighbour's ghost[parity] too. */
 size_t gf_slab_halo_bytes(const gf_ctx* ctx);
+int gf_slab_set_targets(gf_ctx* ctx, void* upper_ghost0, void* upper_ghost1, void* lower_top_in);
 int gf_slab_attach(gf_ctx* ctx, void* dev_halo, size_t halo_workspace_bytes);
 int gf_slab_pack_top(gf_ctx* ctx, int parity);
 int gf_slab_unpack_top(gf_ctx* ctx, int parity);

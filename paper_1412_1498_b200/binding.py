@@ -22,7 +22,7 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
            "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error",
            "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
-           "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_pack_top", "gf_slab_unpack_top",
+           "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"]
 
 
@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
     lib.gf_slab_halo_bytes.argtypes = [c_void_p]
     lib.gf_slab_attach.restype = c_int
     lib.gf_slab_attach.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.gf_slab_set_targets.restype = c_int
+    lib.gf_slab_set_targets.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
     for name in ("gf_slab_pack_top", "gf_slab_unpack_top"):
         getattr(lib, name).restype = c_int
         getattr(lib, name).argtypes = [c_void_p, c_int]
@@ -184,6 +186,11 @@ def gf_slab_halo_bytes(ctx) -> int:
 
 def gf_slab_attach(ctx, dev_halo: int, halo_workspace_bytes: int) -> int:
     return lib.gf_slab_attach(ctx, c_void_p(dev_halo), halo_workspace_bytes)
+
+
+def gf_slab_set_targets(ctx, upper_ghost0: int, upper_ghost1: int, lower_top_in: int) -> int:
+    return lib.gf_slab_set_targets(ctx, c_void_p(upper_ghost0 or None), c_void_p(upper_ghost1 or None),
+                                   c_void_p(lower_top_in or None))
 
 
 def gf_slab_pack_top(ctx, parity: int) -> int:

@@ -80,6 +80,8 @@ struct gf_ctx {
   size_t halo_bytes;  // one message: U_t of one parity of one time slice
   char* top_out;      // packed top-slice links on their way to the upper neighbour's ghost buffer
   char* top_in;       // ghost links coming back from the upper neighbour
+  char* fwd_target[2];  // gf_slab_set_targets: the upper neighbour's ghost[0], ghost[1] (peer-mapped), or null
+  char* ret_target;     //                      the lower neighbour's top_in, or null
   char err[256];
 };
 
@@ -139,9 +141,10 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0; c->fft_own = 1; c->own_table = nullptr;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
-  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr};
+  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr, nullptr};
   c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
   c->top_out = c->top_in = nullptr;
+  c->fwd_target[0] = c->fwd_target[1] = c->ret_target = nullptr;
   c->host_result = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
   cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
@@ -526,6 +529,17 @@ int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
   return GF_OK;
 }
 
+int gf_slab_set_targets(gf_ctx* c, void* upper_ghost0, void* upper_ghost1, void* lower_top_in) {
+  if (!c) return GF_EINVAL;
+  if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_targets: no halo workspace attached (gf_slab_attach)");
+  if ((upper_ghost0 == nullptr) != (upper_ghost1 == nullptr) || (upper_ghost0 == nullptr) != (lower_top_in == nullptr))
+    return fail(c, GF_EINVAL, "gf_slab_set_targets: give all three targets or none");
+  c->fwd_target[0] = (char*)upper_ghost0;
+  c->fwd_target[1] = (char*)upper_ghost1;
+  c->ret_target = (char*)lower_top_in;
+  return GF_OK;
+}
+
 static int slab_check(gf_ctx* c, int parity, const char* who) {
   if (!c) return GF_EINVAL;
   if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_*: no halo workspace attached (gf_slab_attach)");
@@ -536,7 +550,7 @@ static int slab_check(gf_ctx* c, int parity, const char* who) {
 int gf_slab_pack_top(gf_ctx* c, int parity) {
   int rc = slab_check(c, parity, "gf_slab_pack_top: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
-  cudaError_t e = launch_slab_top(c->k, parity, c->top_out, true);
+  cudaError_t e = launch_slab_top(c->k, parity, c->fwd_target[parity] ? c->fwd_target[parity] : c->top_out, true);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_pack_top");
   c->launches += 1;
   return GF_OK;
@@ -558,7 +572,8 @@ int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_border: omega outside [1,2)");
   const Geo& g = c->k.geo;
   // one launch: bottom slice, top slice; the top-slice sites also write their updated U_t(x) into top_out
-  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3, g.vh - g.s3, g.vh, c->top_out);
+  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3, g.vh - g.s3, g.vh,
+                                        c->fwd_target[parity] ? c->fwd_target[parity] : c->top_out, c->ret_target);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_border");
   c->launches += 1;
   c->qblocks = 0;
@@ -571,7 +586,7 @@ int gf_slab_halfsweep_interior(gf_ctx* c, int parity, double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_interior: omega outside [1,2)");
   const Geo& g = c->k.geo;
   if (g.n[3] == 2) return GF_OK;
-  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, g.s3, g.vh - g.s3, 0, 0, nullptr);
+  cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, g.s3, g.vh - g.s3, 0, 0, nullptr, nullptr);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_interior");
   c->launches += 1;
   c->qblocks = 0;

@@ -14,6 +14,7 @@ struct SlabView {
   int nblocks0;          // ... covered by the first nblocks0 blocks; the remaining blocks cover
   int cb2_begin, cb2_end;  //     a second range (border launch: bottom and top slice in one grid)
   void* top_out;         // non-null: top-slice sites also leave their updated U_t(x) here (message layout)
+  void* ret_out;         // non-null: t = 0 sites also leave their updated U_t(x - t) here (message layout, one parity)
 };
 
 struct KernelArgs {
@@ -43,7 +44,7 @@ bool halfsweep_can_fuse_theta(const KernelArgs& a);
 // T-slab: the sites [cb_begin, cb_end) and [cb2_begin, cb2_end) of `parity` in one launch (staged kernel; t = 0 sites
 // use a.slab.ghost; with top_out the top-slice sites also write their updated U_t(x) there)
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
-                                  int cb2_begin, int cb2_end, void* top_out);
+                                  int cb2_begin, int cb2_end, void* top_out, void* ret_out);
 // U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
 cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);

@@ -339,6 +339,11 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       load_link_smem<NELEM, THREADS, false>(sm, 2 * mu + 1, u);
       mul_right_adj<NELEM / 3>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
       store_link<NELEM>(bwd[mu], w);
+      if (SLAB && mu == 3 && sv.ret_out && cb < g.s3) {   // bottom slice: the copy that goes back to the lower neighbour
+        SlabView out = sv;
+        out.ghost = sv.ret_out;
+        store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb), w);
+      }
       sched_fence();
     }
   }
@@ -368,7 +373,7 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
 // the sites [cb_begin, cb_end) of one parity of a T-slab
 template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
-                                    int cb2_begin, int cb2_end, void* top_out) {
+                                    int cb2_begin, int cb2_end, void* top_out, void* ret_out) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
@@ -385,6 +390,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.cb2_begin = cb2_begin; sv.cb2_end = cb2_end;
   sv.nblocks0 = cb_end > cb_begin ? (cb_end - cb_begin + THREADS - 1) / THREADS : 0;
   sv.top_out = top_out;
+  sv.ret_out = ret_out;
   const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv);
   return cudaGetLastError();
@@ -436,8 +442,8 @@ cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool
 }
 
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
-                                  int cb2_begin, int cb2_end, void* top_out) {
-  GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end, cb2_begin, cb2_end, top_out);
+                                  int cb2_begin, int cb2_end, void* top_out, void* ret_out) {
+  GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end, cb2_begin, cb2_end, top_out, ret_out);
 }
 
 // ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------

@@ -49,6 +49,11 @@ class GpuSlabEngine:
     def get_links(self, out=None):
         return self.fx.get_links(out)
 
+    def set_targets(self, upper_ghost0, upper_ghost1, lower_top_in):
+        """Device tensors of the neighbours' halo workspaces the border kernel stores into (None x 3: back to top_out)."""
+        ptr = [t.data_ptr() if t is not None else 0 for t in (upper_ghost0, upper_ghost1, lower_top_in)]
+        self.fx._check(_b.gf_slab_set_targets(self.fx.ctx, *ptr))
+
     def pack_top(self, parity):
         self.fx._check(_b.gf_slab_pack_top(self.fx.ctx, int(parity)))
 
@@ -120,10 +125,14 @@ class ShardedGaugeFixer:
     dims: the GLOBAL lattice (nx, ny, nz, nt).  With torch.distributed initialised every rank constructs the same object
     and owns n_slabs / world_size consecutive slabs; without it (or with group=False) all slabs live in this process.
     engine_factory(local_dims, slab_index) builds one slab (default: GpuSlabEngine on `device`).
+    direct: the border kernels store the halo messages straight into the neighbours' buffers (gf_slab_set_targets)
+    instead of handing them to the transport; possible when every neighbour's halo workspace is addressable from the
+    slab's device, i.e. today when all slabs live in this process (default then).  Between processes the buffers would
+    have to be mapped with CUDA IPC first; that is not built, the transport path is used.
     """
 
     def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
-                 engine_factory=None):
+                 engine_factory=None, direct=None):
         import torch
 
         self.torch = torch
@@ -156,6 +165,15 @@ class ShardedGaugeFixer:
         if self.on_gpu:
             with torch.cuda.device(self.device):
                 self.comm_stream = torch.cuda.Stream(self.device)
+        can_direct = self.world == 1 and self.on_gpu and all(hasattr(e, "set_targets") for e in self.engines.values())
+        if direct and not can_direct:
+            raise ValueError("direct delivery needs all slabs in this process, on GPUs")
+        self.direct = can_direct if direct is None else bool(direct)
+        if self.direct:
+            for s, e in self.engines.items():
+                up, lo = self.engines[(s + 1) % self.n_slabs], self.engines[(s - 1) % self.n_slabs]
+                e.set_targets(up.ghost[0], up.ghost[1], lo.top_in)
+        self._after_unpack = {}
         self.reunit_every = 0
         self.sweeps_total = 0
         self.messages_sent = 0  # remote (torch.distributed) messages posted by this rank
@@ -210,12 +228,21 @@ class ShardedGaugeFixer:
             return group_rank
         return self.dist.get_global_rank(self.group, group_rank)
 
+    def _join_neighbours(self, events):
+        """Direct delivery: slab s goes on once its two neighbours' kernels behind `events` are done."""
+        for s in self.slabs:
+            for nb in {(s - 1) % self.n_slabs, (s + 1) % self.n_slabs} - {s}:
+                self.engines[s].wait(events.get(nb))
+
     def refresh_ghosts(self):
         """Fill both ghost buffers of every slab from its lower neighbour's top slice (after set_links, reunitarize)."""
         for q in (0, 1):
             for s in self.slabs:
                 self.engines[s].pack_top(q)
-            self._exchange(q, kinds=("fwd",))
+            if self.direct:
+                self._join_neighbours({s: self.engines[s].mark() for s in self.slabs})
+            else:
+                self._exchange(q, kinds=("fwd",))
 
     # ---- links in / out ---------------------------------------------------------------------------------------------------
     def set_links(self, links_by_slab):
@@ -235,6 +262,20 @@ class ShardedGaugeFixer:
 
     # ---- Algorithm 1 ---------------------------------------------------------------------------------------------------------
     def half_sweep(self, p, omega):
+        if self.direct:
+            # the border kernels deliver: a slab's border kernel writes its neighbours' ghost[p] / top_in, so it starts
+            # after their last unpack, and the unpack after the neighbours' border kernels
+            self._join_neighbours(self._after_unpack)
+            for s in self.slabs:
+                self.engines[s].border(p, omega)
+            after = {s: self.engines[s].mark() for s in self.slabs}
+            for s in self.slabs:
+                self.engines[s].interior(p, omega)
+            self._join_neighbours(after)
+            for s in self.slabs:
+                self.engines[s].unpack_top(1 - p)
+            self._after_unpack = {s: self.engines[s].mark() for s in self.slabs}
+            return
         for s in self.slabs:
             self.engines[s].border(p, omega)
         # the transport starts as soon as the border kernels are done, beside the interior kernels queued behind them

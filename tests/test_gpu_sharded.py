@@ -50,13 +50,17 @@ LATTICES = [((8, 8, 8, 8), 1), ((8, 8, 8, 8), 2), ((8, 8, 8, 8), 4), ((6, 4, 2, 
             ((2, 2, 2, 4), 2), ((16, 4, 4, 12), 2), ((10, 6, 4, 8), 1)]
 
 
+@pytest.mark.parametrize("direct", [True, False], ids=["direct", "transport"])
 @pytest.mark.parametrize("dims,n_slabs", LATTICES)
 @pytest.mark.parametrize("gauge", ["landau", "coulomb"])
 @pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
-def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_slabs, gauge, prec, storage):
+def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_slabs, gauge, prec, storage, direct):
+    """direct: the border kernels store the halo messages into the neighbours' buffers (gf_slab_set_targets);
+    transport: they leave them in top_out / ghost and the plumbing copies them."""
     omega, sweeps = 1.7, 2
     U, Uo = host_input(dims, 0.5, 31, prec, storage)
-    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False)
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, direct=direct)
+    assert sh.direct == direct
     sh.set_links_global(torch.from_numpy(U).cuda())
     F0, th0 = sh.measure()
     sh.ovr_sweep(sweeps, omega)
@@ -87,15 +91,17 @@ def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_sla
     assert abs(F - Fo) <= TOL_F[prec] * abs(Fo)
     assert tho / 1.5 <= th <= tho * 1.5
     assert n_launch > 0
+    assert (sh.copies == 0) == direct
 
 
 @pytest.mark.parametrize("gauge,prec,storage,n_slabs", [("landau", "f64", 18, 2), ("coulomb", "f64", 12, 4),
                                                         ("landau", "f32", 12, 2)])
-def test_sharded_fix_matches_single_context_trajectory(gf, torch, gauge, prec, storage, n_slabs):
+@pytest.mark.parametrize("direct", [True, False], ids=["direct", "transport"])
+def test_sharded_fix_matches_single_context_trajectory(gf, torch, gauge, prec, storage, n_slabs, direct):
     """The whole driver loop (measurement cadence, stop test, reunitarisation + ghost refresh) on slabs against gf_fix."""
     dims, omega, eps, cap, every, reunit = (8, 8, 8, 8), 1.7, 1e-9 if prec == "f64" else 1e-6, 300, 10, 20
     U, _ = host_input(dims, 0.3, 32, prec, storage)
-    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False)
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, direct=direct)
     sh.set_reunit_every(reunit)
     sh.set_links_global(torch.from_numpy(U).cuda())
     done, hist = sh.fix(omega, eps, cap, every)
@@ -122,11 +128,14 @@ def test_slab_abi_errors(gf, torch):
     # no halo attached yet
     assert gf.gf_slab_halfsweep_border(fx.ctx, 0, 1.7) == gf.GF_EINVAL
     assert gf.gf_slab_pack_top(fx.ctx, 0) == gf.GF_EINVAL
+    assert gf.gf_slab_set_targets(fx.ctx, 0, 0, 0) == gf.GF_EINVAL
     halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
     assert gf.gf_slab_attach(fx.ctx, 0, 4 * B) == gf.GF_EINVAL
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B - 1) == gf.GF_ENOMEM
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr() + 8, 4 * B) == gf.GF_ENOMEM
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_OK
+    assert gf.gf_slab_set_targets(fx.ctx, halo.data_ptr(), 0, 0) == gf.GF_EINVAL  # all three or none
+    assert gf.gf_slab_set_targets(fx.ctx, 0, 0, 0) == gf.GF_OK
     assert gf.gf_slab_halfsweep_border(fx.ctx, 2, 1.7) == gf.GF_EINVAL
     assert gf.gf_slab_halfsweep_interior(fx.ctx, -1, 1.7) == gf.GF_EINVAL
     assert gf.gf_slab_halfsweep_border(fx.ctx, 0, 2.0) == gf.GF_EINVAL
