@@ -115,10 +115,14 @@ enum {
   GF_OPT_FFT_FUSED_T = 5,   /* 1: in Landau gauge with n_t a power of two (<= 256) the transform along t, the Fourier
                                factor and the inverse transform along t are one hand-written pass through shared
                                memory; 0 (default): cuFFT's strided 1-D transforms and a separate factor kernel */
-  GF_OPT_FFT_OWN = 6        /* 1 (default): when every transformed extent is a product of two of {1,2,3,4,6,8,12,16}
+  GF_OPT_FFT_OWN = 6,       /* 1 (default): when every transformed extent is a product of two of {1,2,3,4,6,8,12,16}
                                (<= 256) and an (x,y) plane fits shared memory, the transforms, the Fourier factor and
                                the inverse transforms run as hand-written passes (5 over the fields in Landau gauge,
                                3 in Coulomb gauge), without cuFFT; other lattices, or 0: the cuFFT path */
+  GF_OPT_OVR_SERIES = 7     /* 0 (default): g^omega of every SU(2) subgroup step is the exact power (reading A6);
+                               N = 1..16: the binomial series sum_{n<=N} binom(omega,n) (g-1)^n, normalised back to
+                               SU(2) - the way ref. [1] of the paper evaluates g^omega (reading A21).
+                               Default sweep variant only; GF_EUNSUPPORTED on a slab context. */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 

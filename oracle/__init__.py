@@ -140,6 +140,23 @@ def su2_power(a, omega, dtype=np.float64):
     return out
 
 
+def su2_power_series(a, omega, order, dtype=np.float64):
+    """Truncated binomial series of g^omega (order terms beyond 1), renormalised (reading A21)."""
+    a = np.ascontiguousarray(a, dtype=dtype)
+    out = np.zeros(4, dtype=dtype)
+    _fn("orc_su2_power_series", a)(_p(a), ctypes.c_double(omega), int(order), _p(out))
+    return out
+
+
+def set_series(order: int) -> None:
+    """Process-wide switch: 0 = every update uses the exact power g^omega (default), N > 0 = the order-N series."""
+    _load().orc_set_series(int(order))
+
+
+def get_series() -> int:
+    return int(_load().orc_get_series())
+
+
 def wilson_traces(U, dims, mu, nu, a, b):
     """Tr of the a x b Wilson loop in the (mu,nu) plane at every site, complex array of length V."""
     V = int(np.prod(dims))

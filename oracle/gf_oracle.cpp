@@ -241,6 +241,43 @@ void su2_power(const T a[4], T omega, T out[4]) {
   out[3] = a[3] * f;
 }
 
+// Variant (PAPER.md:50 cites ref. [1], Mandula & Ogilvie, for g -> g^omega; they evaluate it as a truncated binomial
+// series followed by a projection back to the group; reading A21): g^omega ~ sum_{n=0}^{N} binom(omega, n) (g - 1)^n,
+// binom(omega, n) = omega (omega-1) ... (omega-n+1) / n!, written out with quaternion products
+// (p0 + i p.sigma)(q0 + i q.sigma) = (p0 q0 - p.q) + i (p0 q + q0 p - p x q).sigma, then normalised to a unit quaternion.
+// order = 0 selects the exact power above; it is a process-wide switch of this test library (orc_set_series).
+int g_series_order = 0;
+
+template <class T>
+void quat_mul(const T p[4], const T q[4], T out[4]) {
+  out[0] = p[0] * q[0] - (p[1] * q[1] + p[2] * q[2] + p[3] * q[3]);
+  out[1] = p[0] * q[1] + q[0] * p[1] - (p[2] * q[3] - p[3] * q[2]);
+  out[2] = p[0] * q[2] + q[0] * p[2] - (p[3] * q[1] - p[1] * q[3]);
+  out[3] = p[0] * q[3] + q[0] * p[3] - (p[1] * q[2] - p[2] * q[1]);
+}
+
+template <class T>
+void su2_power_series(const T a[4], T omega, int order, T out[4]) {
+  const T u[4] = {a[0] - T(1), a[1], a[2], a[3]};  // g - 1
+  T P[4] = {T(1), T(0), T(0), T(0)};               // (g - 1)^n
+  T acc[4] = {T(0), T(0), T(0), T(0)};
+  T b = T(1);                                      // binom(omega, n)
+  for (int n = 0; n <= order; ++n) {
+    for (int k = 0; k < 4; ++k) acc[k] += b * P[k];
+    T next[4];
+    quat_mul(P, u, next);
+    for (int k = 0; k < 4; ++k) P[k] = next[k];
+    b = b * (omega - T(n)) / T(n + 1);
+  }
+  const T norm = std::sqrt(acc[0] * acc[0] + acc[1] * acc[1] + acc[2] * acc[2] + acc[3] * acc[3]);
+  if (norm == T(0)) {
+    out[0] = T(1);
+    out[1] = out[2] = out[3] = T(0);
+    return;
+  }
+  for (int k = 0; k < 4; ++k) out[k] = acc[k] / norm;
+}
+
 // One SU(2) subgroup step on rows/columns (i,j): maximise Re Tr[g K] over the embedded SU(2) (eq. 1.6 applied to the
 // SU(2)-proportional part of the 2x2 block, reading A5), raise to omega, K <- gK, G <- gG.  a_out = quaternion of g^omega.
 template <class T>
@@ -258,7 +295,8 @@ void su2_subgroup_step(Mat3<T>& K, Mat3<T>& G, int i, int j, T omega, T a_out[4]
     return;
   }
   T a[4] = {r[0] / n, r[1] / n, r[2] / n, r[3] / n};
-  su2_power(a, omega, a_out);
+  if (g_series_order > 0) su2_power_series(a, omega, g_series_order, a_out);
+  else su2_power(a, omega, a_out);
   // g = [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]] on rows/cols (i,j), 1 on the third
   const Cx<T> g00(a_out[0], a_out[3]), g01(a_out[2], a_out[1]), g10(-a_out[2], a_out[1]), g11(a_out[0], -a_out[3]);
   for (int c = 0; c < 3; ++c) {
@@ -482,6 +520,9 @@ void mat_to(T* p, const Mat3<T>& a) {
     mat_to<T>(G18, G);                                                                                                \
   }                                                                                                                   \
   void orc_su2_power_##SUF(const T* a4, double omega, T* out4) { su2_power<T>(a4, (T)omega, out4); }                  \
+  void orc_su2_power_series_##SUF(const T* a4, double omega, int order, T* out4) {                                    \
+    su2_power_series<T>(a4, (T)omega, order, out4);                                                                   \
+  }                                                                                                                   \
   void orc_wilson_traces_##SUF(const T* U, const int* dims, int mu, int nu, int a, int b, double* out) {              \
     wilson_traces<T>(U, make_geom(dims), mu, nu, a, b, out);                                                          \
   }                                                                                                                   \
@@ -495,3 +536,7 @@ void mat_to(T* p, const Mat3<T>& a) {
 
 ORC_API(f64, double)
 ORC_API(f32, float)
+
+// 0: g^omega is the exact power (default); N > 0: the truncated binomial series of order N (su2_power_series)
+extern "C" void orc_set_series(int order) { g_series_order = order < 0 ? 0 : order; }
+extern "C" int orc_get_series() { return g_series_order; }

@@ -126,7 +126,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->k.geo = g;
   c->k.stream = (cudaStream_t)cuda_stream;
   c->k.prec = prec; c->k.storage = storage; c->k.gauge = gauge;
-  c->k.variant = 0; c->k.block_threads = 0;
+  c->k.variant = 0; c->k.block_threads = 0; c->k.series = 0;
   c->sz = sz;
   char* base = (char*)dev_workspace;
   c->k.links = base;
@@ -271,6 +271,12 @@ int gf_set_option(gf_ctx* c, int key, int value) {
       return GF_OK;
     case GF_OPT_FFT_OWN:
       c->fft_own = value != 0;
+      return GF_OK;
+    case GF_OPT_OVR_SERIES:
+      if (value < 0 || value > 16) return fail(c, GF_EINVAL, "gf_set_option: series order outside 0..16");
+      if (value > 0 && c->k.slab.ghost) return fail(c, GF_EUNSUPPORTED, "gf_set_option: no series variant on a slab context");
+      c->k.series = value;
+      c->qblocks = 0;
       return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
@@ -521,6 +527,7 @@ int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
   if (bytes < 4 * c->halo_bytes || ((uintptr_t)dev_halo % ALIGN))
     return fail(c, GF_ENOMEM, "gf_slab_attach: workspace too small or misaligned");
   if (c->fft_w) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: Algorithm 2 is attached to this context");
+  if (c->k.series > 0) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: no series variant (GF_OPT_OVR_SERIES) on a slab");
   char* base = (char*)dev_halo;
   c->k.slab.ghost = base;  // ghost[0], ghost[1]
   c->top_out = base + 2 * c->halo_bytes;

@@ -143,17 +143,46 @@ __device__ __forceinline__ void su2_overrelax(T r0, T r1, T r2, T r3, T omega, T
   q1 = r1 * f; q2 = r2 * f; q3 = r3 * f;
 }
 
+// Variant (GF_OPT_OVR_SERIES, reading A21; PAPER.md:50 cites Mandula & Ogilvie for g^omega, who truncate its binomial
+// series): g^omega ~ sum_{n<=N} binom(omega,n) (g-1)^n, projected back to SU(2) by normalisation.  With a = r/|r| =
+// (a0; a_vec), every power of g - 1 is P0 + i Pv (a_vec.sigma), and (P0, Pv)(g - 1) = (P0 (a0-1) - Pv |a_vec|^2,
+// P0 + (a0-1) Pv); no division by |a_vec|, so the limit a_vec -> 0 needs no special case.
+template <class T>
+__device__ __forceinline__ void su2_overrelax_series(T r0, T r1, T r2, T r3, T omega, int order, T& c, T& q1, T& q2,
+                                                     T& q3) {
+  const T S2 = r1 * r1 + r2 * r2 + r3 * r3;
+  const T n2 = r0 * r0 + S2;
+  if (!(n2 > T(0))) { c = T(1); q1 = q2 = q3 = T(0); return; }  // reading A7
+  const T inv = T(1) / sqrt_(n2);
+  const T u0 = r0 * inv - T(1), s2 = S2 * inv * inv;
+  T P0 = T(1), Pv = T(0), A0 = T(0), Av = T(0), b = T(1);
+  for (int n = 0; n <= order; ++n) {
+    A0 = fma(b, P0, A0); Av = fma(b, Pv, Av);
+    const T t0 = P0 * u0 - Pv * s2, tv = P0 + u0 * Pv;
+    P0 = t0; Pv = tv;
+    b = b * (omega - T(n)) / T(n + 1);
+  }
+  const T norm2 = A0 * A0 + Av * Av * s2;
+  if (!(norm2 > T(0))) { c = T(1); q1 = q2 = q3 = T(0); return; }
+  const T f = T(1) / sqrt_(norm2);
+  c = A0 * f;
+  const T fv = Av * f * inv;  // a_k = r_k / |r|
+  q1 = r1 * fv; q2 = r2 * fv; q3 = r3 * fv;
+}
+
 // One subgroup step on rows/cols (I,J): K <- gK, G <- gG with g = [[c+i q3, q2+i q1], [-q2+i q1, c-i q3]] embedded.
 // K (and g) are in precision T; G may be kept in a lower precision TG (g is rounded once per step).
-template <int I, int J, bool UPDATE_K, class T, class C, class CG>
-__device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega) {
+// SERIES: g^omega by the truncated series of order `order` instead of the exact power.
+template <int I, int J, bool UPDATE_K, bool SERIES = false, class T, class C, class CG>
+__device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega, int order = 0) {
   using TG = decltype(G[0].x);
   const T r0 = K[I * 3 + I].x + K[J * 3 + J].x;
   const T r1 = -(K[I * 3 + J].y + K[J * 3 + I].y);
   const T r2 = K[J * 3 + I].x - K[I * 3 + J].x;
   const T r3 = -(K[I * 3 + I].y - K[J * 3 + J].y);
   T c, q1, q2, q3;
-  su2_overrelax(r0, r1, r2, r3, omega, c, q1, q2, q3);
+  if (SERIES) su2_overrelax_series(r0, r1, r2, r3, omega, order, c, q1, q2, q3);
+  else su2_overrelax(r0, r1, r2, r3, omega, c, q1, q2, q3);
   if (UPDATE_K) {
     const C g00 = mk<T>(c, q3), g01 = mk<T>(q2, q1), g10 = mk<T>(-q2, q1), g11 = mk<T>(c, -q3);
 #pragma unroll
@@ -177,14 +206,14 @@ __device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega) {
 
 // G = g3 g2 g1 for one site from its K (Algorithm 1 l.5-6; subgroup order (0,1),(1,2),(0,2), reading A4; A8)
 // FINAL_K: also carry K through the last step, so that on return K = G K_in (= K(x) of the updated links).
-template <class T, bool FINAL_K = false, class C, class CG>
-__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], CG (&G)[9], T omega) {
+template <class T, bool FINAL_K = false, bool SERIES = false, class C, class CG>
+__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], CG (&G)[9], T omega, int order = 0) {
   using TG = decltype(G[0].x);
 #pragma unroll
   for (int e = 0; e < 9; ++e) G[e] = mk<TG>((e % 4 == 0) ? TG(1) : TG(0), TG(0));
-  su2_step<0, 1, true>(K, G, omega);
-  su2_step<1, 2, true>(K, G, omega);
-  su2_step<0, 2, FINAL_K>(K, G, omega);
+  su2_step<0, 1, true, SERIES>(K, G, omega, order);
+  su2_step<1, 2, true, SERIES>(K, G, omega, order);
+  su2_step<0, 2, FINAL_K, SERIES>(K, G, omega, order);
 }
 
 // rows 0..NROW-1 of G.U

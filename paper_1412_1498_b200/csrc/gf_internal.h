@@ -30,6 +30,7 @@ struct KernelArgs {
   int gauge;    // 0 = Landau, 1 = Coulomb
   int variant;  // half-sweep kernel variant (GF_OPT_SWEEP_VARIANT)
   int block_threads;
+  int series;   // GF_OPT_OVR_SERIES: 0 = exact g^omega, N > 0 = truncated binomial series of order N
   SlabView slab;
 };
 

@@ -266,10 +266,11 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
 // them in this half-sweep).  After the odd half-sweep these are the odd sites' terms of theta of the finished sweep.
 // SLAB: the launch covers the checkerboard range [sv.cb_begin, sv.cb_end) of a T-slab; t = 0 sites take U_t(x - t) from
 // (and return it to) the ghost buffer.  The per-site arithmetic is the same instruction sequence in both cases.
-template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB>
+// SERIES: g^omega by the truncated binomial series of order `series` (GF_OPT_OVR_SERIES) instead of the exact power.
+template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB, bool SERIES = false>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials,
-                            SlabView sv) {
+                            SlabView sv, int series = 0) {
   using C = cplx_t<T>;
   using TK = RotationType;
   using CK = cplx_t<TK>;
@@ -321,7 +322,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     ks.finish(K);
 
     C G[9];
-    site_gauge_rotation<TK, MEASURE>(K, G, (TK)omega);
+    site_gauge_rotation<TK, MEASURE, SERIES>(K, G, (TK)omega, series);
     if (MEASURE) q = (double)delta_norm2<TK>(K);
 
 #pragma unroll
@@ -366,7 +367,24 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{});
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0);
+  return cudaGetLastError();
+}
+
+// GF_OPT_OVR_SERIES > 0: the same launch with the series kernel (no fused theta terms)
+template <class T, int NELEM, int ND, int THREADS>
+static cudaError_t halfsweep_series_T(const KernelArgs& a, int parity, double omega) {
+  using C = cplx_t<T>;
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, false, true>;
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series);
   return cudaGetLastError();
 }
 
@@ -392,7 +410,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0);
   return cudaGetLastError();
 }
 
@@ -406,6 +424,7 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
     constexpr int THREADS = staged_threads<T>();
     if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
+    if (a.series > 0) return halfsweep_series_T<T, NELEM, ND, THREADS>(a, parity, omega);
     if (fuse_theta) {
       *qblocks = (a.geo.vh + THREADS - 1) / THREADS;
       return halfsweep_staged_T<T, NELEM, ND, THREADS, true>(a, parity, omega);
@@ -414,6 +433,7 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
   }
   constexpr int THREADS = 128;
   if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
+  if (a.series > 0) return cudaErrorNotSupported;  // the series is built into the staged kernel only
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   if (a.variant == 2)
     ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1, true><<<blocks, THREADS, 0, a.stream>>>((C*)a.links, a.geo, parity,
@@ -477,7 +497,7 @@ cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pac
   return a.storage == 18 ? slab_top_T<float, 9>(a, parity, buf, pack) : slab_top_T<float, 6>(a, parity, buf, pack);
 }
 
-bool halfsweep_can_fuse_theta(const KernelArgs& a) { return a.variant == 0 || a.variant == 3; }
+bool halfsweep_can_fuse_theta(const KernelArgs& a) { return (a.variant == 0 || a.variant == 3) && a.series == 0; }
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
 // ======================================================================================================================

@@ -319,3 +319,48 @@ def test_two_contexts_on_their_own_streams(gf, torch):
     assert np.abs(g2.cpu().numpy() - O2).max() <= 3e-12
     f1.close()
     f2.close()
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4)])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+@pytest.mark.parametrize("order", [1, 4])
+def test_series_variant_of_the_overrelaxation_power(gf, torch, dims, gauge, prec, storage, order):
+    """GF_OPT_OVR_SERIES: g^omega as the truncated binomial series (reading A21), against the oracle in the same mode."""
+    omega = 1.7
+    U, Uo = host_input(dims, 0.5, 19, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
+    fx.set_option(gf.GF_OPT_OVR_SERIES, order)
+    fx.ovr_sweep(1, omega)
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    F, th = fx.measure()
+    # back to the exact power on the same context
+    fx.set_option(gf.GF_OPT_OVR_SERIES, 0)
+    fx.set_links(torch.from_numpy(U).cuda())
+    fx.ovr_sweep(1, omega)
+    exact = fx.get_links().cpu().numpy().astype(np.float64)
+    fx.close()
+    try:
+        oracle.set_series(order)
+        oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
+    finally:
+        oracle.set_series(0)
+    Fo, tho = oracle.measure(Uo, dims, gauge)
+    assert np.abs(got - Uo).max() <= TOL_LINK[prec]  # north_star's one-sweep bound
+    assert abs(F - Fo) <= TOL_F[prec] * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
+    assert np.abs(got - exact).max() > 1e-3  # the option is live: a visibly different update
+
+
+def test_series_option_errors(gf, torch):
+    fx = gf.GaugeFixer((4, 4, 4, 4))
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, -1) == gf.GF_EINVAL
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, 17) == gf.GF_EINVAL
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, 3) == gf.GF_OK
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_SWEEP_VARIANT, 1) == gf.GF_OK
+    U = gi.make_links((4, 4, 4, 4), 0.3, 1)
+    fx.set_links(torch.from_numpy(U).cuda())
+    assert gf.gf_ovr_sweep(fx.ctx, 1, 1.7) == gf.GF_ECUDA  # the two-pass kernels have no series form
+    B = gf.gf_slab_halo_bytes(fx.ctx)
+    halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
+    assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
+    fx.close()

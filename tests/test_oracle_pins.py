@@ -454,3 +454,81 @@ def test_f32_oracle_tracks_f64():
     F64, t64 = oracle.measure(A, dims, "landau")
     F32, t32 = oracle.measure(U32, dims, "landau")
     assert abs(F64 - F32) < 1e-5 * abs(F64) and abs(t64 - t32) < 1e-3 * t64
+
+
+# ---- variant: g^omega by the truncated binomial series (reading A21, ref. [1]) ------------------------------
+def _quat_to_mat(a):
+    s1 = np.array([[0, 1], [1, 0]], dtype=complex)
+    s2 = np.array([[0, -1j], [1j, 0]], dtype=complex)
+    s3 = np.array([[1, 0], [0, -1]], dtype=complex)
+    return a[0] * np.eye(2) + 1j * (a[1] * s1 + a[2] * s2 + a[3] * s3)
+
+
+def _unit_quat(rng, phi):
+    n = rng.normal(size=3)
+    n /= np.linalg.norm(n)
+    return np.array([np.cos(phi), *(np.sin(phi) * n)])
+
+
+def test_series_power_is_the_binomial_series_of_2x2_matrices():
+    """Brute force with numpy matrices: sum_n binom(omega,n) (g - 1)^n, divided by sqrt(det) (projection to SU(2))."""
+    rng = np.random.default_rng(5)
+    for phi, omega, order in [(0.3, 1.7, 3), (1.0, 1.5, 4), (2.0, 1.9, 6), (0.05, 1.2, 1), (2.9, 1.8, 8)]:
+        a = _unit_quat(rng, phi)
+        g = _quat_to_mat(a)
+        M, P, b = np.zeros((2, 2), complex), np.eye(2, dtype=complex), 1.0
+        for n in range(order + 1):
+            M = M + b * P
+            P = P @ (g - np.eye(2))
+            b = b * (omega - n) / (n + 1)
+        M = M / np.sqrt(np.linalg.det(M).real)
+        got = _quat_to_mat(oracle.su2_power_series(a, omega, order))
+        assert np.abs(got - M).max() < 1e-13
+        assert abs(np.linalg.det(got) - 1) < 1e-13 and np.abs(got @ got.conj().T - np.eye(2)).max() < 1e-13
+
+
+def test_series_power_special_cases():
+    rng = np.random.default_rng(6)
+    for phi in (0.1, 0.9, 2.5):
+        a = _unit_quat(rng, phi)
+        # binom(1,n) = 0 for n >= 2 and binom(2,n) = 0 for n >= 3: the series terminates and is exact
+        for order in (1, 2, 5):
+            assert np.abs(oracle.su2_power_series(a, 1.0, order) - a).max() < 1e-14
+        for order in (2, 3, 7):
+            assert np.abs(oracle.su2_power_series(a, 2.0, order) - oracle.su2_power(a, 2.0)).max() < 1e-13
+        # order 1: 1 + omega (g - 1), normalised
+        w = 1.6
+        lin = np.array([1 + w * (a[0] - 1), w * a[1], w * a[2], w * a[3]])
+        assert np.abs(oracle.su2_power_series(a, w, 1) - lin / np.linalg.norm(lin)).max() < 1e-14
+    # |g - 1| = 2 sin(phi/2) < 1: the series converges to the exact power
+    for phi in (0.2, 0.4, 0.6):  # 0.59^120 ~ 1e-28
+        a = _unit_quat(rng, phi)
+        assert np.abs(oracle.su2_power_series(a, 1.7, 120) - oracle.su2_power(a, 1.7)).max() < 1e-12
+    # g = 1 stays 1; g = -1: g - 1 = -2, the sum is a real number, normalised to +-1
+    assert np.abs(oracle.su2_power_series(np.array([1.0, 0, 0, 0]), 1.7, 4) - [1, 0, 0, 0]).max() == 0
+    assert abs(abs(oracle.su2_power_series(np.array([-1.0, 0, 0, 0]), 1.7, 4)[0]) - 1) < 1e-15
+
+
+def test_series_sweep_is_a_gauge_transformation_and_omega1_equals_exact():
+    dims = (4, 4, 4, 4)
+    U0 = gi.make_links(dims, 0.5, 41)
+    try:
+        oracle.set_series(4)
+        assert oracle.get_series() == 4
+        U = U0.copy()
+        oracle.sweeps(U, dims, "landau", 1.7, n=2)
+        Us = U0.copy()
+        oracle.sweeps(Us, dims, "landau", 1.0, n=1)
+    finally:
+        oracle.set_series(0)
+    Ue = U0.copy()
+    oracle.sweeps(Ue, dims, "landau", 1.0, n=1)
+    assert np.abs(Us - Ue).max() < 1e-13          # omega = 1: series = exact
+    Ux = U0.copy()
+    oracle.sweeps(Ux, dims, "landau", 1.7, n=2)
+    assert np.abs(U - Ux).max() > 1e-4            # omega = 1.7, order 4: a different (still valid) update
+    for mu, nu in [(0, 1), (1, 3), (2, 3)]:       # gauge invariance of the plaquette to 1e-12
+        assert np.abs(oracle.wilson_traces(U, dims, mu, nu, 1, 1) - oracle.wilson_traces(U0, dims, mu, nu, 1, 1)).max() < 1e-12
+    uu, det = oracle.unitarity(U, dims)
+    assert uu < 1e-12 and det < 1e-12
+    assert oracle.measure(U, dims, "landau")[0] > oracle.measure(U0, dims, "landau")[0]
