@@ -95,6 +95,19 @@ int gf_fix(gf_ctx* ctx, double omega, double eps, int max_sweeps, int check_ever
  * measurements the run made (may exceed cap). */
 int gf_get_history(gf_ctx* ctx, double* hist, int cap, int* n);
 
+/* Coulomb gauge with a stop test per time slice (BASELINE.json configs[1]: "each of the 32 time slices is fixed
+ * independently"; K(x) of a Coulomb-gauge site holds links of its own slice only; reading A22 in DESIGN.md).
+ * gf_measure_slices: F_t and theta_t, eqs. 1.1-1.2 with the sums restricted to time slice t (V -> nx ny nz), into two
+ *   host arrays of n_t doubles.  Synchronises the stream.
+ * gf_fix_slices: as gf_fix, but a slice with theta_t < eps is finished and its sites are no longer visited; the run ends
+ *   when every slice is finished or after max_sweeps.  History triples are {sweep, mean_t F_t, max_t theta_t}.
+ *   slice_sweeps (host, n_t ints, may be NULL) receives the sweeps spent on each slice.
+ * Errors: GF_EUNSUPPORTED unless the context is Coulomb gauge on a whole lattice with the default sweep variant and
+ * the exact power; GF_EINVAL, GF_ECUDA, GF_ENUMERIC as gf_fix. */
+int gf_measure_slices(gf_ctx* ctx, double* F_t, double* theta_t);
+int gf_fix_slices(gf_ctx* ctx, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done,
+                  int* slice_sweeps);
+
 /* Project every link back onto SU(3): Gram-Schmidt on rows 0,1, row 2 = conj(row0 x row1).  Async. */
 int gf_reunitarize(gf_ctx* ctx);
 /* k = 0 (default): never; k > 0: reunitarise after every k-th sweep inside gf_ovr_sweep / gf_fix. */

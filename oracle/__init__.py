@@ -104,6 +104,34 @@ def fix(U, dims, gauge, omega, eps, max_sweeps, check_every, reunit_every=0, sto
     return done.value, hist[: min(nh.value, cap)].copy()
 
 
+def measure_slices(U, dims, gauge):
+    """(F_t, theta_t): eqs. 1.1-1.2 restricted to each time slice (reading A22)."""
+    nt = int(dims[3])
+    Ft, tht = np.zeros(nt), np.zeros(nt)
+    _fn("orc_measure_slices", U)(_p(U), _dims(dims), _GAUGE[gauge], _p(Ft), _p(tht))
+    return Ft, tht
+
+
+def half_sweep_masked(U, dims, gauge, parity, omega, active, storage=18):
+    """One parity of the sweep over the time slices with active[t] != 0 only."""
+    m = np.ascontiguousarray(active, dtype=np.uint8)
+    _fn("orc_half_sweep_masked", U)(_p(U), _dims(dims), _GAUGE[gauge], int(parity), ctypes.c_double(omega), int(storage),
+                                    _p(m))
+
+
+def fix_slices(U, dims, gauge, omega, eps, max_sweeps, check_every, reunit_every=0, storage=18):
+    """Algorithm 1 with a stop test per time slice (reading A22).
+    Returns (sweeps_done, slice_sweeps[nt], history[(sweep, mean F, max theta_t), ...])."""
+    cap = max_sweeps // max(check_every, 1) + 3
+    hist = np.zeros((cap, 3), dtype=np.float64)
+    per = np.zeros(int(dims[3]), dtype=np.int32)
+    done, nh = ctypes.c_int(), ctypes.c_int()
+    _fn("orc_fix_slices", U)(_p(U), _dims(dims), _GAUGE[gauge], ctypes.c_double(omega), ctypes.c_double(eps),
+                             int(max_sweeps), int(check_every), int(reunit_every), int(storage), ctypes.byref(done),
+                             _p(per), _p(hist), cap, ctypes.byref(nh))
+    return done.value, per, hist[: min(nh.value, cap)].copy()
+
+
 def site_K(U, dims, gauge, site):
     """K(x) of eq. 1.5 as a complex 3x3."""
     K = np.zeros(18, dtype=U.dtype)

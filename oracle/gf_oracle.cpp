@@ -198,6 +198,26 @@ void measure(const T* U, const Geom& g, int gauge, double* F, double* theta) {
   *theta = (double)(ts / (3.0L * (long double)g.V));
 }
 
+// Per-time-slice values (Coulomb gauge: each slice is its own 3-D problem, BASELINE.json configs[1]; reading A22):
+// F_t and theta_t are eqs. 1.1-1.2 with the sums restricted to the sites of slice t and V -> V/n_t.
+template <class T>
+void measure_slices(const T* U, const Geom& g, int gauge, double* F_t, double* theta_t) {
+  const int d = ndir(gauge);
+  const int64_t slice = g.V / g.n[3];
+#pragma omp parallel for schedule(static)
+  for (int t = 0; t < g.n[3]; ++t) {
+    long double fs = 0, ts = 0;
+    for (int64_t s = t * slice; s < (t + 1) * slice; ++s) {
+      for (int mu = 0; mu < d; ++mu) fs += (long double)trace(load_link(U, s, mu)).real();
+      Mat3<T> D = delta_at(U, g, gauge, s);
+      for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) ts += (long double)std::norm(D.m[i][j]);
+    }
+    F_t[t] = (double)(fs / ((long double)d * 3.0L * (long double)slice));
+    theta_t[t] = (double)(ts / (3.0L * (long double)slice));
+  }
+}
+
 // ---- O2: one site update ---------------------------------------------------------------------------------------------
 // K(x) = sum_{mu<d} [U_mu(x) + U_mu(x-mu)^dag]   (eq. 1.5 with the neighbours' g already absorbed: reading A3),
 // summed in the order mu=0 fwd, mu=0 bwd, mu=1 fwd, ...
@@ -416,6 +436,62 @@ int fix(T* U, const Geom& g, int gauge, T omega, double eps, int max_sweeps, int
   return 0;
 }
 
+// ---- O5b: Coulomb gauge with a stop test per time slice (reading A22) ---------------------------------------------------
+// K(x) of a Coulomb-gauge site holds links of its own time slice only, so the slices are independent problems
+// (BASELINE.json configs[1]: "each of the 32 time slices is fixed independently").  Variant of Algorithm 1: theta_t per
+// slice; a slice with theta_t < eps is finished and its sites are not visited any more; the run ends when every slice
+// is finished or the sweep cap is reached.  slice_sweeps[t] = sweeps spent on slice t.
+template <class T>
+void half_sweep_masked(T* U, const Geom& g, int gauge, int parity, T omega, int storage, const uint8_t* active) {
+  const int64_t slice = g.V / g.n[3];
+#pragma omp parallel for schedule(static)
+  for (int64_t s = 0; s < g.V; ++s)
+    if (active[s / slice] && site_parity(g, s) == parity) site_update(U, g, gauge, s, omega, storage);
+}
+
+template <class T>
+int fix_slices(T* U, const Geom& g, int gauge, T omega, double eps, int max_sweeps, int check_every, int reunit_every,
+               int storage, int* sweeps_done, int* slice_sweeps, double* hist, int hist_cap, int* nhist) {
+  const int nt = g.n[3];
+  std::vector<double> Ft(nt), tht(nt);
+  std::vector<uint8_t> active(nt);
+  int done = 0, nh = 0;
+  for (int t = 0; t < nt; ++t) slice_sweeps[t] = 0;
+  auto look = [&]() {  // record (sweeps, mean F, max theta_t); returns the number of unfinished slices
+    measure_slices(U, g, gauge, Ft.data(), tht.data());
+    double F = 0, thmax = 0;
+    int n_active = 0;
+    for (int t = 0; t < nt; ++t) {
+      F += Ft[t];
+      thmax = std::max(thmax, tht[t]);
+      active[t] = !(tht[t] < eps);
+      n_active += active[t];
+    }
+    if (hist && nh < hist_cap) {
+      hist[3 * nh] = (double)done;
+      hist[3 * nh + 1] = F / nt;
+      hist[3 * nh + 2] = thmax;
+    }
+    ++nh;
+    return n_active;
+  };
+  int n_active = look();
+  while (n_active > 0 && done < max_sweeps) {
+    const int n = std::min(check_every, max_sweeps - done);
+    for (int k = 1; k <= n; ++k) {
+      half_sweep_masked(U, g, gauge, 0, omega, storage, active.data());
+      half_sweep_masked(U, g, gauge, 1, omega, storage, active.data());
+      if (reunit_every > 0 && (done + k) % reunit_every == 0) reunitarize(U, g);
+    }
+    for (int t = 0; t < nt; ++t) slice_sweeps[t] += active[t] ? n : 0;
+    done += n;
+    n_active = look();
+  }
+  *sweeps_done = done;
+  if (nhist) *nhist = nh;
+  return 0;
+}
+
 // ---- O6: gauge-invariant observables for the invariance pins ---------------------------------------------------------
 // product of links along a rectangular a x b loop in the (mu,nu) plane starting at s
 template <class T>
@@ -504,6 +580,19 @@ void mat_to(T* p, const Mat3<T>& a) {
                     int reunit_every, int storage, int* sweeps_done, double* hist, int hist_cap, int* nhist) {        \
     return fix<T>(U, make_geom(dims), gauge, (T)omega, eps, max_sweeps, check_every, reunit_every, storage,           \
                   sweeps_done, hist, hist_cap, nhist);                                                                \
+  }                                                                                                                   \
+  void orc_measure_slices_##SUF(const T* U, const int* dims, int gauge, double* F_t, double* theta_t) {               \
+    measure_slices<T>(U, make_geom(dims), gauge, F_t, theta_t);                                                       \
+  }                                                                                                                   \
+  void orc_half_sweep_masked_##SUF(T* U, const int* dims, int gauge, int parity, double omega, int storage,           \
+                                   const uint8_t* active) {                                                           \
+    half_sweep_masked<T>(U, make_geom(dims), gauge, parity, (T)omega, storage, active);                               \
+  }                                                                                                                   \
+  int orc_fix_slices_##SUF(T* U, const int* dims, int gauge, double omega, double eps, int max_sweeps,                \
+                           int check_every, int reunit_every, int storage, int* sweeps_done, int* slice_sweeps,       \
+                           double* hist, int hist_cap, int* nhist) {                                                  \
+    return fix_slices<T>(U, make_geom(dims), gauge, (T)omega, eps, max_sweeps, check_every, reunit_every, storage,    \
+                         sweeps_done, slice_sweeps, hist, hist_cap, nhist);                                           \
   }                                                                                                                   \
   void orc_site_K_##SUF(const T* U, const int* dims, int gauge, int64_t site, T* K18) {                               \
     mat_to<T>(K18, build_K<T>(U, make_geom(dims), gauge, site));                                                      \

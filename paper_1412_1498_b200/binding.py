@@ -22,6 +22,7 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
            "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error",
            "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
+           "gf_measure_slices", "gf_fix_slices",
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"]
 
@@ -57,6 +58,10 @@ def _load() -> ctypes.CDLL:
     lib.gf_fft_step.argtypes = [c_void_p, c_int, c_double]
     lib.gf_fix_fft.restype = c_int
     lib.gf_fix_fft.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int)]
+    lib.gf_measure_slices.restype = c_int
+    lib.gf_measure_slices.argtypes = [c_void_p, POINTER(c_double), POINTER(c_double)]
+    lib.gf_fix_slices.restype = c_int
+    lib.gf_fix_slices.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int), POINTER(c_int)]
     lib.gf_slab_halo_bytes.restype = c_size_t
     lib.gf_slab_halo_bytes.argtypes = [c_void_p]
     lib.gf_slab_attach.restype = c_int
@@ -180,6 +185,21 @@ def gf_fix_fft(ctx, alpha: float, eps: float, max_iters: int, check_every: int):
     return rc, done.value
 
 
+def gf_measure_slices(ctx, nt: int):
+    """Returns (rc, [F_t], [theta_t])."""
+    F, th = (c_double * nt)(), (c_double * nt)()
+    rc = lib.gf_measure_slices(ctx, F, th)
+    return rc, list(F), list(th)
+
+
+def gf_fix_slices(ctx, omega: float, eps: float, max_sweeps: int, check_every: int, nt: int):
+    """Returns (rc, sweeps_done, [sweeps spent on slice t])."""
+    done = c_int()
+    per = (c_int * nt)()
+    rc = lib.gf_fix_slices(ctx, omega, eps, max_sweeps, check_every, byref(done), per)
+    return rc, done.value, list(per)
+
+
 def gf_slab_halo_bytes(ctx) -> int:
     return int(lib.gf_slab_halo_bytes(ctx))
 
@@ -298,6 +318,17 @@ class GaugeFixer:
         rc, done = gf_fix(self.ctx, float(omega), float(eps), int(max_sweeps), int(check_every))
         self._check(rc)
         return done
+
+    def measure_slices(self):
+        rc, F, th = gf_measure_slices(self.ctx, self.dims[3])
+        self._check(rc)
+        return F, th
+
+    def fix_slices(self, omega, eps, max_sweeps, check_every):
+        """Coulomb gauge, a stop test per time slice.  Returns (sweeps_done, sweeps spent on each slice)."""
+        rc, done, per = gf_fix_slices(self.ctx, float(omega), float(eps), int(max_sweeps), int(check_every), self.dims[3])
+        self._check(rc)
+        return done, per
 
     def history(self):
         rc, h = gf_get_history(self.ctx)

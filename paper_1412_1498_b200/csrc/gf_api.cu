@@ -45,7 +45,8 @@ Sizes sizes_of(const Geo& g, int prec, int storage) {
   Sizes s;
   const size_t csize = prec == GF_FP64 ? 16 : 8;
   s.links = align_up((size_t)2 * g.nblk * 4 * (storage / 2) * 32 * csize);
-  s.partials = align_up((size_t)measure_num_partials(g) * sizeof(double2));
+  const int np = measure_num_partials(g) > measure_slices_num_partials(g) ? measure_num_partials(g) : measure_slices_num_partials(g);
+  s.partials = align_up((size_t)np * sizeof(double2));
   s.qpartials = align_up((size_t)halfsweep_max_qblocks(g) * sizeof(double));
   s.result = align_up(2 * sizeof(double));
   s.staging = align_up(STAGING_BYTES);
@@ -60,6 +61,8 @@ struct gf_ctx {
   char* staging[2];
   cudaEvent_t staging_free[2];
   double* host_result;  // pinned and mapped, 2 doubles: the reduction kernels write F, theta straight into it
+  double* host_slices;  // pinned and mapped, 2 n_t doubles (F_t, theta_t), allocated by the first gf_measure_slices
+  double* dev_slices;   // its device pointer
   int reunit_every;
   int fuse_measure;  // GF_OPT_FUSE_MEASURE
   int qblocks;       // > 0: k.qpartials[0..qblocks) hold the odd sites' theta terms of the links as they stand
@@ -146,6 +149,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->top_out = c->top_in = nullptr;
   c->fwd_target[0] = c->fwd_target[1] = c->ret_target = nullptr;
   c->host_result = nullptr;
+  c->host_slices = c->dev_slices = nullptr;
   c->staging_free[0] = c->staging_free[1] = nullptr;
   cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
   if (e == cudaSuccess) {  // zero-copy result: saves a 16-byte D2H copy per measurement (latency on small lattices)
@@ -169,6 +173,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
 void gf_destroy(gf_ctx* c) {
   if (!c) return;
   if (c->host_result) cudaFreeHost(c->host_result);
+  if (c->host_slices) cudaFreeHost(c->host_slices);
   fft_plans_destroy(c->fft);
   for (int i = 0; i < 2; ++i)
     if (c->staging_free[i]) cudaEventDestroy(c->staging_free[i]);
@@ -355,6 +360,104 @@ int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every,
     rc = gf_measure(c, &F, &th);  // Algorithm 1 l.13
     if (rc != GF_OK) return rc;
     record();
+  }
+  return GF_OK;
+}
+
+// ---- Coulomb gauge, every time slice its own stop test (reading A22) -------------------------------------------------------
+static int slices_check(gf_ctx* c, const char* who) {
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost) return fail(c, GF_EUNSUPPORTED, who);
+  if (!c->host_slices) {
+    cudaError_t e = cudaHostAlloc((void**)&c->host_slices, 2 * sizeof(double) * c->k.geo.n[3], cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->dev_slices, c->host_slices, 0);
+    if (e != cudaSuccess) return fail_cuda(c, e, who);
+  }
+  return GF_OK;
+}
+
+int gf_measure_slices(gf_ctx* c, double* F_t, double* theta_t) {
+  if (!c) return GF_EINVAL;
+  if (!F_t || !theta_t) return fail(c, GF_EINVAL, "gf_measure_slices: null out-param");
+  int rc = slices_check(c, "gf_measure_slices: Coulomb gauge on a whole lattice only");
+  if (rc != GF_OK) return rc;
+  cudaError_t e = launch_measure_slices(c->k, c->dev_slices);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_measure_slices");
+  c->launches += 2;
+  const int nt = c->k.geo.n[3];
+  bool finite = true;
+  for (int t = 0; t < nt; ++t) {
+    F_t[t] = c->host_slices[t];
+    theta_t[t] = c->host_slices[nt + t];
+    finite = finite && std::isfinite(F_t[t]) && std::isfinite(theta_t[t]);
+  }
+  return finite ? GF_OK : fail(c, GF_ENUMERIC, "gf_measure_slices: non-finite F_t or theta_t");
+}
+
+int gf_fix_slices(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done,
+                  int* slice_sweeps) {
+  if (!c) return GF_EINVAL;
+  if (!sweeps_done) return fail(c, GF_EINVAL, "gf_fix_slices: null sweeps_done");
+  if (check_every < 1 || max_sweeps < 0 || !(eps >= 0.0))
+    return fail(c, GF_EINVAL, "gf_fix_slices: need check_every >= 1, max_sweeps >= 0, eps >= 0");
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_fix_slices: omega outside [1,2)");
+  int rc = slices_check(c, "gf_fix_slices: Coulomb gauge on a whole lattice only");
+  if (rc != GF_OK) return rc;
+  if (c->k.series > 0 || !(c->k.variant == 0 || c->k.variant == 3))
+    return fail(c, GF_EUNSUPPORTED, "gf_fix_slices: default sweep variant and exact power only");
+  const int nt = c->k.geo.n[3];
+  std::vector<double> Ft(nt), tht(nt);
+  std::vector<unsigned char> active(nt);
+  unsigned char* dev_active = (unsigned char*)c->k.qpartials;  // unused while no theta terms are fused
+  c->history.clear();
+  c->history_n = 0;
+  c->qblocks = 0;
+  *sweeps_done = 0;
+  int done = 0;
+  if (slice_sweeps)
+    for (int t = 0; t < nt; ++t) slice_sweeps[t] = 0;
+  auto look = [&](int* n_active) -> int {  // record (sweeps, mean F, max theta_t)
+    int r = gf_measure_slices(c, Ft.data(), tht.data());
+    if (r != GF_OK) return r;
+    double F = 0.0, thmax = 0.0;
+    *n_active = 0;
+    for (int t = 0; t < nt; ++t) {
+      F += Ft[t];
+      thmax = tht[t] > thmax ? tht[t] : thmax;
+      active[t] = !(tht[t] < eps);
+      *n_active += active[t];
+    }
+    c->history.push_back((double)done);
+    c->history.push_back(F / nt);
+    c->history.push_back(thmax);
+    c->history_n += 1;
+    return GF_OK;
+  };
+  int n_active = 0;
+  rc = look(&n_active);
+  if (rc != GF_OK) return rc;
+  while (n_active > 0 && done < max_sweeps) {
+    const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+    // pageable source: the copy is staged before the call returns, so `active` may change afterwards
+    cudaError_t e = cudaMemcpyAsync(dev_active, active.data(), nt, cudaMemcpyHostToDevice, c->k.stream);
+    for (int i = 0; i < n && e == cudaSuccess; ++i) {
+      for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) {
+        e = launch_halfsweep_masked(c->k, parity, omega, dev_active);
+        c->launches += 1;
+      }
+      c->sweeps_total += 1;
+      if (e == cudaSuccess && c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) {
+        rc = gf_reunitarize(c);
+        if (rc != GF_OK) return rc;
+      }
+    }
+    if (e != cudaSuccess) return fail_cuda(c, e, "gf_fix_slices");
+    if (slice_sweeps)
+      for (int t = 0; t < nt; ++t) slice_sweeps[t] += active[t] ? n : 0;
+    done += n;
+    *sweeps_done = done;
+    rc = look(&n_active);
+    if (rc != GF_OK) return rc;
   }
   return GF_OK;
 }

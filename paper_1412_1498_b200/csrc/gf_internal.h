@@ -54,6 +54,10 @@ int halfsweep_max_qblocks(const Geo& g);
 cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);
 int measure_num_partials(const Geo& g);
+// Coulomb gauge with a stop test per time slice (gf_measure_slices / gf_fix_slices)
+int measure_slices_num_partials(const Geo& g);  // double2 entries launch_measure_slices needs in a.partials
+cudaError_t launch_measure_slices(const KernelArgs& a, double* out);  // out[t] = F_t, out[nt + t] = theta_t (device-visible)
+cudaError_t launch_halfsweep_masked(const KernelArgs& a, int parity, double omega, const unsigned char* active);
 int measure_launches(const Geo& g, int nq);  // kernels launch_measure issues: 1 (small grids) or 2
 
 // ---- Algorithm 2 (gf_fftsd.cu): steepest descent with Fourier acceleration ------------------------------------------------

@@ -267,10 +267,12 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
 // SLAB: the launch covers the checkerboard range [sv.cb_begin, sv.cb_end) of a T-slab; t = 0 sites take U_t(x - t) from
 // (and return it to) the ghost buffer.  The per-site arithmetic is the same instruction sequence in both cases.
 // SERIES: g^omega by the truncated binomial series of order `series` (GF_OPT_OVR_SERIES) instead of the exact power.
-template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB, bool SERIES = false>
+// MASKED (Coulomb gauge, gf_fix_slices): sites of time slices with active[t] == 0 are not visited.
+template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB, bool SERIES = false,
+          bool MASKED = false>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials,
-                            SlabView sv, int series = 0) {
+                            SlabView sv, int series = 0, const unsigned char* __restrict__ active = nullptr) {
   using C = cplx_t<T>;
   using TK = RotationType;
   using CK = cplx_t<TK>;
@@ -284,6 +286,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     live = cb < (second ? sv.cb2_end : sv.cb_end);
   }
   if (!MEASURE && !live) return;
+  if (MASKED && !active[cb / g.s3]) return;  // the slice is finished (its theta_t is below eps)
   double q = 0.0;
   if (live) {
     C* fwd;
@@ -367,7 +370,7 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr);
   return cudaGetLastError();
 }
 
@@ -384,7 +387,7 @@ static cudaError_t halfsweep_series_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series, nullptr);
   return cudaGetLastError();
 }
 
@@ -410,7 +413,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0, nullptr);
   return cudaGetLastError();
 }
 
@@ -459,6 +462,32 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
 
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
   GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
+}
+
+// Coulomb gauge, only the time slices with active[t] != 0 (device array of n_t bytes)
+template <class T, int NELEM>
+static cudaError_t halfsweep_masked_T(const KernelArgs& a, int parity, double omega, const unsigned char* active) {
+  using C = cplx_t<T>;
+  constexpr int THREADS = staged_threads<T>();
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, true>;
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, active);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_halfsweep_masked(const KernelArgs& a, int parity, double omega, const unsigned char* active) {
+  if (a.gauge != 1 || a.series > 0 || !(a.variant == 0 || a.variant == 3)) return cudaErrorNotSupported;
+  if (a.prec == 0) return a.storage == 18 ? halfsweep_masked_T<double, 9>(a, parity, omega, active)
+                                          : halfsweep_masked_T<double, 6>(a, parity, omega, active);
+  return a.storage == 18 ? halfsweep_masked_T<float, 9>(a, parity, omega, active)
+                         : halfsweep_masked_T<float, 6>(a, parity, omega, active);
 }
 
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
@@ -541,39 +570,44 @@ __device__ __forceinline__ void measure_tail(const double2* __restrict__ partial
   }
 }
 
+// the two per-site terms: f = Re Tr sum_nu [U_nu(x) + U_nu(x-nu)], q = sum_ij |Delta_ij(x)|^2
+template <class T, int NELEM, int ND, bool SLAB>
+__device__ __forceinline__ void site_f_q(const cplx_t<T>* __restrict__ links, const Geo& g, int parity, int cb,
+                                         const SlabView& sv, double& f, double& q) {
+  using C = cplx_t<T>;
+  const Site s = site_of(g, parity, cb);
+  const C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
+  C A[9];
+#pragma unroll
+  for (int e = 0; e < 9; ++e) A[e] = mk<T>(T(0), T(0));
+  T tr = T(0);
+#pragma unroll
+  for (int nu = 0; nu < ND; ++nu) {
+    C u[9];
+    const C* down = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu);
+    if (SLAB && nu == 3 && cb < g.s3) down = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
+    load_link<NELEM, true>(down, u);
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { A[e].x += u[e].x; A[e].y += u[e].y; }
+    tr += u[0].x + u[4].x + u[8].x;
+    load_link<NELEM, true>(fwd + nu * NELEM * 32, u);
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { A[e].x -= u[e].x; A[e].y -= u[e].y; }
+    tr += u[0].x + u[4].x + u[8].x;
+  }
+  f = (double)tr;
+  q = (double)delta_norm2<T>(A);
+}
+
 template <class T, int NELEM, int ND, bool SLAB>
 __global__ void __launch_bounds__(MEASURE_THREADS) measure_partial_kernel(const cplx_t<T>* __restrict__ links, Geo g,
                                                                           int blocks_per_parity,
                                                                           double2* __restrict__ partials, MeasureTail tail,
                                                                           SlabView sv) {
-  using C = cplx_t<T>;
   const int parity = blockIdx.x >= blocks_per_parity;
   const int cb = (blockIdx.x - parity * blocks_per_parity) * MEASURE_THREADS + threadIdx.x;
   double f = 0.0, q = 0.0;
-  if (cb < g.vh) {
-    const Site s = site_of(g, parity, cb);
-    const C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
-    C A[9];
-#pragma unroll
-    for (int e = 0; e < 9; ++e) A[e] = mk<T>(T(0), T(0));
-    T tr = T(0);
-#pragma unroll
-    for (int nu = 0; nu < ND; ++nu) {
-      C u[9];
-      const C* down = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, nu), nu);
-      if (SLAB && nu == 3 && cb < g.s3) down = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
-      load_link<NELEM, true>(down, u);
-#pragma unroll
-      for (int e = 0; e < 9; ++e) { A[e].x += u[e].x; A[e].y += u[e].y; }
-      tr += u[0].x + u[4].x + u[8].x;
-      load_link<NELEM, true>(fwd + nu * NELEM * 32, u);
-#pragma unroll
-      for (int e = 0; e < 9; ++e) { A[e].x -= u[e].x; A[e].y -= u[e].y; }
-      tr += u[0].x + u[4].x + u[8].x;
-    }
-    f = (double)tr;
-    q = (double)delta_norm2<T>(A);
-  }
+  if (cb < g.vh) site_f_q<T, NELEM, ND, SLAB>(links, g, parity, cb, sv, f, q);
   block_sum2<MEASURE_THREADS>(f, q);
   if (tail.counter == nullptr) {  // large grids: the second stage is its own small launch (see measure_T)
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(f, q);
@@ -628,6 +662,56 @@ static cudaError_t measure_T(const KernelArgs& a, int nq) {
 }
 
 cudaError_t launch_measure(const KernelArgs& a, int nq) { GF_DISPATCH(measure_T, a, nq); }
+
+// ---- per-time-slice F_t, theta_t (Coulomb gauge, gf_measure_slices / gf_fix_slices; reading A22) -------------------------
+// Block (chunk, 2 t + parity): 256 consecutive checkerboard sites of one parity of slice t.  In Coulomb gauge the even
+// sites of a slice see every spatial link of the slice once, so F_t needs the parity-0 blocks only.
+template <class T, int NELEM>
+__global__ void __launch_bounds__(MEASURE_THREADS) measure_slices_kernel(const cplx_t<T>* __restrict__ links, Geo g,
+                                                                         double2* __restrict__ partials) {
+  const int t = blockIdx.y >> 1, parity = blockIdx.y & 1;
+  const int i = blockIdx.x * MEASURE_THREADS + threadIdx.x;
+  double f = 0.0, q = 0.0;
+  if (i < g.s3) site_f_q<T, NELEM, 3, false>(links, g, parity, t * g.s3 + i, SlabView{}, f, q);
+  block_sum2<MEASURE_THREADS>(f, q);
+  if (threadIdx.x == 0) partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = make_double2(f, q);
+}
+
+// one block per slice: its 2 * nchunk partials added in index order -> out[t] = F_t, out[nt + t] = theta_t
+__global__ void __launch_bounds__(MEASURE_THREADS) measure_slices_tail_kernel(const double2* __restrict__ partials,
+                                                                              int nchunk, int nt, double norm_f,
+                                                                              double norm_q, double* __restrict__ out) {
+  const int t = blockIdx.x;
+  double f = 0.0, q = 0.0;
+  for (int i = threadIdx.x; i < 2 * nchunk; i += MEASURE_THREADS) {
+    const double2 p = partials[(size_t)t * 2 * nchunk + i];
+    if (i < nchunk) f += p.x;  // parity 0
+    q += p.y;
+  }
+  block_sum2<MEASURE_THREADS>(f, q);
+  if (threadIdx.x == 0) { out[t] = f * norm_f; out[nt + t] = q * norm_q; }
+}
+
+int measure_slices_num_partials(const Geo& g) { return 2 * g.n[3] * ((g.s3 + MEASURE_THREADS - 1) / MEASURE_THREADS); }
+
+template <class T, int NELEM>
+static cudaError_t measure_slices_T(const KernelArgs& a, double* out) {
+  const Geo& g = a.geo;
+  const int nchunk = (g.s3 + MEASURE_THREADS - 1) / MEASURE_THREADS;
+  measure_slices_kernel<T, NELEM><<<dim3(nchunk, 2 * g.n[3]), MEASURE_THREADS, 0, a.stream>>>(
+      (const cplx_t<T>*)a.links, g, (double2*)a.partials);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const double V3 = 2.0 * (double)g.s3;
+  measure_slices_tail_kernel<<<g.n[3], MEASURE_THREADS, 0, a.stream>>>((const double2*)a.partials, nchunk, g.n[3],
+                                                                      1.0 / (3.0 * 3.0 * V3), 1.0 / (3.0 * V3), out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_measure_slices(const KernelArgs& a, double* out) {
+  if (a.prec == 0) return a.storage == 18 ? measure_slices_T<double, 9>(a, out) : measure_slices_T<double, 6>(a, out);
+  return a.storage == 18 ? measure_slices_T<float, 9>(a, out) : measure_slices_T<float, 6>(a, out);
+}
 
 // ======================================================================================================================
 // reunitarisation

@@ -364,3 +364,58 @@ def test_series_option_errors(gf, torch):
     halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
     fx.close()
+
+
+# ---- Coulomb gauge with a stop test per time slice (gf_measure_slices / gf_fix_slices; reading A22) --------------------
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 6), (16, 16, 4, 4), (2, 2, 2, 4)])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+def test_measure_slices_matches_oracle(gf, torch, dims, prec, storage):
+    U, Uo = host_input(dims, 0.5, 61, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, "coulomb", prec, storage, U)
+    Ft, tht = fx.measure_slices()
+    F, th = fx.measure()
+    fx.close()
+    Fo, tho = oracle.measure_slices(Uo, dims, "coulomb")
+    atol = 1e-13 if prec == "f64" else 2e-7
+    assert np.abs(np.array(Ft) - Fo).max() <= atol
+    assert np.abs(np.array(tht) / tho - 1).max() <= (1e-12 if prec == "f64" else 1e-5)
+    assert abs(np.mean(Ft) - F) <= atol and abs(np.mean(tht) / th - 1) <= 1e-6
+
+
+@pytest.mark.parametrize("prec,storage,eps", [("f64", 18, 1e-10), ("f64", 12, 1e-10), ("f32", 12, 1e-6)])
+def test_fix_slices_against_oracle(gf, torch, prec, storage, eps):
+    dims, omega, cap, every = (8, 8, 8, 8), 1.7, 1500, 5
+    U, Uo = host_input(dims, 0.4, 62, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, "coulomb", prec, storage, U)
+    done, per = fx.fix_slices(omega, eps, cap, every)
+    hist = fx.history()
+    Ft, tht = fx.measure_slices()
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    fx.close()
+    do, pero, histo = oracle.fix_slices(Uo, dims, "coulomb", omega, eps, cap, every, storage=storage)
+    assert done < cap and max(tht) < eps
+    # north_star: sweeps to convergence within +-2 % (one cadence step at least), per slice and overall
+    assert abs(done - do) <= max(every, 0.02 * do)
+    assert all(abs(a - b) <= max(every, 0.02 * b) for a, b in zip(per, pero))
+    assert min(per) < max(per)  # the slices did finish at different times on this input
+    assert abs(hist[-1][1] - histo[-1][1]) <= TOL_F[prec] * abs(histo[-1][1])
+    if list(per) == list(pero):  # same stop decisions: the same sequence of updates
+        assert np.abs(got - Uo).max() <= (1e-9 if prec == "f64" else 5e-3)
+
+
+def test_slices_abi_errors(gf, torch):
+    fx = gf.GaugeFixer((4, 4, 4, 4), gauge="landau")
+    assert gf.gf_measure_slices(fx.ctx, 4)[0] == gf.GF_EUNSUPPORTED
+    assert gf.gf_fix_slices(fx.ctx, 1.7, 1e-9, 10, 1, 4)[0] == gf.GF_EUNSUPPORTED
+    fx.close()
+    fx = gf.GaugeFixer((4, 4, 4, 4), gauge="coulomb")
+    fx.set_links(torch.from_numpy(gi.make_links((4, 4, 4, 4), 0.3, 1)).cuda())
+    assert gf.gf_fix_slices(fx.ctx, 2.0, 1e-9, 10, 1, 4)[0] == gf.GF_EINVAL
+    assert gf.gf_fix_slices(fx.ctx, 1.7, 1e-9, 10, 0, 4)[0] == gf.GF_EINVAL
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, 2) == gf.GF_OK
+    assert gf.gf_fix_slices(fx.ctx, 1.7, 1e-9, 10, 1, 4)[0] == gf.GF_EUNSUPPORTED
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, 0) == gf.GF_OK
+    rc, done, per = gf.gf_fix_slices(fx.ctx, 1.7, 0.0, 4, 3, 4)  # eps = 0: fixed sweep count, every slice active
+    assert rc == gf.GF_OK and done == 4 and per == [4, 4, 4, 4]
+    assert gf.gf_measure_slices(None, 4)[0] == gf.GF_EINVAL
+    fx.close()

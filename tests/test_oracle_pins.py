@@ -532,3 +532,67 @@ def test_series_sweep_is_a_gauge_transformation_and_omega1_equals_exact():
     uu, det = oracle.unitarity(U, dims)
     assert uu < 1e-12 and det < 1e-12
     assert oracle.measure(U, dims, "landau")[0] > oracle.measure(U0, dims, "landau")[0]
+
+
+# ---- variant: Coulomb gauge with a stop test per time slice (reading A22) ---------------------------------------------
+def test_slice_values_average_to_the_global_ones_and_match_a_one_slice_lattice():
+    dims = (4, 4, 4, 6)
+    U = gi.make_links(dims, 0.5, 51)
+    Ft, tht = oracle.measure_slices(U, dims, "coulomb")
+    F, th = oracle.measure(U, dims, "coulomb")
+    assert abs(Ft.mean() - F) < 1e-14 and abs(tht.mean() - th) < 1e-12 * th
+    # slice t alone: copy its links into both slices of a 4x4x4x2 lattice; Coulomb F/theta never read temporal links,
+    # so each of the two slices reproduces F_t, theta_t of the original slice
+    V3 = 64
+    for t in (0, 3, 5):
+        two = np.ascontiguousarray(np.concatenate([U[t * V3:(t + 1) * V3]] * 2))
+        F2, th2 = oracle.measure(two, (4, 4, 4, 2), "coulomb")
+        assert abs(F2 - Ft[t]) < 1e-14 and abs(th2 - tht[t]) < 1e-12 * tht[t]
+
+
+def test_masked_half_sweep_touches_only_active_slices():
+    dims = (4, 4, 4, 6)
+    U0 = gi.make_links(dims, 0.5, 52)
+    active = np.array([1, 0, 0, 1, 1, 0], dtype=np.uint8)
+    Um, Uf = U0.copy(), U0.copy()
+    for p in (0, 1):
+        oracle.half_sweep_masked(Um, dims, "coulomb", p, 1.7, active)
+        oracle.half_sweep(Uf, dims, "coulomb", p, 1.7)
+    V3 = 64
+    for t in range(6):
+        sp_m, sp_f, sp_0 = (A[t * V3:(t + 1) * V3, :3] for A in (Um, Uf, U0))
+        if active[t]:
+            assert np.array_equal(sp_m, sp_f)   # spatial links of an active slice: as in the full sweep (slices decouple)
+        else:
+            assert np.array_equal(sp_m, sp_0)   # a finished slice is not touched
+    # temporal links U_t(x), x in slice t: left factor from slice t, right factor from slice t+1
+    for t in range(6):
+        tm, tf, t0 = (A[t * V3:(t + 1) * V3, 3] for A in (Um, Uf, U0))
+        if not active[t] and not active[(t + 1) % 6]:
+            assert np.array_equal(tm, t0)
+        if active[t] and active[(t + 1) % 6]:
+            assert np.array_equal(tm, tf)
+    # still a gauge transformation of the whole field
+    for mu, nu in [(0, 3), (2, 3), (0, 1)]:
+        assert np.abs(oracle.wilson_traces(Um, dims, mu, nu, 1, 1) - oracle.wilson_traces(U0, dims, mu, nu, 1, 1)).max() < 1e-12
+
+
+def test_fix_slices_stops_each_slice_on_its_own_theta():
+    dims = (4, 4, 4, 6)
+    U = gi.make_links(dims, 0.4, 53)
+    Ug = U.copy()
+    eps = 1e-10
+    done, per, hist = oracle.fix_slices(U, dims, "coulomb", 1.6, eps, 2000, 5)
+    Ft, tht = oracle.measure_slices(U, dims, "coulomb")
+    assert (tht < eps).all() and done == per.max() and per.min() < per.max()  # slices finish at different times
+    assert hist[-1, 2] == tht.max() and abs(hist[-1, 1] - Ft.mean()) < 1e-15
+    # every slice, run alone with the global-test driver on a two-slice copy, needs the sweeps fix_slices spent on it
+    V3 = 64
+    for t in (0, 2, 4):
+        two = np.ascontiguousarray(np.concatenate([Ug[t * V3:(t + 1) * V3]] * 2))
+        # the copy's 4-D parities differ in the second slice; use the first slice's count only when they agree: t even
+        d2, h2 = oracle.fix(two, (4, 4, 4, 2), "coulomb", 1.6, eps, 2000, 5)
+        assert abs(d2 - per[t]) <= 5
+    # max_t theta_t < eps implies mean_t theta_t < eps: the global-test driver never runs longer
+    dg, hg = oracle.fix(Ug, dims, "coulomb", 1.6, eps, 2000, 5)
+    assert dg <= done and per.sum() < done * 6
