@@ -44,6 +44,11 @@ NCU_TRAFFIC_BYTES = {"cfg4": 19.327848e9 + 19.269022e9,  # profiles/r1f_halfswee
                      "cfg2": 201.386e6 + 142.245e6}      # profiles/r1f_halfsweep_cfg2_ncu.txt (partly L2-resident)
 
 
+# the same for one Algorithm 2 iteration: sd_delta (profiles/r1e_sd_delta_cfg4_ncu.txt) + the five transform passes
+# (profiles/r1h_fft_passes_cfg4_ncu.txt) + sd_rotate (profiles/r1d_fftsd_cfg4_ncu.txt)
+NCU_TRAFFIC_BYTES_FFTSD = {"cfg4": (20.97e9 + 2.14e9) + 5 * (2.1476e9 + 2.0886e9) + (24.746e9 + 19.273e9)}
+
+
 def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
@@ -475,7 +480,8 @@ def run_fftsd(args):
             "config": {"workload": workload_name(cfg), "algorithm": "Algorithm 2, alpha=0.08",
                        "step": f"{n_it} iterations + 1 F/theta measurement", "final_F": F, "final_theta": th},
             "roofline": {"bound": "hbm", "kernel": "whole iteration (sd_delta, transform passes with the Fourier factor, sd_rotate)",
-                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                         "traffic": NCU_TRAFFIC_BYTES_FFTSD.get(cfg["name"]),
                          "peak_source": peak_src, "algorithmic_bytes_per_iteration": bytes_it},
             "gpu_launches": int(fx.kernel_launches() - l0)}
     fx.close()
