@@ -9,8 +9,11 @@
  *     power omega, then g(x) applied to U_mu(x) and U_mu(x-mu) for all four mu (Alg. 1 l.7-8);
  *   - the reduction that gives F (eq. 1.1) and theta (eqs. 1.2-1.3);
  *   - link reunitarisation every k sweeps;
- *   - the driver loop of Algorithm 1 with a measurement cadence.
- * Readings taken where the paper is silent or ambiguous are listed in DESIGN.md (A1-A20).
+ *   - the driver loop of Algorithm 1 with a measurement cadence;
+ * and, to the same parity bar (sections further down): Algorithm 2, steepest descent with Fourier acceleration
+ * (gf_fft_*); the paper's multi-GPU decomposition of the sweep into T-slabs (gf_slab_*); two variants of Algorithm 1
+ * (g^omega as a truncated series, GF_OPT_OVR_SERIES; Coulomb gauge with a stop test per time slice, gf_fix_slices).
+ * Readings taken where the paper is silent or ambiguous are listed in DESIGN.md (A1-A22, B1-B6).
  *
  * Conventions
  *   - Every function returns 0 (GF_OK) or a negative GF_E* code; nothing throws, nothing aborts.

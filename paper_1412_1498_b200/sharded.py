@@ -236,6 +236,8 @@ class ShardedGaugeFixer:
 
     def refresh_ghosts(self):
         """Fill both ghost buffers of every slab from its lower neighbour's top slice (after set_links, reunitarize)."""
+        if self.direct:  # pack_top writes into the upper neighbour's ghost buffer: wait for whatever it still runs
+            self._join_neighbours({s: self.engines[s].mark() for s in self.slabs})
         for q in (0, 1):
             for s in self.slabs:
                 self.engines[s].pack_top(q)
