@@ -111,6 +111,21 @@ int gf_measure_slices(gf_ctx* ctx, double* F_t, double* theta_t);
 int gf_fix_slices(gf_ctx* ctx, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done,
                   int* slice_sweeps);
 
+/* Coulomb gauge with deferred temporal links (SURVEY.md reading A9, "cheaper alternative").  K(x) and
+ * theta never read a temporal link in Coulomb gauge, so U_t need not be rewritten by every site update: once a buffer
+ * is attached, gf_ovr_sweep / gf_fix update the six spatial links of a site and multiply its accumulated rotation
+ * A(x) <- G(x) A(x) (one matrix per site): 6 links + A read and written per site-update instead of 8 links.
+ * U_t(x) <- A(x) U_t(x) A(x+t)^dagger is applied - and A reset to 1 - by gf_defer_flush, and automatically before
+ * gf_get_links[_host], gf_reunitarize, gf_fft_* and on detach; gf_set_links[_host] reset A.  Same result as the in-place
+ * update up to rounding (the products are associated differently).
+ * gf_defer_bytes: size of the buffer (one direction of the link field).  gf_defer_attach(ctx, dev, bytes): caller-owned,
+ *   256-byte aligned, valid until detached with gf_defer_attach(ctx, NULL, 0) or gf_destroy.  Async.
+ * Errors: GF_EUNSUPPORTED unless Coulomb gauge on a whole lattice (gf_fix_slices and gf_slab_attach refuse a context
+ * with deferred links); GF_ENOMEM; GF_ECUDA (also from gf_ovr_sweep with a non-default sweep variant or series). */
+size_t gf_defer_bytes(const gf_ctx* ctx);
+int gf_defer_attach(gf_ctx* ctx, void* dev_acc, size_t bytes);
+int gf_defer_flush(gf_ctx* ctx);
+
 /* Project every link back onto SU(3): Gram-Schmidt on rows 0,1, row 2 = conj(row0 x row1).  Async. */
 int gf_reunitarize(gf_ctx* ctx);
 /* k = 0 (default): never; k > 0: reunitarise after every k-th sweep inside gf_ovr_sweep / gf_fix. */

@@ -22,7 +22,7 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",
            "gf_set_reunit_every", "gf_set_option", "gf_kernel_launches", "gf_destroy", "gf_strerror", "gf_last_error",
            "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
-           "gf_measure_slices", "gf_fix_slices",
+           "gf_measure_slices", "gf_fix_slices", "gf_defer_bytes", "gf_defer_attach", "gf_defer_flush",
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"]
 
@@ -62,6 +62,12 @@ def _load() -> ctypes.CDLL:
     lib.gf_measure_slices.argtypes = [c_void_p, POINTER(c_double), POINTER(c_double)]
     lib.gf_fix_slices.restype = c_int
     lib.gf_fix_slices.argtypes = [c_void_p, c_double, c_double, c_int, c_int, POINTER(c_int), POINTER(c_int)]
+    lib.gf_defer_bytes.restype = c_size_t
+    lib.gf_defer_bytes.argtypes = [c_void_p]
+    lib.gf_defer_attach.restype = c_int
+    lib.gf_defer_attach.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.gf_defer_flush.restype = c_int
+    lib.gf_defer_flush.argtypes = [c_void_p]
     lib.gf_slab_halo_bytes.restype = c_size_t
     lib.gf_slab_halo_bytes.argtypes = [c_void_p]
     lib.gf_slab_attach.restype = c_int
@@ -200,6 +206,18 @@ def gf_fix_slices(ctx, omega: float, eps: float, max_sweeps: int, check_every: i
     return rc, done.value, list(per)
 
 
+def gf_defer_bytes(ctx) -> int:
+    return int(lib.gf_defer_bytes(ctx))
+
+
+def gf_defer_attach(ctx, dev_acc: int, nbytes: int) -> int:
+    return lib.gf_defer_attach(ctx, c_void_p(dev_acc or None), nbytes)
+
+
+def gf_defer_flush(ctx) -> int:
+    return lib.gf_defer_flush(ctx)
+
+
 def gf_slab_halo_bytes(ctx) -> int:
     return int(lib.gf_slab_halo_bytes(ctx))
 
@@ -318,6 +336,20 @@ class GaugeFixer:
         rc, done = gf_fix(self.ctx, float(omega), float(eps), int(max_sweeps), int(check_every))
         self._check(rc)
         return done
+
+    def defer_temporal_links(self, on=True):
+        """Coulomb gauge: keep the sites' accumulated rotations instead of rewriting the temporal links every update."""
+        if on:
+            n = gf_defer_bytes(self.ctx)
+            with self.torch.cuda.device(self.device):
+                self.defer_buffer = self.torch.empty(max(n, 256), dtype=self.torch.uint8, device=self.device)
+            self._check(gf_defer_attach(self.ctx, self.defer_buffer.data_ptr(), n))
+        else:
+            self._check(gf_defer_attach(self.ctx, 0, 0))
+            self.defer_buffer = None
+
+    def defer_flush(self):
+        self._check(gf_defer_flush(self.ctx))
 
     def measure_slices(self):
         rc, F, th = gf_measure_slices(self.ctx, self.dims[3])

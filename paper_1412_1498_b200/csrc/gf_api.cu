@@ -61,6 +61,8 @@ struct gf_ctx {
   char* staging[2];
   cudaEvent_t staging_free[2];
   double* host_result;  // pinned and mapped, 2 doubles: the reduction kernels write F, theta straight into it
+  char* defer_acc;      // gf_defer_attach: the accumulated rotation A(x) of every site, or null
+  bool defer_dirty;     // sweeps have run since the last flush
   double* host_slices;  // pinned and mapped, 2 n_t doubles (F_t, theta_t), allocated by the first gf_measure_slices
   double* dev_slices;   // its device pointer
   int reunit_every;
@@ -150,6 +152,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->fwd_target[0] = c->fwd_target[1] = c->ret_target = nullptr;
   c->host_result = nullptr;
   c->host_slices = c->dev_slices = nullptr;
+  c->defer_acc = nullptr; c->defer_dirty = false;
   c->staging_free[0] = c->staging_free[1] = nullptr;
   cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
   if (e == cudaSuccess) {  // zero-copy result: saves a 16-byte D2H copy per measurement (latency on small lattices)
@@ -180,20 +183,64 @@ void gf_destroy(gf_ctx* c) {
   delete c;
 }
 
+// ---- Coulomb gauge, deferred temporal links (SURVEY.md A9 "cheaper alternative") ---------------------------------------
+static size_t defer_bytes(const gf_ctx* c) {
+  return align_up((size_t)2 * c->k.geo.nblk * (c->k.storage / 2) * 32 * (c->k.prec == GF_FP64 ? 16 : 8));
+}
+static int defer_flush(gf_ctx* c) {
+  if (!c->defer_acc || !c->defer_dirty) return GF_OK;
+  cudaError_t e = launch_defer(c->k, c->defer_acc, true);
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_defer_flush");
+  c->launches += 2;
+  c->defer_dirty = false;
+  return GF_OK;
+}
+
+size_t gf_defer_bytes(const gf_ctx* c) { return c ? defer_bytes(c) : 0; }
+
+int gf_defer_attach(gf_ctx* c, void* dev_acc, size_t bytes) {
+  if (!c) return GF_EINVAL;
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost)
+    return fail(c, GF_EUNSUPPORTED, "gf_defer_attach: Coulomb gauge on a whole lattice only");
+  if (!dev_acc) {  // detach: bring the temporal links up to date first
+    int rc = defer_flush(c);
+    if (rc == GF_OK) c->defer_acc = nullptr;
+    return rc;
+  }
+  if (bytes < defer_bytes(c) || ((uintptr_t)dev_acc % ALIGN)) return fail(c, GF_ENOMEM, "gf_defer_attach: buffer too small or misaligned");
+  int rc = defer_flush(c);
+  if (rc != GF_OK) return rc;
+  c->defer_acc = (char*)dev_acc;
+  cudaError_t e = launch_defer(c->k, c->defer_acc, false);  // A = 1
+  if (e != cudaSuccess) { c->defer_acc = nullptr; return fail_cuda(c, e, "gf_defer_attach"); }
+  c->launches += 1;
+  c->defer_dirty = false;
+  return GF_OK;
+}
+
+int gf_defer_flush(gf_ctx* c) {
+  if (!c) return GF_EINVAL;
+  return defer_flush(c);
+}
+
 int gf_set_links(gf_ctx* c, const void* dev_links) {
   if (!c) return GF_EINVAL;
   if (!dev_links) return fail(c, GF_EINVAL, "gf_set_links: null links");
   cudaError_t e = launch_reorder(c->k, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
+  if (e == cudaSuccess && c->defer_acc && c->defer_dirty) e = launch_defer(c->k, c->defer_acc, false);  // A = 1
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links");
   c->launches += 1;
   c->sweeps_total = 0;
   c->qblocks = 0;
+  c->defer_dirty = false;
   return GF_OK;
 }
 
 int gf_get_links(gf_ctx* c, void* dev_links_out) {
   if (!c) return GF_EINVAL;
   if (!dev_links_out) return fail(c, GF_EINVAL, "gf_get_links: null output");
+  int rc = defer_flush(c);
+  if (rc != GF_OK) return rc;
   cudaError_t e = launch_reorder(c->k, false, dev_links_out, 0, volume(c), nullptr);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_get_links");
   c->launches += 1;
@@ -230,6 +277,11 @@ static int links_host(gf_ctx* c, void* host, bool in) {
 int gf_set_links_host(gf_ctx* c, const void* host_links) {
   if (!c) return GF_EINVAL;
   if (!host_links) return fail(c, GF_EINVAL, "gf_set_links_host: null links");
+  if (c->defer_acc && c->defer_dirty) {
+    cudaError_t e = launch_defer(c->k, c->defer_acc, false);  // A = 1
+    if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links_host");
+    c->defer_dirty = false;
+  }
   c->sweeps_total = 0;
   c->qblocks = 0;
   return links_host(c, const_cast<void*>(host_links), true);
@@ -238,11 +290,15 @@ int gf_set_links_host(gf_ctx* c, const void* host_links) {
 int gf_get_links_host(gf_ctx* c, void* host_links_out) {
   if (!c) return GF_EINVAL;
   if (!host_links_out) return fail(c, GF_EINVAL, "gf_get_links_host: null output");
+  int rc = defer_flush(c);
+  if (rc != GF_OK) return rc;
   return links_host(c, host_links_out, false);
 }
 
 int gf_reunitarize(gf_ctx* c) {
   if (!c) return GF_EINVAL;
+  int rc = defer_flush(c);  // every link is projected as it would stand after an in-place update
+  if (rc != GF_OK) return rc;
   c->qblocks = 0;
   cudaError_t e = launch_reunit(c->k);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_reunitarize");
@@ -298,6 +354,22 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
   if (c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_ovr_sweep: the context is a slab, use gf_slab_halfsweep_*");
   if (n > 0) c->qblocks = 0;
+  if (c->defer_acc) {  // Coulomb gauge, temporal links deferred: 6 links + A(x) per site-update
+    for (int i = 0; i < n; ++i) {
+      for (int parity = 0; parity < 2; ++parity) {
+        cudaError_t e = launch_halfsweep_defer(c->k, parity, omega, c->defer_acc);
+        if (e != cudaSuccess) return fail_cuda(c, e, "gf_ovr_sweep (deferred temporal links)");
+        c->launches += 1;
+      }
+      c->defer_dirty = true;
+      c->sweeps_total += 1;
+      if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) {
+        int rc = gf_reunitarize(c);
+        if (rc != GF_OK) return rc;
+      }
+    }
+    return GF_OK;
+  }
   for (int i = 0; i < n; ++i) {
     for (int parity = 0; parity < 2; ++parity) {  // even first
       // the last odd half-sweep of the call also leaves the odd sites' theta terms for a gf_measure that may follow
@@ -403,8 +475,8 @@ int gf_fix_slices(gf_ctx* c, double omega, double eps, int max_sweeps, int check
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_fix_slices: omega outside [1,2)");
   int rc = slices_check(c, "gf_fix_slices: Coulomb gauge on a whole lattice only");
   if (rc != GF_OK) return rc;
-  if (c->k.series > 0 || !(c->k.variant == 0 || c->k.variant == 3))
-    return fail(c, GF_EUNSUPPORTED, "gf_fix_slices: default sweep variant and exact power only");
+  if (c->k.series > 0 || !(c->k.variant == 0 || c->k.variant == 3) || c->defer_acc)
+    return fail(c, GF_EUNSUPPORTED, "gf_fix_slices: default sweep variant, exact power, no deferred temporal links");
   const int nt = c->k.geo.n[3];
   std::vector<double> Ft(nt), tht(nt);
   std::vector<unsigned char> active(nt);
@@ -551,6 +623,8 @@ static int fft_update(gf_ctx* c, double alpha) {
 }
 
 static int fft_delta(gf_ctx* c) {
+  int rc = defer_flush(c);  // the rotation of Algorithm 2 works on all four directions in place
+  if (rc != GF_OK) return rc;
   cudaError_t e = launch_sd_delta(c->k, c->fft_w);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_fft_step (Delta)");
   c->launches += 1;
@@ -631,6 +705,7 @@ int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
     return fail(c, GF_ENOMEM, "gf_slab_attach: workspace too small or misaligned");
   if (c->fft_w) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: Algorithm 2 is attached to this context");
   if (c->k.series > 0) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: no series variant (GF_OPT_OVR_SERIES) on a slab");
+  if (c->defer_acc) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: temporal links are deferred on this context");
   char* base = (char*)dev_halo;
   c->k.slab.ghost = base;  // ghost[0], ghost[1]
   c->top_out = base + 2 * c->halo_bytes;

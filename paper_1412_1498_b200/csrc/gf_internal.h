@@ -58,6 +58,9 @@ int measure_num_partials(const Geo& g);
 int measure_slices_num_partials(const Geo& g);  // double2 entries launch_measure_slices needs in a.partials
 cudaError_t launch_measure_slices(const KernelArgs& a, double* out);  // out[t] = F_t, out[nt + t] = theta_t (device-visible)
 cudaError_t launch_halfsweep_masked(const KernelArgs& a, int parity, double omega, const unsigned char* active);
+// Coulomb gauge with deferred temporal links (gf_defer_*): acc = one matrix per site, layout of one link direction
+cudaError_t launch_halfsweep_defer(const KernelArgs& a, int parity, double omega, void* acc);
+cudaError_t launch_defer(const KernelArgs& a, void* acc, bool flush);  // flush: U_t <- A U_t A(x+t)^dag; then A <- 1
 int measure_launches(const Geo& g, int nq);  // kernels launch_measure issues: 1 (small grids) or 2
 
 // ---- Algorithm 2 (gf_fftsd.cu): steepest descent with Fourier acceleration ------------------------------------------------

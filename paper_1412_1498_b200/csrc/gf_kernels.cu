@@ -268,11 +268,15 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
 // (and return it to) the ghost buffer.  The per-site arithmetic is the same instruction sequence in both cases.
 // SERIES: g^omega by the truncated binomial series of order `series` (GF_OPT_OVR_SERIES) instead of the exact power.
 // MASKED (Coulomb gauge, gf_fix_slices): sites of time slices with active[t] == 0 are not visited.
+// DEFER (Coulomb gauge, gf_defer_*): the temporal links are not touched; instead the site's accumulated rotation
+// A(x) <- G(x) A(x) is kept in `acc` (one matrix per site, layout of one direction of the link field) and applied to
+// them later in one pass (defer_flush_kernel): 6 links + A read and written per site-update instead of 8 links.
 template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB, bool SERIES = false,
-          bool MASKED = false>
+          bool MASKED = false, bool DEFER = false>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials,
-                            SlabView sv, int series = 0, const unsigned char* __restrict__ active = nullptr) {
+                            SlabView sv, int series = 0, const unsigned char* __restrict__ active = nullptr,
+                            cplx_t<T>* __restrict__ acc = nullptr) {
   using C = cplx_t<T>;
   using TK = RotationType;
   using CK = cplx_t<TK>;
@@ -294,14 +298,21 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
     if (SLAB && cb < g.s3) bwd[3] = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
 
-    // links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu)
+    // links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu); DEFER: slot 6 = A(x), the temporal links stay where they are
+    constexpr int NMU = DEFER ? 3 : 4;
+    C* accp = nullptr;
+    if (DEFER) accp = acc + (((size_t)parity * g.nblk + (size_t)(cb >> 5)) * NELEM) * 32 + (cb & 31);
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
+    for (int mu = 0; mu < NMU; ++mu) {
 #pragma unroll
       for (int e = 0; e < NELEM; ++e) {
         cp_async<sizeof(C)>(sm + ((2 * mu) * NELEM + e) * THREADS, fwd + (mu * NELEM + e) * 32);
         cp_async<sizeof(C)>(sm + ((2 * mu + 1) * NELEM + e) * THREADS, bwd[mu] + e * 32);
       }
+    }
+    if (DEFER) {
+#pragma unroll
+      for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + (6 * NELEM + e) * THREADS, accp + e * 32);
     }
     cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
 
@@ -329,7 +340,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     if (MEASURE) q = (double)delta_norm2<TK>(K);
 
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
+    for (int mu = 0; mu < NMU; ++mu) {
       C u[9], w[9];
       load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
       mul_left<NELEM / 3>(G, u, w);                       // U_mu(x) <- G U_mu(x)
@@ -349,6 +360,12 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
         store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb), w);
       }
       sched_fence();
+    }
+    if (DEFER) {                                          // A(x) <- G A(x)
+      C u[9], w[9];
+      load_link_smem<NELEM, THREADS, true>(sm, 6, u);
+      mul_left<NELEM / 3>(G, u, w);
+      store_link<NELEM>(accp, w);
     }
   }
   if (MEASURE) {
@@ -370,7 +387,7 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr, nullptr);
   return cudaGetLastError();
 }
 
@@ -387,7 +404,7 @@ static cudaError_t halfsweep_series_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series, nullptr);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series, nullptr, nullptr);
   return cudaGetLastError();
 }
 
@@ -413,7 +430,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0, nullptr);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0, nullptr, nullptr);
   return cudaGetLastError();
 }
 
@@ -478,7 +495,7 @@ static cudaError_t halfsweep_masked_T(const KernelArgs& a, int parity, double om
     attr_set = true;
   }
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, active);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, active, nullptr);
   return cudaGetLastError();
 }
 
@@ -488,6 +505,81 @@ cudaError_t launch_halfsweep_masked(const KernelArgs& a, int parity, double omeg
                                           : halfsweep_masked_T<double, 6>(a, parity, omega, active);
   return a.storage == 18 ? halfsweep_masked_T<float, 9>(a, parity, omega, active)
                          : halfsweep_masked_T<float, 6>(a, parity, omega, active);
+}
+
+// Coulomb gauge with deferred temporal links
+template <class T, int NELEM>
+static cudaError_t halfsweep_defer_T(const KernelArgs& a, int parity, double omega, void* acc) {
+  using C = cplx_t<T>;
+  constexpr int THREADS = staged_threads<T>();
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, false, true>;
+  static bool attr_set = false;  // per instantiation
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, nullptr, (C*)acc);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_halfsweep_defer(const KernelArgs& a, int parity, double omega, void* acc) {
+  if (a.gauge != 1 || a.series > 0 || !(a.variant == 0 || a.variant == 3)) return cudaErrorNotSupported;
+  if (a.prec == 0) return a.storage == 18 ? halfsweep_defer_T<double, 9>(a, parity, omega, acc)
+                                          : halfsweep_defer_T<double, 6>(a, parity, omega, acc);
+  return a.storage == 18 ? halfsweep_defer_T<float, 9>(a, parity, omega, acc)
+                         : halfsweep_defer_T<float, 6>(a, parity, omega, acc);
+}
+
+// U_t(x) <- A(x) U_t(x) A(x+t)^dagger for every site (one thread per site, both parities), then A <- 1 (second kernel:
+// a site's A is also its lower t-neighbour's right factor).
+template <class T, int NELEM>
+__global__ void __launch_bounds__(256) defer_flush_kernel(cplx_t<T>* __restrict__ links, Geo g,
+                                                          const cplx_t<T>* __restrict__ acc) {
+  using C = cplx_t<T>;
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= 2 * g.vh) return;
+  const int parity = i >= g.vh, cb = i - parity * g.vh;
+  const Site s = site_of(g, parity, cb);
+  const int cb_up = s.t == g.n[3] - 1 ? cb - g.s3 * (g.n[3] - 1) : cb + g.s3;
+  C* ut = links + link_offset<NELEM>(g, parity, cb, 3);
+  C A[9], u[9], w[9];
+  load_link<NELEM, true>(acc + (((size_t)parity * g.nblk + (size_t)(cb >> 5)) * NELEM) * 32 + (cb & 31), A);
+  load_link<NELEM, true>(ut, u);
+  mul_left<NELEM / 3>(A, u, w);
+  load_link<NELEM, true>(acc + (((size_t)(parity ^ 1) * g.nblk + (size_t)(cb_up >> 5)) * NELEM) * 32 + (cb_up & 31), A);
+  mul_right_adj<NELEM / 3>(w, A, u);
+  store_link<NELEM>(ut, u);
+}
+
+template <class T, int NELEM>
+__global__ void __launch_bounds__(256) defer_identity_kernel(cplx_t<T>* __restrict__ acc, long long ntiles) {
+  const long long tid = (long long)blockIdx.x * 256 + threadIdx.x;
+  if ((tid >> 5) >= ntiles) return;
+  cplx_t<T>* p = acc + (size_t)(tid >> 5) * NELEM * 32 + (tid & 31);
+#pragma unroll
+  for (int e = 0; e < NELEM; ++e) p[e * 32] = mk<T>((e % 4 == 0) ? T(1) : T(0), T(0));
+}
+
+template <class T, int NELEM>
+static cudaError_t defer_T(const KernelArgs& a, void* acc, bool flush) {
+  if (flush) {
+    defer_flush_kernel<T, NELEM><<<(unsigned)((2LL * a.geo.vh + 255) / 256), 256, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo,
+                                                                                              (const cplx_t<T>*)acc);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  const long long ntiles = 2LL * a.geo.nblk;
+  defer_identity_kernel<T, NELEM><<<(unsigned)((ntiles * 32 + 255) / 256), 256, 0, a.stream>>>((cplx_t<T>*)acc, ntiles);
+  return cudaGetLastError();
+}
+
+// flush = true: apply the accumulated rotations to the temporal links; then (always) A <- 1
+cudaError_t launch_defer(const KernelArgs& a, void* acc, bool flush) {
+  if (a.prec == 0) return a.storage == 18 ? defer_T<double, 9>(a, acc, flush) : defer_T<double, 6>(a, acc, flush);
+  return a.storage == 18 ? defer_T<float, 9>(a, acc, flush) : defer_T<float, 6>(a, acc, flush);
 }
 
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,

@@ -419,3 +419,74 @@ def test_slices_abi_errors(gf, torch):
     assert rc == gf.GF_OK and done == 4 and per == [4, 4, 4, 4]
     assert gf.gf_measure_slices(None, 4)[0] == gf.GF_EINVAL
     fx.close()
+
+
+# ---- Coulomb gauge with deferred temporal links (gf_defer_*) -------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4), (2, 2, 2, 2), (16, 4, 4, 6)])
+@pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
+@pytest.mark.parametrize("sweeps", [1, 3])
+def test_deferred_temporal_links_against_oracle_and_in_place(gf, torch, dims, prec, storage, sweeps):
+    omega = 1.7
+    U, Uo = host_input(dims, 0.5, 71, prec, storage)
+    fx = gpu_fixer(gf, torch, dims, "coulomb", prec, storage, U)
+    fx.defer_temporal_links()
+    l0 = fx.kernel_launches()
+    fx.ovr_sweep(sweeps, omega)
+    assert fx.kernel_launches() - l0 == 2 * sweeps
+    F, th = fx.measure()                      # Coulomb F and theta do not read temporal links: valid before the flush
+    got = fx.get_links().cpu().numpy().astype(np.float64)   # flushes
+    again = fx.get_links().cpu().numpy().astype(np.float64)  # nothing left to flush
+    fx.defer_flush()
+    fx.defer_temporal_links(False)
+    fx.set_links(torch.from_numpy(U).cuda())
+    fx.ovr_sweep(sweeps, omega)
+    inplace = fx.get_links().cpu().numpy().astype(np.float64)
+    Fi, thi = fx.measure()
+    fx.close()
+    oracle.sweeps(Uo, dims, "coulomb", omega, n=sweeps, storage=storage)
+    Fo, tho = oracle.measure(Uo, dims, "coulomb")
+    assert np.array_equal(got, again)
+    assert np.abs(got - Uo).max() <= sweeps * TOL_LINK[prec]
+    assert np.array_equal(got[:, :3], inplace[:, :3])          # spatial links: the same instruction sequence
+    assert np.abs(got[:, 3] - inplace[:, 3]).max() <= sweeps * (1e-14 if prec == "f64" else 5e-6)
+    assert abs(F - Fo) <= TOL_F[prec] * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
+    assert abs(F - Fi) <= 1e-6 * abs(Fi)
+
+
+def test_deferred_links_whole_run_with_reunitarisation_and_errors(gf, torch):
+    dims, omega, eps, cap, every = (8, 8, 8, 8), 1.7, 1e-9, 600, 10
+    U, Uo = host_input(dims, 0.3, 72, "f64", 18)
+    fx = gpu_fixer(gf, torch, dims, "coulomb", "f64", 18, U)
+    fx.set_reunit_every(20)
+    fx.defer_temporal_links()
+    done = fx.fix(omega, eps, cap, every)
+    hist = fx.history()
+    got = fx.get_links().cpu().numpy()
+    assert gf.gf_fix_slices(fx.ctx, omega, eps, cap, every, dims[3])[0] == gf.GF_EUNSUPPORTED
+    fx.close()
+    do, histo = oracle.fix(Uo, dims, "coulomb", omega, eps, cap, every, reunit_every=20)
+    assert abs(done - do) <= max(every, 0.02 * do) and done < cap
+    assert abs(hist[-1][1] - histo[-1][1]) <= 1e-10 * abs(histo[-1][1])
+    if done == do:
+        assert np.abs(got - Uo).max() <= 1e-9
+    a, b = oracle.unitarity(np.ascontiguousarray(got), dims)
+    assert a < 1e-12 and b < 1e-12
+    # gauge invariance of the flushed field: temporal plaquettes as in the input
+    for mu in (0, 2):
+        assert np.abs(oracle.wilson_traces(np.ascontiguousarray(got), dims, mu, 3, 1, 1)
+                      - oracle.wilson_traces(np.ascontiguousarray(U), dims, mu, 3, 1, 1)).max() < 1e-11
+    fx = gf.GaugeFixer((4, 4, 4, 4), gauge="landau")
+    assert gf.gf_defer_attach(fx.ctx, 256, 1 << 20) == gf.GF_EUNSUPPORTED
+    fx.close()
+    fx = gf.GaugeFixer((4, 4, 4, 4), gauge="coulomb")
+    n = gf.gf_defer_bytes(fx.ctx)
+    buf = torch.empty(n, dtype=torch.uint8, device="cuda")
+    assert n >= 4 ** 4 * 9 * 16 and gf.gf_defer_bytes(None) == 0
+    assert gf.gf_defer_attach(fx.ctx, buf.data_ptr(), n - 1) == gf.GF_ENOMEM
+    assert gf.gf_defer_attach(fx.ctx, buf.data_ptr(), n) == gf.GF_OK
+    B = gf.gf_slab_halo_bytes(fx.ctx)
+    halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
+    assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
+    assert gf.gf_defer_attach(fx.ctx, 0, 0) == gf.GF_OK and gf.gf_defer_flush(fx.ctx) == gf.GF_OK
+    assert gf.gf_defer_flush(None) == gf.GF_EINVAL
+    fx.close()
