@@ -13,7 +13,11 @@
 // a 2^4 lattice; eq. 1.6 closed form on SU(2)-embedded fields; g^omega group properties; gauge invariance of
 // plaquettes, Wilson and Polyakov loops to 1e-12; unitarity/det to 1e-12; F monotone at omega=1 (per site update and
 // per sweep); site-order independence; 2-site translation covariance; Coulomb slice independence; 12-real emulation;
-// reunitarisation idempotence.  The whole trajectory on the five configs (sweep counts, final F) is "parity unpinned"
+// reunitarisation idempotence; for the two variants (readings A21, A22): the truncated series of g^omega against the
+// binomial series of 2x2 numpy matrices, its terminating (omega = 1, 2) and order-1 closed forms, convergence to the
+// exact power, gauge invariance of a series sweep; per-slice F_t / theta_t against the global values and against the
+// slice copied into a two-slice lattice, masked half-sweeps (finished slices untouched, active ones as in the full
+// sweep), per-slice sweep counts against each slice run alone.  The whole trajectory on the five configs (sweep counts, final F) is "parity unpinned"
 // by the paper, which prints no numbers (last row of the pin table).
 //
 // Canonical layout: links[site][mu][row][col][re,im], site = x + nx*(y + ny*(z + nz*t)) (x fastest),
