@@ -353,19 +353,24 @@ def run_ours(args):
             host2.copy_(host)
             lanes.append((fx2, host2))
 
+        import threading
+
+        # one upload and one download at a time: two copies in the same direction would only share the bus
+        up_lock, down_lock = threading.Lock(), threading.Lock()
+
         def e2e_step(lane, uploaded=None):
             f, h = lane
-            f.set_links_host(h)
+            with up_lock:
+                f.set_links_host(h)
             if uploaded is not None:
                 uploaded.set()
             f.ovr_sweep(n_sw, omega)
             r = f.measure()
-            f.get_links_host(h)
+            with down_lock:
+                f.get_links_host(h)
             return r
 
         def run_lanes(n):
-            import threading
-
             # lane k starts once lane k-1 has finished its first upload: the lanes run out of phase, so one lane's
             # upload meets another's download instead of its upload
             gates = [threading.Event() for _ in lanes]
@@ -606,7 +611,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=4, help="end-to-end steps per lane")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-lanes", type=int, default=2,
-                    help="fields in flight in the end-to-end leg (measured on cfg4: 1 lane 0.69 G, 2 lanes 0.97 G, 3 lanes 0.85 G)")
+                    help="fields in flight in the end-to-end leg (measured on cfg4: 1 lane 0.69 G, 2 lanes 1.00 G, 4 lanes 1.05 G)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-contract", action="store_true", help="skip the timed whole-config gf_fix run")
     ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
