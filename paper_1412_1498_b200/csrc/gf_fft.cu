@@ -199,8 +199,10 @@ struct LineArgs {
   double scale_p2max;
 };
 
+// The fused pass with 16-point FP64 transforms wants 164 registers (3 blocks of 128 threads per SM); capped at 128
+// (a 128-byte spill) a fourth block fits.
 template <class T, int MODE, int MAXR>
-__global__ void __launch_bounds__(256) fft_line_kernel(cplx_t<T>* __restrict__ w, LineArgs a) {
+__global__ void __launch_bounds__(256, (MODE == LINE_FUSED && MAXR == 16) ? 2 : 1) fft_line_kernel(cplx_t<T>* __restrict__ w, LineArgs a) {
   using C = cplx_t<T>;
   extern __shared__ __align__(16) unsigned char line_smem[];
   C* tile = reinterpret_cast<C*>(line_smem);
