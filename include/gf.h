@@ -43,14 +43,18 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 
 enum { GF_LANDAU = 0, GF_COULOMB = 1 }; /* PAPER.md:35 */
 enum { GF_FP64 = 0, GF_FP32 = 1 };      /* PAPER.md:140 (SP/DP) */
-/* storage: 18 (full 3x3) or 12 (rows 0,1 stored; row 2 = conj(row0 x row1) rebuilt at every load) reals per link,
- * PAPER.md:128, 144 */
+/* storage: 18 (full 3x3), 12 (rows 0,1 stored; row 2 = conj(row0 x row1) rebuilt at every load) or 8 reals per link,
+ * PAPER.md:128, 144, 174.  8 (GF_FP64 only; reading A23 in DESIGN.md): a2, a3, b1 and the phases of a1 and c1 are kept,
+ * the rest follows from unitarity and det = 1 with a division by N = |a2|^2 + |a3|^2 - undefined for block-diagonal
+ * links (N = 0, e.g. the unit field) and less accurate the smaller N is.  With storage = 8 the library offers
+ * gf_set/get_links[_host], gf_ovr_sweep, gf_measure, gf_fix, gf_reunitarize; the gf_fft_*, gf_slab_*, gf_defer_*,
+ * gf_*_slices calls and GF_OPT_OVR_SERIES return GF_EUNSUPPORTED. */
 
 enum {
   GF_OK = 0,
   GF_EINVAL = -1,       /* null pointer, n < 0, check_every < 1, omega outside [1,2) (PAPER.md:50), bad option */
   GF_EODD = -2,         /* an extent is odd or < 2 (PAPER.md:132-134: all lattice dimensions must be even) */
-  GF_EUNSUPPORTED = -3, /* storage not in {12,18}, unknown gauge / precision, V >= 2^31 */
+  GF_EUNSUPPORTED = -3, /* storage not in {8,12,18} (8: FP64 only), unknown gauge / precision, V >= 2^31 */
   GF_ENOMEM = -4,       /* workspace too small or misaligned (256-byte alignment required) */
   GF_ECUDA = -5,        /* a CUDA call failed; text via gf_last_error */
   GF_ENUMERIC = -6      /* F or theta came back NaN/Inf */

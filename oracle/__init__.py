@@ -93,6 +93,11 @@ def project12(U, dims):
     _fn("orc_project12", U)(_p(U), _dims(dims))
 
 
+def project8(U, dims):
+    """Send every link through the 8-real parametrisation and back: what 8-real storage does to its input (A23)."""
+    _fn("orc_project8", U)(_p(U), _dims(dims))
+
+
 def fix(U, dims, gauge, omega, eps, max_sweeps, check_every, reunit_every=0, storage=18):
     """Algorithm 1 with a measurement cadence.  Returns (sweeps_done, history[(sweep, F, theta), ...])."""
     cap = max_sweeps // max(check_every, 1) + 3

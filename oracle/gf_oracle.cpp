@@ -152,6 +152,26 @@ void rebuild_row2(Mat3<T>& a) {
   a.m[2][2] = std::conj(a.m[0][0] * a.m[1][1] - a.m[0][1] * a.m[1][0]);
 }
 
+// 8-real storage ("Elems = 4", 144, 174; reading A23): a link is kept as a2, a3, b1 (row 0 columns 1,2;
+// row 1 column 0) and the phases of a1 and c1 (rows a, b, c).  Everything else follows from unitarity and det = 1:
+//   N = |a2|^2 + |a3|^2;  |a1| = sqrt(1 - N);  |c1| = sqrt(N - |b1|^2)      (row a and column 0 have unit norm)
+//   (b2, b3) = alpha (a2, a3) + beta (-conj a3, conj a2),  alpha = -conj(a1) b1 / N  (row b orthogonal to row a),
+//   beta = conj(c1) / N  (c1 = conj(a2 b3 - a3 b2));  row c = conj(a x b).
+// Undefined for N = 0 (block-diagonal links) and ill-conditioned near it: rounding is amplified by 1/N.
+template <class T>
+void roundtrip8(Mat3<T>& u) {
+  const Cx<T> a2 = u.m[0][1], a3 = u.m[0][2], b1 = u.m[1][0];
+  const T th_a = std::arg(u.m[0][0]), th_c = std::arg(u.m[2][0]);
+  const T N = std::norm(a2) + std::norm(a3);
+  const Cx<T> a1 = std::polar(std::sqrt(std::max(T(0), T(1) - N)), th_a);
+  const Cx<T> c1 = std::polar(std::sqrt(std::max(T(0), N - std::norm(b1))), th_c);
+  const Cx<T> alpha = -std::conj(a1) * b1 / N, beta = std::conj(c1) / N;
+  u.m[0][0] = a1;
+  u.m[1][1] = alpha * a2 - beta * std::conj(a3);
+  u.m[1][2] = alpha * a3 + beta * std::conj(a2);
+  rebuild_row2(u);  // row c = conj(a x b); its first entry reproduces c1 up to rounding
+}
+
 int ndir(int gauge) { return gauge == 1 ? 3 : 4; }  // Landau mu=0..3, Coulomb mu=0..2
 
 // ---- O1: F (eq. 1.1) and theta (eqs. 1.2-1.3), g == 1 because transformations are applied to the links in place -----
@@ -347,10 +367,12 @@ void site_update(T* U, const Geom& g, int gauge, int64_t s, T omega, int storage
   for (int mu = 0; mu < 4; ++mu) {
     Mat3<T> f = mul(G, load_link(U, s, mu));  // U_mu(x) <- G U_mu(x)
     if (storage == 12) rebuild_row2(f);
+    if (storage == 8) roundtrip8(f);
     store_link(U, s, mu, f);
     const int64_t sb = neighbour(g, s, mu, -1);
     Mat3<T> b = mul(load_link(U, sb, mu), Gd);  // U_mu(x-mu) <- U_mu(x-mu) G^dag
     if (storage == 12) rebuild_row2(b);
+    if (storage == 8) roundtrip8(b);
     store_link(U, sb, mu, b);
   }
 }
@@ -396,6 +418,17 @@ void project12(T* U, const Geom& g) {  // what gf_set_links does to the input wh
     for (int mu = 0; mu < 4; ++mu) {
       Mat3<T> a = load_link(U, s, mu);
       rebuild_row2(a);
+      store_link(U, s, mu, a);
+    }
+}
+
+template <class T>
+void project8(T* U, const Geom& g) {  // what gf_set_links does to the input when storage = 8 (reading A23)
+#pragma omp parallel for schedule(static)
+  for (int64_t s = 0; s < g.V; ++s)
+    for (int mu = 0; mu < 4; ++mu) {
+      Mat3<T> a = load_link(U, s, mu);
+      roundtrip8(a);
       store_link(U, s, mu, a);
     }
 }
@@ -580,6 +613,7 @@ void mat_to(T* p, const Mat3<T>& a) {
   }                                                                                                                   \
   void orc_reunitarize_##SUF(T* U, const int* dims) { reunitarize<T>(U, make_geom(dims)); }                           \
   void orc_project12_##SUF(T* U, const int* dims) { project12<T>(U, make_geom(dims)); }                               \
+  void orc_project8_##SUF(T* U, const int* dims) { project8<T>(U, make_geom(dims)); }                                 \
   int orc_fix_##SUF(T* U, const int* dims, int gauge, double omega, double eps, int max_sweeps, int check_every,      \
                     int reunit_every, int storage, int* sweeps_done, double* hist, int hist_cap, int* nhist) {        \
     return fix<T>(U, make_geom(dims), gauge, (T)omega, eps, max_sweeps, check_every, reunit_every, storage,           \

@@ -108,7 +108,8 @@ extern "C" {
 size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage) {
   int err;
   if (!valid_lattice(nx, ny, nz, nt, &err)) return 0;
-  if ((prec != GF_FP64 && prec != GF_FP32) || (storage != 18 && storage != 12)) return 0;
+  if ((prec != GF_FP64 && prec != GF_FP32) || (storage != 18 && storage != 12 && storage != 8)) return 0;
+  if (storage == 8 && prec != GF_FP64) return 0;
   return sizes_of(make_geo(nx, ny, nz, nt), prec, storage).total;
 }
 
@@ -120,7 +121,8 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   if (!valid_lattice(nx, ny, nz, nt, &err)) return err;
   if (gauge != GF_LANDAU && gauge != GF_COULOMB) return GF_EUNSUPPORTED;
   if (prec != GF_FP64 && prec != GF_FP32) return GF_EUNSUPPORTED;
-  if (storage != 18 && storage != 12) return GF_EUNSUPPORTED;
+  if (storage != 18 && storage != 12 && storage != 8) return GF_EUNSUPPORTED;
+  if (storage == 8 && prec != GF_FP64) return GF_EUNSUPPORTED;  // 1/N amplification of rounding: FP64 only (reading A23)
   if (!dev_workspace) return GF_EINVAL;
   const Geo g = make_geo(nx, ny, nz, nt);
   const Sizes sz = sizes_of(g, prec, storage);
@@ -200,8 +202,8 @@ size_t gf_defer_bytes(const gf_ctx* c) { return c ? defer_bytes(c) : 0; }
 
 int gf_defer_attach(gf_ctx* c, void* dev_acc, size_t bytes) {
   if (!c) return GF_EINVAL;
-  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost)
-    return fail(c, GF_EUNSUPPORTED, "gf_defer_attach: Coulomb gauge on a whole lattice only");
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8)
+    return fail(c, GF_EUNSUPPORTED, "gf_defer_attach: Coulomb gauge on a whole lattice only, 18- or 12-real storage");
   if (!dev_acc) {  // detach: bring the temporal links up to date first
     int rc = defer_flush(c);
     if (rc == GF_OK) c->defer_acc = nullptr;
@@ -335,7 +337,8 @@ int gf_set_option(gf_ctx* c, int key, int value) {
       return GF_OK;
     case GF_OPT_OVR_SERIES:
       if (value < 0 || value > 16) return fail(c, GF_EINVAL, "gf_set_option: series order outside 0..16");
-      if (value > 0 && c->k.slab.ghost) return fail(c, GF_EUNSUPPORTED, "gf_set_option: no series variant on a slab context");
+      if (value > 0 && (c->k.slab.ghost || c->k.storage == 8))
+        return fail(c, GF_EUNSUPPORTED, "gf_set_option: no series variant on a slab context or with 8-real storage");
       c->k.series = value;
       c->qblocks = 0;
       return GF_OK;
@@ -438,7 +441,7 @@ int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every,
 
 // ---- Coulomb gauge, every time slice its own stop test (reading A22) -------------------------------------------------------
 static int slices_check(gf_ctx* c, const char* who) {
-  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost) return fail(c, GF_EUNSUPPORTED, who);
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, who);
   if (!c->host_slices) {
     cudaError_t e = cudaHostAlloc((void**)&c->host_slices, 2 * sizeof(double) * c->k.geo.n[3], cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->dev_slices, c->host_slices, 0);
@@ -545,6 +548,7 @@ int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
 
 // ---- Algorithm 2: steepest descent with Fourier acceleration -------------------------------------
 static int fft_plan(gf_ctx* c) {
+  if (c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not built for 8-real storage");
   if (c->k.slab.ghost)  // no multi-GPU steepest descent (no distributed 4-D transform)
     return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not available on a slab context");
   if (c->fft) return GF_OK;
@@ -701,6 +705,7 @@ size_t gf_slab_halo_bytes(const gf_ctx* c) { return c ? c->halo_bytes : 0; }
 int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
   if (!c) return GF_EINVAL;
   if (!dev_halo) return fail(c, GF_EINVAL, "gf_slab_attach: null workspace");
+  if (c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: not built for 8-real storage");
   if (bytes < 4 * c->halo_bytes || ((uintptr_t)dev_halo % ALIGN))
     return fail(c, GF_ENOMEM, "gf_slab_attach: workspace too small or misaligned");
   if (c->fft_w) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: Algorithm 2 is attached to this context");

@@ -90,17 +90,65 @@ __device__ __forceinline__ int cb_down(const Geo& g, const Site& s, int cb, int 
   }
 }
 
+// ---- 8-real storage (NELEM = 4; "Elems = 4", 144, 174; reading A23) --------------------------------------------
+// Stored: a2, a3, b1 and (arg a1, arg c1) for the rows a, b, c of the link.  With N = |a2|^2 + |a3|^2:
+//   |a1| = sqrt(1 - N), |c1| = sqrt(N - |b1|^2)  (row a and column 0 have unit norm);
+//   (b2, b3) = alpha (a2, a3) + beta (-conj a3, conj a2), alpha = -conj(a1) b1 / N, beta = conj(c1) / N;  c = conj(a x b).
+// Undefined for N = 0 (block-diagonal links); rounding is amplified by 1/N near it.
+__device__ __forceinline__ double hypot2_(double x, double y) { return x * x + y * y; }
+__device__ __forceinline__ float hypot2_(float x, float y) { return x * x + y * y; }
+__device__ __forceinline__ void sincos8_(double a, double* s, double* c) { sincos(a, s, c); }
+__device__ __forceinline__ void sincos8_(float a, float* s, float* c) { sincosf(a, s, c); }
+
+template <class T, class C>
+__device__ __forceinline__ void decode8(const C a2, const C a3, const C b1, const C phases, C (&u)[9]) {
+  const T N = hypot2_(a2.x, a2.y) + hypot2_(a3.x, a3.y);
+  T sn, cs;
+  sincos8_(phases.x, &sn, &cs);
+  const T ra = sqrt(fmax(T(0), T(1) - N));
+  const C a1 = mk<T>(ra * cs, ra * sn);
+  sincos8_(phases.y, &sn, &cs);
+  const T rc = sqrt(fmax(T(0), N - hypot2_(b1.x, b1.y)));
+  const C c1 = mk<T>(rc * cs, rc * sn);
+  const T invN = T(1) / N;
+  // alpha = -conj(a1) b1 / N, beta = conj(c1) / N
+  const C alpha = mk<T>(-(a1.x * b1.x + a1.y * b1.y) * invN, -(a1.x * b1.y - a1.y * b1.x) * invN);
+  const C beta = mk<T>(c1.x * invN, -c1.y * invN);
+  u[0] = a1; u[1] = a2; u[2] = a3; u[3] = b1;
+  // b2 = alpha a2 - beta conj(a3);  b3 = alpha a3 + beta conj(a2)
+  u[4] = mk<T>(alpha.x * a2.x - alpha.y * a2.y - (beta.x * a3.x + beta.y * a3.y),
+               alpha.x * a2.y + alpha.y * a2.x - (beta.y * a3.x - beta.x * a3.y));
+  u[5] = mk<T>(alpha.x * a3.x - alpha.y * a3.y + (beta.x * a2.x + beta.y * a2.y),
+               alpha.x * a3.y + alpha.y * a3.x + (beta.y * a2.x - beta.x * a2.y));
+  rebuild_row2(u);
+}
+
+// rows of a product that a store of this storage format needs: 18 reals 3, 12 reals 2, 8 reals 3 (it reads c1)
+template <int NELEM> struct LinkRows { static constexpr int value = NELEM == 6 ? 2 : 3; };
+
 // ---- link load / store in the internal layout ------------------------------------------------------------------------------
-template <int NELEM, bool FULL, class C>
+// STRIDE: distance between consecutive elements of one link (32 in the global layout; THREADS in the shared staging area)
+template <int NELEM, bool FULL, int STRIDE = 32, class C>
 __device__ __forceinline__ void load_link(const C* __restrict__ p, C (&u)[9]) {
+  if constexpr (NELEM == 4) {
+    using T = decltype(u[0].x);
+    decode8<T>(p[0], p[STRIDE], p[2 * STRIDE], p[3 * STRIDE], u);
+  } else {
 #pragma unroll
-  for (int e = 0; e < NELEM; ++e) u[e] = p[e * 32];
-  if (NELEM == 6 && FULL) rebuild_row2(u);
+    for (int e = 0; e < NELEM; ++e) u[e] = p[e * STRIDE];
+    if (NELEM == 6 && FULL) rebuild_row2(u);
+  }
 }
 template <int NELEM, class C>
 __device__ __forceinline__ void store_link(C* __restrict__ p, const C (&u)[9]) {
+  if constexpr (NELEM == 4) {
+    using T = decltype(u[0].x);
+    p[0] = u[1]; p[32] = u[2]; p[64] = u[3];
+    p[96] = mk<T>(atan2(u[0].y, u[0].x), atan2(u[6].y, u[6].x));
+  } else {
 #pragma unroll
-  for (int e = 0; e < NELEM; ++e) p[e * 32] = u[e];
+    for (int e = 0; e < NELEM; ++e) p[e * 32] = u[e];
+  }
 }
 
 // ---- SU(2) subgroup step with overrelaxation -------------------------------------------------------------------------------

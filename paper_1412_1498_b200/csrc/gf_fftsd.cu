@@ -405,8 +405,8 @@ __global__ void __launch_bounds__(SD_THREADS) sd_rotate_kernel(cplx_t<T>* __rest
     C gup[9], u[9], v[9], o[9];
     rotation_from_packed<T>(w, V, lex_up(g, s, lex, mu), gup);
     load_link<NELEM, true>(fwd + mu * NELEM * 32, u);
-    mul_left<NELEM / 3>(gx, u, v);
-    mul_right_adj<NELEM / 3>(v, gup, o);
+    mul_left<LinkRows<NELEM>::value>(gx, u, v);
+    mul_right_adj<LinkRows<NELEM>::value>(v, gup, o);
     store_link<NELEM>(fwd + mu * NELEM * 32, o);
   }
 }

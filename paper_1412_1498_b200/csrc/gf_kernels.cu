@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(256) reorder_kernel(cplx_t<T>* __restrict__ in
   if (IN) {
     const cplx_t<T>* cc = reinterpret_cast<const cplx_t<T>*>(c);
 #pragma unroll
-    for (int e = 0; e < NELEM; ++e) u[e] = cc[e];
+    for (int e = 0; e < (NELEM == 4 ? 9 : NELEM); ++e) u[e] = cc[e];  // the 8-real form needs a1 and c1 too
     store_link<NELEM>(p, u);
   } else {
     load_link<NELEM, true>(p, u);
@@ -63,6 +63,7 @@ static cudaError_t reorder_T(const KernelArgs& a, bool in, void* canon, long lon
 
 cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long lex_begin, long long lex_end,
                            const void* chunk_base) {
+  if (a.storage == 8) return reorder_T<double, 4>(a, in, canon, lex_begin, lex_end, chunk_base);  // FP64 only
   if (a.prec == 0) return a.storage == 18 ? reorder_T<double, 9>(a, in, canon, lex_begin, lex_end, chunk_base)
                                           : reorder_T<double, 6>(a, in, canon, lex_begin, lex_end, chunk_base);
   return a.storage == 18 ? reorder_T<float, 9>(a, in, canon, lex_begin, lex_end, chunk_base)
@@ -228,10 +229,10 @@ ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) 
   for (int mu = 0; mu < 4; ++mu) {
     C u[9], w[9];
     load_link<NELEM, true>(fwd + mu * NELEM * 32, u);
-    mul_left<NELEM / 3>(G, u, w);                       // U_mu(x) <- G U_mu(x)
+    mul_left<LinkRows<NELEM>::value>(G, u, w);                       // U_mu(x) <- G U_mu(x)
     store_link<NELEM>(fwd + mu * NELEM * 32, w);
     load_link<NELEM, false>(bwd[mu], u);
-    mul_right_adj<NELEM / 3>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+    mul_right_adj<LinkRows<NELEM>::value>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
     store_link<NELEM>(bwd[mu], w);
   }
 }
@@ -256,9 +257,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // shared slot of (link l, element e) of this thread: [l][e][THREADS] complex numbers, lane-contiguous (no bank conflicts)
 template <int NELEM, int THREADS, bool FULL, class C>
 __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
-#pragma unroll
-  for (int e = 0; e < NELEM; ++e) u[e] = sm[(l * NELEM + e) * THREADS];
-  if (NELEM == 6 && FULL) rebuild_row2(u);
+  load_link<NELEM, FULL, THREADS>(sm + l * NELEM * THREADS, u);
 }
 
 // MEASURE: the launch also leaves, per block, the sum over its sites of sum_ij |Delta_ij(x)|^2 AFTER the update, taken
@@ -343,7 +342,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     for (int mu = 0; mu < NMU; ++mu) {
       C u[9], w[9];
       load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
-      mul_left<NELEM / 3>(G, u, w);                       // U_mu(x) <- G U_mu(x)
+      mul_left<LinkRows<NELEM>::value>(G, u, w);                       // U_mu(x) <- G U_mu(x)
       store_link<NELEM>(fwd + mu * NELEM * 32, w);
       if (SLAB && mu == 3 && sv.top_out && cb >= g.vh - g.s3) {  // top slice: the copy that goes to the upper neighbour
         SlabView out = sv;
@@ -352,7 +351,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       }
       sched_fence();
       load_link_smem<NELEM, THREADS, false>(sm, 2 * mu + 1, u);
-      mul_right_adj<NELEM / 3>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+      mul_right_adj<LinkRows<NELEM>::value>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
       store_link<NELEM>(bwd[mu], w);
       if (SLAB && mu == 3 && sv.ret_out && cb < g.s3) {   // bottom slice: the copy that goes back to the lower neighbour
         SlabView out = sv;
@@ -364,7 +363,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     if (DEFER) {                                          // A(x) <- G A(x)
       C u[9], w[9];
       load_link_smem<NELEM, THREADS, true>(sm, 6, u);
-      mul_left<NELEM / 3>(G, u, w);
+      mul_left<LinkRows<NELEM>::value>(G, u, w);
       store_link<NELEM>(accp, w);
     }
   }
@@ -478,6 +477,9 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
   } while (0)
 
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
+  if (a.storage == 8)  // FP64 only (gf_create)
+    return a.gauge == 1 ? halfsweep_T<double, 4, 3>(a, parity, omega, fuse_theta, qblocks)
+                        : halfsweep_T<double, 4, 4>(a, parity, omega, fuse_theta, qblocks);
   GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
 }
 
@@ -548,9 +550,9 @@ __global__ void __launch_bounds__(256) defer_flush_kernel(cplx_t<T>* __restrict_
   C A[9], u[9], w[9];
   load_link<NELEM, true>(acc + (((size_t)parity * g.nblk + (size_t)(cb >> 5)) * NELEM) * 32 + (cb & 31), A);
   load_link<NELEM, true>(ut, u);
-  mul_left<NELEM / 3>(A, u, w);
+  mul_left<LinkRows<NELEM>::value>(A, u, w);
   load_link<NELEM, true>(acc + (((size_t)(parity ^ 1) * g.nblk + (size_t)(cb_up >> 5)) * NELEM) * 32 + (cb_up & 31), A);
-  mul_right_adj<NELEM / 3>(w, A, u);
+  mul_right_adj<LinkRows<NELEM>::value>(w, A, u);
   store_link<NELEM>(ut, u);
 }
 
@@ -753,7 +755,10 @@ static cudaError_t measure_T(const KernelArgs& a, int nq) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_measure(const KernelArgs& a, int nq) { GF_DISPATCH(measure_T, a, nq); }
+cudaError_t launch_measure(const KernelArgs& a, int nq) {
+  if (a.storage == 8) return a.gauge == 1 ? measure_T<double, 4, 3>(a, nq) : measure_T<double, 4, 4>(a, nq);
+  GF_DISPATCH(measure_T, a, nq);
+}
 
 // ---- per-time-slice F_t, theta_t (Coulomb gauge, gf_measure_slices / gf_fix_slices; reading A22) -------------------------
 // Block (chunk, 2 t + parity): 256 consecutive checkerboard sites of one parity of slice t.  In Coulomb gauge the even
@@ -817,6 +822,7 @@ __global__ void __launch_bounds__(256) reunit_kernel(cplx_t<T>* __restrict__ lin
   if (tile >= ntiles) return;
   C* p = links + (size_t)tile * NELEM * 32 + (tid & 31);
   C u[9];
+  if (NELEM == 4 && p[0].x == T(0) && p[0].y == T(0) && p[32].x == T(0) && p[32].y == T(0)) return;  // padding lane
   load_link<NELEM, false>(p, u);
   // padding lanes of the last block hold zeros: leave them alone (0/0)
   if (u[0].x == T(0) && u[0].y == T(0) && u[1].x == T(0) && u[1].y == T(0) && u[2].x == T(0) && u[2].y == T(0)) return;
@@ -833,6 +839,7 @@ static cudaError_t reunit_T(const KernelArgs& a) {
 }
 
 cudaError_t launch_reunit(const KernelArgs& a) {
+  if (a.storage == 8) return reunit_T<double, 4>(a);
   if (a.prec == 0) return a.storage == 18 ? reunit_T<double, 9>(a) : reunit_T<double, 6>(a);
   return a.storage == 18 ? reunit_T<float, 9>(a) : reunit_T<float, 6>(a);
 }

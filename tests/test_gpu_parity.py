@@ -490,3 +490,57 @@ def test_deferred_links_whole_run_with_reunitarisation_and_errors(gf, torch):
     assert gf.gf_defer_attach(fx.ctx, 0, 0) == gf.GF_OK and gf.gf_defer_flush(fx.ctx) == gf.GF_OK
     assert gf.gf_defer_flush(None) == gf.GF_EINVAL
     fx.close()
+
+
+# ---- 8-real storage (reading A23): FP64 only; tolerance scaled by the conditioning 1/N of the reconstruction --------------
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4), (2, 2, 2, 2)])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_8_real_storage_against_oracle(gf, torch, dims, gauge):
+    omega = 1.7
+    U = gi.make_links(dims, 0.5, 84)
+    Uo = U.copy()
+    oracle.project8(Uo, dims)
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec="f64", storage=8)
+    fx.set_links(torch.from_numpy(U).cuda())
+    back = fx.get_links().cpu().numpy()
+    F0, th0 = fx.measure()
+    Fo0, tho0 = oracle.measure(Uo, dims, gauge)
+    Uc = U[..., 0] + 1j * U[..., 1]
+    Nmin = (np.abs(Uc[:, :, 0, 1]) ** 2 + np.abs(Uc[:, :, 0, 2]) ** 2).min()
+    assert np.abs(back - Uo).max() <= 1e-14 / Nmin             # storing and reading back = the oracle's round trip
+    assert abs(F0 - Fo0) <= 1e-12 and abs(th0 / tho0 - 1) <= 1e-10
+    fx.ovr_sweep(1, omega)
+    got = fx.get_links().cpu().numpy()
+    F, th = fx.measure()
+    fx.reunitarize()
+    after = fx.get_links().cpu().numpy()
+    fx.close()
+    oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=8)
+    Fo, tho = oracle.measure(Uo, dims, gauge)
+    assert np.abs(got - Uo).max() <= max(1e-12, 1e-13 / Nmin)  # the one-sweep bound, widened where 1/N demands it
+    assert abs(F - Fo) <= 1e-10 * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
+    assert np.abs(after - got).max() <= 1e-12 / Nmin           # the links were unitary: reunitarisation changes nothing
+    assert sum(fx_bytes for fx_bytes in [gf.gf_workspace_bytes(*dims, gf.GF_FP64, 8)]) < gf.gf_workspace_bytes(*dims, gf.GF_FP64, 12)
+
+
+def test_8_real_storage_fix_and_unsupported_calls(gf, torch):
+    dims = (8, 8, 8, 8)
+    U = gi.make_links(dims, 0.3, 85)
+    Uo = U.copy()
+    oracle.project8(Uo, dims)
+    fx = gf.GaugeFixer(dims, gauge="landau", prec="f64", storage=8)
+    fx.set_links(torch.from_numpy(U).cuda())
+    done = fx.fix(1.7, 1e-10, 600, 10)
+    hist = fx.history()
+    do, histo = oracle.fix(Uo, dims, "landau", 1.7, 1e-10, 600, 10, storage=8)
+    assert abs(done - do) <= max(10, 0.02 * do) and done < 600
+    assert abs(hist[-1][1] - histo[-1][1]) <= 1e-10 * abs(histo[-1][1])
+    assert gf.gf_fft_workspace_bytes(fx.ctx)[0] == gf.GF_EUNSUPPORTED
+    assert gf.gf_set_option(fx.ctx, gf.GF_OPT_OVR_SERIES, 2) == gf.GF_EUNSUPPORTED
+    B = gf.gf_slab_halo_bytes(fx.ctx)
+    halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
+    assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
+    fx.close()
+    assert gf.gf_workspace_bytes(8, 8, 8, 8, gf.GF_FP32, 8) == 0
+    with pytest.raises(gf.GFError):
+        gf.GaugeFixer(dims, gauge="landau", prec="f32", storage=8)

@@ -596,3 +596,44 @@ def test_fix_slices_stops_each_slice_on_its_own_theta():
     # max_t theta_t < eps implies mean_t theta_t < eps: the global-test driver never runs longer
     dg, hg = oracle.fix(Ug, dims, "coulomb", 1.6, eps, 2000, 5)
     assert dg <= done and per.sum() < done * 6
+
+
+# ---- 8-real storage (reading A23; "Elems = 4") -------------------------------------------------------------
+def test_8_real_round_trip_reproduces_su3_links():
+    """The 8 stored reals determine an SU(3) matrix: the round trip is the identity up to rounding / N, the result is
+    unitary with det 1, and the formulas agree with an independent numpy reconstruction."""
+    dims = (4, 4, 4, 4)
+    U = gi.make_links(dims, 0.5, 81)
+    V = U.copy()
+    oracle.project8(V, dims)
+    Uc = to_c(U)
+    N = (np.abs(Uc[:, :, 0, 1]) ** 2 + np.abs(Uc[:, :, 0, 2]) ** 2)
+    assert (np.abs(to_c(V) - Uc).max(axis=(2, 3)) * N).max() < 1e-14   # error x N stays at rounding level
+    a, b = oracle.unitarity(V, dims)
+    assert a < 1e-13 and b < 1e-13
+    # independent reconstruction: complete (a, b1) to an SU(3) matrix by solving the linear conditions with numpy
+    rng = np.random.default_rng(82)
+    for idx in rng.integers(0, Uc.shape[0], size=20):
+        u = Uc[idx, 1]
+        a1 = np.sqrt(1 - N[idx, 1]) * np.exp(1j * np.angle(u[0, 0]))
+        arow = np.array([a1, u[0, 1], u[0, 2]])
+        c1 = np.sqrt(N[idx, 1] - abs(u[1, 0]) ** 2) * np.exp(1j * np.angle(u[2, 0]))
+        # unknowns b2, b3: conj(a).b = 0 and conj(a2 b3 - a3 b2) = c1
+        A = np.array([[np.conj(arow[1]), np.conj(arow[2])], [-arow[2], arow[1]]])
+        rhs = np.array([-np.conj(arow[0]) * u[1, 0], np.conj(c1)])
+        b2, b3 = np.linalg.solve(A, rhs)
+        brow = np.array([u[1, 0], b2, b3])
+        crow = np.conj(np.cross(arow, brow))
+        assert np.abs(np.array([arow, brow, crow]) - to_c(V)[idx, 1]).max() < 1e-13
+
+
+def test_8_real_sweep_stays_close_to_full_storage_and_gauge_invariant():
+    dims = (4, 4, 4, 4)
+    U0 = gi.make_links(dims, 0.5, 83)
+    oracle.project8(U0, dims)
+    U8, U18 = U0.copy(), U0.copy()
+    oracle.sweeps(U8, dims, "landau", 1.7, n=2, storage=8)
+    oracle.sweeps(U18, dims, "landau", 1.7, n=2)
+    assert np.abs(U8 - U18).max() < 1e-11
+    for mu, nu in [(0, 1), (1, 3)]:
+        assert np.abs(oracle.wilson_traces(U8, dims, mu, nu, 1, 1) - oracle.wilson_traces(U0, dims, mu, nu, 1, 1)).max() < 1e-11
