@@ -142,3 +142,60 @@ def test_fullsize_one_sweep_every_link(name):
     oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
     Uo -= got
     assert np.abs(Uo).max() <= TOL_LINK[prec]
+
+
+# ---- the sharded path and the hand-written transforms at full size -----------------------------------------------------
+# The single-context sweep at these sizes is checked against the oracle above; the two paths below are compared with it
+# (sharded: bit for bit) and with the library's cuFFT path (transforms), on the same device-generated fields.
+@pytest.mark.parametrize("name,n_slabs", [("cfg2", 2), ("cfg2", 4), ("cfg3", 3)])
+def test_full_size_sharded_sweep_is_bit_identical_to_the_single_context(name, n_slabs):
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    cfg = next(c for c in gi.CONFIGS if c["name"] == name)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage)
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], prec,
+                         torch.cuda.current_stream().cuda_stream)
+    fx.set_links(canon)
+    fx.ovr_sweep(2, cfg["omega"])
+    single = fx.get_links()
+    Fs, ths = fx.measure()
+    fx.close()
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, group=False)
+    sh.set_links_global(canon)
+    sh.ovr_sweep(2, cfg["omega"])
+    links = sh.get_links()
+    F, th = sh.measure()
+    V = sh.local_volume
+    for s in range(n_slabs):
+        assert torch.equal(links[s].reshape(-1), single[s * V:(s + 1) * V].reshape(-1)), f"slab {s}"
+    sh.close()
+    assert abs(F - Fs) <= 1e-6 * abs(Fs) and abs(th - ths) <= 1e-5 * ths
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg1"])
+def test_full_size_hand_written_transforms_against_the_cufft_path(name):
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    cfg = next(c for c in gi.CONFIGS if c["name"] == name)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    res = {}
+    for own in (1, 0):
+        fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage)
+        fx.set_option(gf.GF_OPT_FFT_OWN, own)
+        canon = fx.new_links_buffer()
+        gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], prec,
+                             torch.cuda.current_stream().cuda_stream)
+        fx.set_links(canon)
+        fx.fft_step(2, 0.08)
+        res[own] = (fx.get_links(), fx.measure())
+        fx.close()
+        del canon
+    diff = float((res[1][0] - res[0][0]).abs().max())
+    assert diff <= (1e-12 if prec == "f64" else 2e-5), diff
+    assert abs(res[1][1][0] - res[0][1][0]) <= (1e-12 if prec == "f64" else 1e-6)
