@@ -36,7 +36,7 @@ if ROOT not in sys.path:
 
 METRIC = "ovr_site_updates_per_s"
 UNIT = "site-updates/s"
-LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48}
+LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48, ("f64", 8): 64}
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the committed ncu --set full capture
 # (profiles/): filled per config once a capture exists, else null.
 NCU_TRAFFIC_BYTES = {"cfg4": 19.327848e9 + 19.269022e9,  # profiles/r1f_halfsweep_cfg4_ncu.txt
@@ -234,6 +234,12 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     cfg = get_cfg(args.config)
+    # kernel studies on a config's lattice (secondary lines, named in config.workload): another storage format, Coulomb
+    # gauge, deferred temporal links
+    if args.storage:
+        cfg["storage"] = args.storage
+    if args.gauge:
+        cfg["gauge"] = args.gauge
     dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
     V = gi.volume(dims)
     L = LINK_BYTES[(prec, storage)]
@@ -241,6 +247,8 @@ def run_ours(args):
     omega = cfg["omega"]
 
     fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
+    if args.defer:
+        fx.defer_temporal_links()
     if args.variant:
         fx.set_option(gf.GF_OPT_SWEEP_VARIANT, args.variant)
     if args.block:
@@ -293,7 +301,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (half-sweep): 2*n_sw launches per step, back to back on the stream
     peak, peak_src = load_peaks()
     n_half = 2 * n_sw * args.steps
-    bytes_per_launch = 16 * L * (V // 2)
+    bytes_per_launch = (14 if args.defer else 16) * L * (V // 2)  # deferred: 6 links + the accumulator, read and written
     # the reunitarisation launches inside the sweep region (config 2 only) are subtracted at their algorithmic cost
     ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
     achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
@@ -428,7 +436,9 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": prec, "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "step": f"{n_sw} sweeps + 1 F/theta measurement",
+        "config": {"workload": workload_name(cfg) + (" (deferred temporal links)" if args.defer else "")
+                   + (" [study: not the config's own storage / gauge]" if args.storage or args.gauge else ""),
+                   "step": f"{n_sw} sweeps + 1 F/theta measurement",
                    "sites": V, "l2": "inputs exceed L2 (field %.2f GB vs 126 MB)" % (4 * V * L / 1e9)
                    if 4 * V * L > 4 * 126e6 else "field fits L2: not an HBM measurement", "parallelism": "replicas only",
                    "final_F": F, "final_theta": th},
@@ -621,6 +631,9 @@ def main():
     ap.add_argument("--algo", default="ovr", choices=["ovr", "fftsd"], help="ovr = Algorithm 1 (headline); fftsd = Algorithm 2")
     ap.add_argument("--sharded", type=int, default=0, metavar="K",
                     help="T-slab sharded sweep with K slabs per rank (secondary line; default 0 = single context / replicas)")
+    ap.add_argument("--storage", type=int, default=0, help="kernel study: 18, 12 or 8 (FP64) instead of the config's storage")
+    ap.add_argument("--gauge", default="", choices=["", "landau", "coulomb"], help="kernel study: another gauge on the config's lattice")
+    ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
     args = ap.parse_args()
     if args.impl == "reference":
