@@ -439,7 +439,10 @@ template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
   using C = cplx_t<T>;
   *qblocks = 0;
-  if (a.variant == 0 || a.variant == 3) {
+  // 8-real storage: the default is the two-pass kernel (no staging area, so occupancy is set by registers alone, which
+  // the dependent chains of the link reconstruction need: 7.6 ms against 10.8 ms staged on the cfg4 lattice)
+  const int variant = (a.variant == 0 && NELEM == 4) ? 1 : a.variant;
+  if (variant == 0 || variant == 3) {
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
     constexpr int THREADS = staged_threads<T>();
     if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
@@ -454,10 +457,10 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
   if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
   if (a.series > 0) return cudaErrorNotSupported;  // the series is built into the staged kernel only
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
-  if (a.variant == 2)
+  if (variant == 2)
     ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1, true><<<blocks, THREADS, 0, a.stream>>>((C*)a.links, a.geo, parity,
                                                                                           (T)omega);
-  else if (a.variant == 1)
+  else if (variant == 1)
     ovr_halfsweep_kernel<T, NELEM, ND, THREADS, 1, false><<<blocks, THREADS, 0, a.stream>>>((C*)a.links, a.geo, parity,
                                                                                            (T)omega);
   else
@@ -620,7 +623,9 @@ cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pac
   return a.storage == 18 ? slab_top_T<float, 9>(a, parity, buf, pack) : slab_top_T<float, 6>(a, parity, buf, pack);
 }
 
-bool halfsweep_can_fuse_theta(const KernelArgs& a) { return (a.variant == 0 || a.variant == 3) && a.series == 0; }
+bool halfsweep_can_fuse_theta(const KernelArgs& a) {
+  return (a.variant == 3 || (a.variant == 0 && a.storage != 8)) && a.series == 0;
+}
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
 // ======================================================================================================================
