@@ -24,7 +24,8 @@ Readings (B1-B6; A-numbers are those of Algorithm 1 and carry ove
 
 Parity unpinned: whole-trajectory values (iteration counts, final F) — the paper prints none.  Everything else is
 pinned in tests/test_fftsd_oracle_pins.py (p^2 against the lattice Laplacian, dF/dalpha against the closed form
-theta/(4d) and its momentum-space generalisation, gauge invariance, unitarity, convergence to F = 1 on a pure gauge).
+theta/(4d) and its momentum-space generalisation, gauge invariance, unitarity, convergence to F = 1 on a pure gauge);
+fix()'s iteration / reunitarisation order in tests/test_oracle_order_pins.py (against step + reunitarize_links unrolled).
 """
 from __future__ import annotations
 

@@ -17,7 +17,12 @@
 // binomial series of 2x2 numpy matrices, its terminating (omega = 1, 2) and order-1 closed forms, convergence to the
 // exact power, gauge invariance of a series sweep; per-slice F_t / theta_t against the global values and against the
 // slice copied into a two-slice lattice, masked half-sweeps (finished slices untouched, active ones as in the full
-// sweep), per-slice sweep counts against each slice run alone.  The whole trajectory on the five configs (sweep counts, final F) is "parity unpinned"
+// sweep), per-slice sweep counts against each slice run alone.  The drivers' ORDER (tests/test_oracle_order_pins.py):
+// sweeps() = even half-sweep then odd half-sweep against the two calls written out, against a numpy
+// gauge transformation by G on the (x+y+z+t)-even sites first, and by stationarity of the parity visited last;
+// reunitarisation after global sweep s iff s % k == 0 against the unrolled call sequence and the
+// unitarity defect of an off-group input; fix() / fix_slices() histories and links against the same sequences.
+// The whole trajectory on the five configs (sweep counts, final F) is "parity unpinned"
 // by the paper, which prints no numbers (last row of the pin table).
 //
 // Canonical layout: links[site][mu][row][col][re,im], site = x + nx*(y + ny*(z + nz*t)) (x fastest),
