@@ -36,14 +36,22 @@ def run_gpu(cfg, dims=None):
     return done, hist, links, U
 
 
-def compare_histories(hist, gold, tolF, converged, floor=1e-9):
-    """hist, gold: [(sweep, F, theta)].  F at every common checkpoint, theta within x1.5 wherever it is above the
-    rounding floor, and the final values."""
+# Below which theta the x1.5 comparison is no longer meaningful: theta is a sum of |Delta_ij|^2, and an
+# evaluated Delta entry (a sum of 2d link entries of size O(1)) carries an absolute rounding error e ~ sqrt(2d) u,
+# u = 1.1e-16 (FP64) or 6e-8 (FP32 storage), so the evaluated theta differs from the exact one by a relative
+# 2 e / sqrt(theta / 3) + O(e^2 / theta).  Requiring that to stay below 0.2 (well inside the 1.5 window) gives
+# theta >= 300 e^2: 3e-29 in FP64 and 9e-12 in FP32.  Every checkpoint of every config lies above these floors
+# (cfg0 stops at 1e-12, cfg2 at 1e-7), so the bound is checked through the LAST checkpoint of every run.
+THETA_FLOOR = {"f64": 1e-28, "f32": 1e-11}
+
+
+def compare_histories(hist, gold, tolF, prec="f64"):
+    """hist, gold: [(sweep, F, theta)].  F and theta (within x1.5) at every common checkpoint."""
     n = min(len(hist), len(gold))
     for (s, F, th), (so, Fo, tho) in zip(hist[:n], gold[:n]):
         assert s == so
         assert abs(F - Fo) <= tolF * abs(Fo), (s, F, Fo)
-        if tho > floor or not converged:
+        if tho > THETA_FLOOR[prec]:
             assert tho / 1.5 <= th <= tho * 1.5, (s, th, tho)
 
 
@@ -63,7 +71,7 @@ def test_fix_matches_stored_oracle_trajectory(name):
     del U
     converged = ghist[-1][2] < cfg["eps"]
     assert abs(done - gold["sweeps_done"]) <= 0.02 * gold["sweeps_done"]
-    compare_histories(hist, ghist, tolF, converged, 1e-9 if f64 else 1e-6)
+    compare_histories(hist, ghist, tolF, cfg["prec"])
     Ff, thf = hist[-1][1], hist[-1][2]
     assert abs(Ff - ghist[-1][1]) <= tolF * abs(ghist[-1][1])
     if converged:
@@ -91,7 +99,6 @@ def test_fix_small_lattice_live_oracle(name, dims):
                               cfg["reunit_every"], cfg["storage"])
     tolF = 1e-10 if cfg["prec"] == "f64" else 1e-5
     assert abs(done - odone) <= max(0.02 * odone, 0)
-    converged = ohist[-1][2] < cfg["eps"]
-    compare_histories(hist, [tuple(h) for h in ohist], tolF, converged)
+    compare_histories(hist, [tuple(h) for h in ohist], tolF, cfg["prec"])
     if cfg["prec"] == "f64":
         assert np.abs(links - Uo).max() <= 1e-8  # hundreds of sweeps: rounding grows in the early, random phase only
