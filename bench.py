@@ -37,16 +37,28 @@ if ROOT not in sys.path:
 METRIC = "ovr_site_updates_per_s"
 UNIT = "site-updates/s"
 LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48, ("f64", 8): 64}
-# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the committed ncu --set full capture
-# (profiles/): filled per config once a capture exists, else null.
-NCU_TRAFFIC_BYTES = {"cfg4": 19.327848e9 + 19.269022e9,  # profiles/r1f_halfsweep_cfg4_ncu.txt
-                     "cfg3": 4.076932e9 + 4.017487e9,    # profiles/r1c_halfsweep_cfg3_ncu.txt
-                     "cfg2": 201.386e6 + 142.245e6}      # profiles/r1f_halfsweep_cfg2_ncu.txt (partly L2-resident)
+# nominal flop per site-update (add = mul = 1, FMA = 2; reconstruct + K + 3 subgroup steps + 8
+# products), split into the part the kernels run in FP64 in BOTH storage precisions (K(x) and the three SU(2) steps,
+# DESIGN.md §2 "Precision of the site rotation") and the part that runs in the storage precision.
+FLOPS_ROTATION = 144 + 597                       # K(x) + 3 subgroup steps: always FP64
+FLOPS_LINKS = {18: 1584, 12: 336 + 1056, 8: 1584 + 8 * 90}  # the 8 products (+ row-2 / 8-real reconstruction)
 
 
-# the same for one Algorithm 2 iteration: sd_delta (profiles/r1e_sd_delta_cfg4_ncu.txt) + the five transform passes
-# (profiles/r1h_fft_passes_cfg4_ncu.txt) + sd_rotate (profiles/r1d_fftsd_cfg4_ncu.txt)
-NCU_TRAFFIC_BYTES_FFTSD = {"cfg4": (20.97e9 + 2.14e9) + 5 * (2.1476e9 + 2.0886e9) + (24.746e9 + 19.273e9)}
+def ncu_traffic(cfg_name, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `cfg_name`, from the committed
+    `ncu --set full` captures (profiles/ncu_traffic.csv names the summary each row was read from); None if absent."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None, None
+    import csv
+
+    best = None
+    for row in csv.DictReader(l for l in open(path) if not l.startswith("#")):
+        if row["config"] == cfg_name and row["kernel"] == kernel:
+            best = row  # the last matching row is the newest capture
+    if best is None:
+        return None, None
+    return float(best["dram_read_bytes"]) + float(best["dram_write_bytes"]), best["source"]
 
 
 def log(*a):
@@ -59,6 +71,61 @@ def load_peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, read+write copy)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def halfsweep_kernel_name(storage, variant, defer=False):
+    """The kernel gf_ovr_sweep launches for this storage format / GF_OPT_SWEEP_VARIANT (csrc/gf_kernels.cu, halfsweep_T)."""
+    v = variant or (1 if storage == 8 else 3)
+    return {1: "ovr_halfsweep_kernel", 2: "ovr_halfsweep_kernel (L2 bulk prefetch)", 3: "ovr_halfsweep_staged_kernel",
+            4: "ovr_halfsweep_bulk_kernel"}[v] + (" (deferred temporal links)" if defer else "")
+
+
+def measure_fp_peaks(seconds=0.25):
+    """FP64 / FP32 FMA-chain peaks of the current device, measured now through the C ABI (gf_peak_fma)."""
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    scratch = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    out = {}
+    for name, prec in (("f64_tflops", gf.GF_FP64), ("f32_tflops", gf.GF_FP32)):
+        rc, t = gf.gf_peak_fma(prec, seconds, scratch.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        if rc != gf.GF_OK:
+            raise RuntimeError(f"gf_peak_fma failed: {gf.gf_strerror(rc)}")
+        out[name] = t
+    out["how"] = "gf_peak_fma: register-only FMA chains (16 per thread, 8 blocks of 256 threads per SM), FMA = 2 flop"
+    return out
+
+
+def run_peaks(args):
+    """--peaks: the measured CUDA-core peaks with the clocks seen while they ran."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    measure_fp_peaks(0.05)
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    fp = measure_fp_peaks(2.0)
+    clocks = sampler.stop()
+    hbm, src = load_peaks()
+    print(json.dumps({"metric": "fma_chain_peak", "f64_tflops": fp["f64_tflops"], "f32_tflops": fp["f32_tflops"],
+                      "how": fp["how"], "hbm_gbs": hbm, "hbm_source": src, "clocks": clocks,
+                      "nominal": "148 SMs x 64 (FP64) / 128 (FP32) FMA lanes x 2 flop x 1.965 GHz = 37.2 / 74.5 TFLOP/s"}),
+          flush=True)
+    return 0
+
+
+def spawn_command(gpus, argv, port=None):
+    """`python bench.py --gpus N` without a launcher: the command that runs N ranks of this file, one per GPU."""
+    import socket
+
+    if port is None:
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr",
+            "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
 
 
 def get_cfg(name):
@@ -150,7 +217,8 @@ class OracleRun:
             oracle.project12(self.U, self.dims)
         self.cores = oracle.num_threads()
         self.sweeps_done = 0
-        self.sample = (f"oracle (g++ -O2, {self.cores} OpenMP threads), {self.dims[0]}x{self.dims[1]}x{self.dims[2]}x"
+        self.sample = (f"oracle as it stands: an unoptimised checker (g++ -O2 -ffp-contract=off, {self.cores} OpenMP "
+                       f"threads), {self.dims[0]}x{self.dims[1]}x{self.dims[2]}x"
                        f"{self.dims[3]} slab of the workload lattice, same generator / gauge / storage / omega; "
                        f"one step = {cfg['check_every']} sweeps + 1 F/theta measurement (the GPU arm's cadence)")
 
@@ -176,6 +244,9 @@ def run_reference(args):
     """--impl reference: the oracle timed on the host cores with the arm's metric/config.  Rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return 0
+    if "WORLD_SIZE" in os.environ and os.environ.get("OMP_NUM_THREADS") == "1":
+        # torchrun's default for its ranks; rank 0 is the only one that works here, so it takes the host's cores
+        os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
     cfg = get_cfg(args.config)
     run = OracleRun(cfg)
     value, dt = run.time_steps(args.steps, args.warmup)
@@ -305,9 +376,27 @@ def run_ours(args):
     # the reunitarisation launches inside the sweep region (config 2 only) are subtracted at their algorithmic cost
     ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
     achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "ovr_halfsweep_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg["name"]), "peak_source": peak_src,
+    kernel = halfsweep_kernel_name(storage, args.variant, args.defer)
+    traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer) else (None, None)
+    # flops leg: the FMA-chain peaks measured now, on this GPU, under the clocks it runs at after
+    # the timed region (gf_peak_fma); the site rotation is FP64 in both storage precisions, the link products are in
+    # the storage precision
+    fp = measure_fp_peaks(0.25)
+    flops64 = FLOPS_ROTATION + (FLOPS_LINKS[storage] if prec == "f64" else 0)
+    flops32 = FLOPS_LINKS[storage] if prec == "f32" else 0
+    t_bytes_ms = bytes_per_launch / (peak * 1e9) * 1e3
+    t_flops_ms = (V // 2) * (flops64 / (fp["f64_tflops"] * 1e12) + flops32 / (fp["f32_tflops"] * 1e12)) * 1e3
+    roofline = {"bound": "hbm" if t_bytes_ms >= t_flops_ms else "alu", "kernel": kernel, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src,
+                "peak_note": "a read+write copy, the same 50/50 mix as this kernel; frac > 1 means the kernel moves its "
+                             "bytes faster than torch's copy does, not that it beats the memory system (read-only passes "
+                             "reach 7.3-7.4 TB/s on this part, HBM3e nominal is 7.7-8 TB/s)",
                 "algorithmic_bytes_per_launch": bytes_per_launch, "ms_per_launch": ms_half,
+                "roofline_ms_per_launch": max(t_bytes_ms, t_flops_ms), "bytes_leg_ms": t_bytes_ms, "flops_leg_ms": t_flops_ms,
+                "frac_of_roofline_time": max(t_bytes_ms, t_flops_ms) / ms_half,
+                "flops_per_site_update": {"fp64": flops64, "fp32": flops32, "source": "SURVEY.md 8(d), nominal counts"},
+                "fp_peaks": fp,
                 "launches_timed": n_half, "share_of_step": ms_sweeps / ms_total,
                 "measure_ms": ms_measure / args.steps,
                 "measure_gbs": 4 * V * L / (ms_measure / args.steps * 1e-3) / 1e9,
@@ -500,7 +589,7 @@ def run_fftsd(args):
                        "step": f"{n_it} iterations + 1 F/theta measurement", "final_F": F, "final_theta": th},
             "roofline": {"bound": "hbm", "kernel": "whole iteration (sd_delta, transform passes with the Fourier factor, sd_rotate)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                         "traffic": NCU_TRAFFIC_BYTES_FFTSD.get(cfg["name"]),
+                         "traffic": ncu_traffic(cfg["name"], "fftsd_iteration")[0],
                          "peak_source": peak_src, "algorithmic_bytes_per_iteration": bytes_it},
             "gpu_launches": int(fx.kernel_launches() - l0)}
     fx.close()
@@ -635,7 +724,13 @@ def main():
     ap.add_argument("--gauge", default="", choices=["", "landau", "coulomb"], help="kernel study: another gauge on the config's lattice")
     ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
+    ap.add_argument("--peaks", action="store_true", help="print the measured FP64 / FP32 FMA-chain peaks and exit")
     args = ap.parse_args()
+    if args.peaks:
+        return run_peaks(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started without a launcher: become N ranks, one per GPU (the driver's torchrun line does the same)
+        return subprocess.call(spawn_command(args.gpus, sys.argv[1:]))
     if args.impl == "reference":
         return run_reference(args)
     if args.sharded:

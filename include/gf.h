@@ -238,6 +238,13 @@ int gf_slab_halfsweep_interior(gf_ctx* ctx, int parity, double omega);
 /* Number of kernels this context has launched since gf_create (for benchmark bookkeeping). */
 long long gf_kernel_launches(const gf_ctx* ctx);
 
+/* Measurement aid, not a step of the method (the flops leg of the roofline needs a MEASURED FP64 / FP32
+ * CUDA-core peak): runs a register-only FMA-chain kernel (16 independent chains per thread, 2048 threads per SM asked
+ * for) on the current device for about seconds_target seconds (0 < seconds_target <= 10) and writes the achieved
+ * TFLOP/s (FMA = 2 flop) of precision prec (GF_FP64: DFMA, GF_FP32: FFMA) to *tflops (host).  dev_scratch: at least 8
+ * bytes of device memory (never written in practice).  Synchronises cuda_stream.  Errors: GF_EINVAL, GF_ECUDA. */
+int gf_peak_fma(int prec, double seconds_target, void* dev_scratch, void* cuda_stream, double* tflops);
+
 void gf_destroy(gf_ctx* ctx);
 const char* gf_strerror(int code);
 /* Text of the last failure on this context (CUDA error string for GF_ECUDA); valid until the next call. */

@@ -24,7 +24,7 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
            "gf_measure_slices", "gf_fix_slices", "gf_defer_bytes", "gf_defer_attach", "gf_defer_flush",
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
-           "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"]
+           "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma"]
 
 
 def _load() -> ctypes.CDLL:
@@ -80,6 +80,8 @@ def _load() -> ctypes.CDLL:
     for name in ("gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"):
         getattr(lib, name).restype = c_int
         getattr(lib, name).argtypes = [c_void_p, c_int, c_double]
+    lib.gf_peak_fma.restype = c_int
+    lib.gf_peak_fma.argtypes = [c_int, c_double, c_void_p, c_void_p, POINTER(c_double)]
     lib.gf_kernel_launches.restype = c_longlong
     lib.gf_kernel_launches.argtypes = [c_void_p]
     lib.gf_destroy.restype = None
@@ -247,6 +249,13 @@ def gf_slab_halfsweep_interior(ctx, parity: int, omega: float) -> int:
     return lib.gf_slab_halfsweep_interior(ctx, parity, omega)
 
 
+def gf_peak_fma(prec: int, seconds_target: float, dev_scratch: int, stream: int = 0):
+    """Returns (rc, TFLOP/s) of the FMA-chain micro-kernel on the current device."""
+    t = c_double()
+    rc = lib.gf_peak_fma(prec, seconds_target, c_void_p(dev_scratch), c_void_p(stream or None), byref(t))
+    return rc, t.value
+
+
 def gf_kernel_launches(ctx) -> int:
     return int(lib.gf_kernel_launches(ctx))
 
@@ -288,12 +297,20 @@ class GaugeFixer:
             nbytes = 256
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.workspace = self._alloc(nbytes)
             rc, self.ctx = gf_create(*self.dims, _GAUGE[gauge], _PREC[prec], self.storage, self.workspace.data_ptr(),
                                      nbytes, self.stream.cuda_stream)
         if rc != GF_OK:
             self.ctx = None
             raise GFError(rc)
+
+    def _alloc(self, nbytes):
+        """Device bytes the library will use on self.stream: allocated under that stream, so that the caching
+        allocator ties the block to it (a block freed later is not handed to another stream while kernels of this
+        one may still be running on it)."""
+        torch = self.torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
 
     def _check(self, rc):
         if rc != GF_OK:
@@ -341,8 +358,7 @@ class GaugeFixer:
         """Coulomb gauge: keep the sites' accumulated rotations instead of rewriting the temporal links every update."""
         if on:
             n = gf_defer_bytes(self.ctx)
-            with self.torch.cuda.device(self.device):
-                self.defer_buffer = self.torch.empty(max(n, 256), dtype=self.torch.uint8, device=self.device)
+            self.defer_buffer = self._alloc(n)
             self._check(gf_defer_attach(self.ctx, self.defer_buffer.data_ptr(), n))
         else:
             self._check(gf_defer_attach(self.ctx, 0, 0))
@@ -382,8 +398,7 @@ class GaugeFixer:
             return
         rc, nbytes = gf_fft_workspace_bytes(self.ctx)
         self._check(rc)
-        with self.torch.cuda.device(self.device):
-            self.fft_workspace = self.torch.empty(max(nbytes, 256), dtype=self.torch.uint8, device=self.device)
+        self.fft_workspace = self._alloc(nbytes)
         self._check(gf_fft_attach(self.ctx, self.fft_workspace.data_ptr(), nbytes))
 
     def fft_step(self, n, alpha):
@@ -401,10 +416,12 @@ class GaugeFixer:
 
     def close(self):
         if getattr(self, "ctx", None):
+            self.stream.synchronize()  # nothing of this context is in flight when its memory goes back to torch
             gf_destroy(self.ctx)
             self.ctx = None
             self.workspace = None
             self.fft_workspace = None
+            self.defer_buffer = None
 
     def __del__(self):
         try:

@@ -58,8 +58,11 @@ Sizes sizes_of(const Geo& g, int prec, int storage) {
 struct gf_ctx {
   KernelArgs k;
   Sizes sz;
+  int device;                 // the CUDA device that was current at gf_create: every entry point runs on it
   char* staging[2];
-  cudaEvent_t staging_free[2];
+  cudaStream_t copy_stream;   // host <-> staging copies of the *_host calls, beside the reorder kernels on k.stream
+  cudaEvent_t staging_free[2];  // staging[b] may be overwritten (its last reader has finished)
+  cudaEvent_t staging_full[2];  // staging[b] holds a chunk (its last writer has finished)
   double* host_result;  // pinned and mapped, 2 doubles: the reduction kernels write F, theta straight into it
   char* defer_acc;      // gf_defer_attach: the accumulated rotation A(x) of every site, or null
   bool defer_dirty;     // sweeps have run since the last flush
@@ -91,6 +94,22 @@ struct gf_ctx {
 };
 
 namespace {
+// Makes the context's device current for the duration of an entry point (a caller may drive contexts on several GPUs
+// from one thread) and puts the caller's device back afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(const gf_ctx* c) {
+    int cur = -1;
+    if (c && cudaGetDevice(&cur) == cudaSuccess && cur != c->device && cudaSetDevice(c->device) == cudaSuccess) prev = cur;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+#define GF_ENTER(c)              \
+  if (!(c)) return GF_EINVAL;    \
+  DeviceGuard gf_device_guard_(c)
+
 int fail_cuda(gf_ctx* c, cudaError_t e, const char* where) {
   snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e));
   return GF_ECUDA;
@@ -155,15 +174,20 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->host_result = nullptr;
   c->host_slices = c->dev_slices = nullptr;
   c->defer_acc = nullptr; c->defer_dirty = false;
-  c->staging_free[0] = c->staging_free[1] = nullptr;
-  cudaError_t e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
+  c->staging_free[0] = c->staging_free[1] = c->staging_full[0] = c->staging_full[1] = nullptr;
+  c->copy_stream = nullptr;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->host_result, 2 * sizeof(double), cudaHostAllocMapped);
   if (e == cudaSuccess) {  // zero-copy result: saves a 16-byte D2H copy per measurement (latency on small lattices)
     void* dev = nullptr;
     e = cudaHostGetDevicePointer(&dev, c->host_result, 0);
     if (e == cudaSuccess) c->k.result = dev;
   }
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[0], cudaEventDisableTiming);
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_free[1], cudaEventDisableTiming);
+  for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+    e = cudaEventCreateWithFlags(&c->staging_free[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->staging_full[i], cudaEventDisableTiming);
+  }
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
   // padding lanes of the last 32-site block must read as zeros
   if (e == cudaSuccess) e = cudaMemsetAsync(c->k.links, 0, sz.links, c->k.stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->k.counter, 0, sz.result, c->k.stream);
@@ -177,11 +201,17 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
 
 void gf_destroy(gf_ctx* c) {
   if (!c) return;
-  if (c->host_result) cudaFreeHost(c->host_result);
-  if (c->host_slices) cudaFreeHost(c->host_slices);
-  fft_plans_destroy(c->fft);
-  for (int i = 0; i < 2; ++i)
-    if (c->staging_free[i]) cudaEventDestroy(c->staging_free[i]);
+  {
+    DeviceGuard guard(c);
+    if (c->host_result) cudaFreeHost(c->host_result);
+    if (c->host_slices) cudaFreeHost(c->host_slices);
+    fft_plans_destroy(c->fft);
+    for (int i = 0; i < 2; ++i) {
+      if (c->staging_free[i]) cudaEventDestroy(c->staging_free[i]);
+      if (c->staging_full[i]) cudaEventDestroy(c->staging_full[i]);
+    }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  }
   delete c;
 }
 
@@ -201,7 +231,7 @@ static int defer_flush(gf_ctx* c) {
 size_t gf_defer_bytes(const gf_ctx* c) { return c ? defer_bytes(c) : 0; }
 
 int gf_defer_attach(gf_ctx* c, void* dev_acc, size_t bytes) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8)
     return fail(c, GF_EUNSUPPORTED, "gf_defer_attach: Coulomb gauge on a whole lattice only, 18- or 12-real storage");
   if (!dev_acc) {  // detach: bring the temporal links up to date first
@@ -221,12 +251,12 @@ int gf_defer_attach(gf_ctx* c, void* dev_acc, size_t bytes) {
 }
 
 int gf_defer_flush(gf_ctx* c) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   return defer_flush(c);
 }
 
 int gf_set_links(gf_ctx* c, const void* dev_links) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!dev_links) return fail(c, GF_EINVAL, "gf_set_links: null links");
   cudaError_t e = launch_reorder(c->k, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
   if (e == cudaSuccess && c->defer_acc && c->defer_dirty) e = launch_defer(c->k, c->defer_acc, false);  // A = 1
@@ -239,7 +269,7 @@ int gf_set_links(gf_ctx* c, const void* dev_links) {
 }
 
 int gf_get_links(gf_ctx* c, void* dev_links_out) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!dev_links_out) return fail(c, GF_EINVAL, "gf_get_links: null output");
   int rc = defer_flush(c);
   if (rc != GF_OK) return rc;
@@ -249,35 +279,49 @@ int gf_get_links(gf_ctx* c, void* dev_links_out) {
   return GF_OK;
 }
 
-// Host <-> device through the two staging buffers: chunk i uses buffer i&1; the copy of chunk i+1 overlaps the reorder
-// kernel of chunk i when the host memory is pinned.
+// Host <-> device through the two staging buffers: chunk i uses buffer i & 1.  The copies run on the context's own copy
+// stream, the reorder kernels on the context's stream, ordered by events per buffer, so that (with pinned host
+// memory) the copy of chunk i+1 runs beside the reorder kernel of chunk i.
 static int links_host(gf_ctx* c, void* host, bool in) {
   const size_t link_bytes = 18 * elem_size(c);
   const long long sites_per_chunk = (long long)(STAGING_BYTES / (4 * link_bytes));
   const long long V = volume(c);
-  cudaError_t e = cudaSuccess;
+  cudaStream_t main = c->k.stream, copy = c->copy_stream;
+  // everything enqueued on the context's stream so far (an earlier get/set, the sweeps) comes first
+  cudaError_t e = cudaEventRecord(c->staging_free[0], main);
+  if (e == cudaSuccess) e = cudaEventRecord(c->staging_free[1], main);
   int i = 0;
   for (long long s0 = 0; s0 < V && e == cudaSuccess; s0 += sites_per_chunk, ++i) {
     const long long s1 = s0 + sites_per_chunk < V ? s0 + sites_per_chunk : V;
     const size_t bytes = (size_t)(s1 - s0) * 4 * link_bytes;
     char* h = (char*)host + (size_t)s0 * 4 * link_bytes;
-    char* st = c->staging[i & 1];
+    const int b = i & 1;
+    char* st = c->staging[b];
     if (in) {
-      e = cudaMemcpyAsync(st, h, bytes, cudaMemcpyHostToDevice, c->k.stream);
+      e = cudaStreamWaitEvent(copy, c->staging_free[b], 0);  // the reorder kernel of chunk i-2 has read it
+      if (e == cudaSuccess) e = cudaMemcpyAsync(st, h, bytes, cudaMemcpyHostToDevice, copy);
+      if (e == cudaSuccess) e = cudaEventRecord(c->staging_full[b], copy);
+      if (e == cudaSuccess) e = cudaStreamWaitEvent(main, c->staging_full[b], 0);
       if (e == cudaSuccess) e = launch_reorder(c->k, true, nullptr, s0, s1, st);
+      if (e == cudaSuccess) e = cudaEventRecord(c->staging_free[b], main);
     } else {
-      e = launch_reorder(c->k, false, nullptr, s0, s1, st);
-      if (e == cudaSuccess) e = cudaMemcpyAsync(h, st, bytes, cudaMemcpyDeviceToHost, c->k.stream);
+      if (i >= 2) e = cudaStreamWaitEvent(main, c->staging_free[b], 0);  // the copy of chunk i-2 has left it
+      if (e == cudaSuccess) e = launch_reorder(c->k, false, nullptr, s0, s1, st);
+      if (e == cudaSuccess) e = cudaEventRecord(c->staging_full[b], main);
+      if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, c->staging_full[b], 0);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(h, st, bytes, cudaMemcpyDeviceToHost, copy);
+      if (e == cudaSuccess) e = cudaEventRecord(c->staging_free[b], copy);
     }
     c->launches += 1;
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(copy);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(main);
   if (e != cudaSuccess) return fail_cuda(c, e, in ? "gf_set_links_host" : "gf_get_links_host");
   return GF_OK;
 }
 
 int gf_set_links_host(gf_ctx* c, const void* host_links) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!host_links) return fail(c, GF_EINVAL, "gf_set_links_host: null links");
   if (c->defer_acc && c->defer_dirty) {
     cudaError_t e = launch_defer(c->k, c->defer_acc, false);  // A = 1
@@ -290,7 +334,7 @@ int gf_set_links_host(gf_ctx* c, const void* host_links) {
 }
 
 int gf_get_links_host(gf_ctx* c, void* host_links_out) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!host_links_out) return fail(c, GF_EINVAL, "gf_get_links_host: null output");
   int rc = defer_flush(c);
   if (rc != GF_OK) return rc;
@@ -298,7 +342,7 @@ int gf_get_links_host(gf_ctx* c, void* host_links_out) {
 }
 
 int gf_reunitarize(gf_ctx* c) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   int rc = defer_flush(c);  // every link is projected as it would stand after an in-place update
   if (rc != GF_OK) return rc;
   c->qblocks = 0;
@@ -309,14 +353,14 @@ int gf_reunitarize(gf_ctx* c) {
 }
 
 int gf_set_reunit_every(gf_ctx* c, int k) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (k < 0) return fail(c, GF_EINVAL, "gf_set_reunit_every: k < 0");
   c->reunit_every = k;
   return GF_OK;
 }
 
 int gf_set_option(gf_ctx* c, int key, int value) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   switch (key) {
     case GF_OPT_SWEEP_VARIANT:
       if (value < 0 || value > 3) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
@@ -352,7 +396,7 @@ int gf_set_option(gf_ctx* c, int key, int value) {
 }
 
 int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (n < 0) return fail(c, GF_EINVAL, "gf_ovr_sweep: n < 0");
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
   if (c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_ovr_sweep: the context is a slab, use gf_slab_halfsweep_*");
@@ -393,7 +437,7 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
 }
 
 int gf_measure(gf_ctx* c, double* F, double* theta) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!F || !theta) return fail(c, GF_EINVAL, "gf_measure: null out-param");
   cudaError_t e = launch_measure(c->k, c->qblocks);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
@@ -406,7 +450,7 @@ int gf_measure(gf_ctx* c, double* F, double* theta) {
 }
 
 int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!sweeps_done) return fail(c, GF_EINVAL, "gf_fix: null sweeps_done");
   if (check_every < 1 || max_sweeps < 0 || !(eps >= 0.0))
     return fail(c, GF_EINVAL, "gf_fix: need check_every >= 1, max_sweeps >= 0, eps >= 0");
@@ -451,7 +495,7 @@ static int slices_check(gf_ctx* c, const char* who) {
 }
 
 int gf_measure_slices(gf_ctx* c, double* F_t, double* theta_t) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!F_t || !theta_t) return fail(c, GF_EINVAL, "gf_measure_slices: null out-param");
   int rc = slices_check(c, "gf_measure_slices: Coulomb gauge on a whole lattice only");
   if (rc != GF_OK) return rc;
@@ -471,7 +515,7 @@ int gf_measure_slices(gf_ctx* c, double* F_t, double* theta_t) {
 
 int gf_fix_slices(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every, int* sweeps_done,
                   int* slice_sweeps) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!sweeps_done) return fail(c, GF_EINVAL, "gf_fix_slices: null sweeps_done");
   if (check_every < 1 || max_sweeps < 0 || !(eps >= 0.0))
     return fail(c, GF_EINVAL, "gf_fix_slices: need check_every >= 1, max_sweeps >= 0, eps >= 0");
@@ -538,7 +582,7 @@ int gf_fix_slices(gf_ctx* c, double omega, double eps, int max_sweeps, int check
 }
 
 int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!n || (cap > 0 && !hist) || cap < 0) return fail(c, GF_EINVAL, "gf_get_history: bad arguments");
   *n = (int)c->history_n;
   const long long m = c->history_n < cap ? c->history_n : cap;
@@ -564,7 +608,7 @@ static int fft_plan(gf_ctx* c) {
 }
 
 int gf_fft_workspace_bytes(gf_ctx* c, size_t* bytes) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!bytes) return fail(c, GF_EINVAL, "gf_fft_workspace_bytes: null out-param");
   int rc = fft_plan(c);
   if (rc != GF_OK) return rc;
@@ -573,7 +617,7 @@ int gf_fft_workspace_bytes(gf_ctx* c, size_t* bytes) {
 }
 
 int gf_fft_attach(gf_ctx* c, void* dev_workspace, size_t workspace_bytes) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!dev_workspace) return fail(c, GF_EINVAL, "gf_fft_attach: null workspace");
   int rc = fft_plan(c);
   if (rc != GF_OK) return rc;
@@ -648,7 +692,7 @@ static int fft_read_result(gf_ctx* c, double* F, double* theta) {
 }
 
 int gf_fft_step(gf_ctx* c, int n, double alpha) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (n < 0) return fail(c, GF_EINVAL, "gf_fft_step: n < 0");
   if (!(alpha > 0.0) || !std::isfinite(alpha)) return fail(c, GF_EINVAL, "gf_fft_step: alpha must be positive");
   if (!c->fft_w) return fail(c, GF_EINVAL, "gf_fft_step: no workspace attached (gf_fft_attach)");
@@ -661,7 +705,7 @@ int gf_fft_step(gf_ctx* c, int n, double alpha) {
 }
 
 int gf_fix_fft(gf_ctx* c, double alpha, double eps, int max_iters, int check_every, int* iters_done) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!iters_done) return fail(c, GF_EINVAL, "gf_fix_fft: null iters_done");
   if (check_every < 1 || max_iters < 0 || !(eps >= 0.0))
     return fail(c, GF_EINVAL, "gf_fix_fft: need check_every >= 1, max_iters >= 0, eps >= 0");
@@ -703,7 +747,7 @@ int gf_fix_fft(gf_ctx* c, double alpha, double eps, int max_iters, int check_eve
 size_t gf_slab_halo_bytes(const gf_ctx* c) { return c ? c->halo_bytes : 0; }
 
 int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!dev_halo) return fail(c, GF_EINVAL, "gf_slab_attach: null workspace");
   if (c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: not built for 8-real storage");
   if (bytes < 4 * c->halo_bytes || ((uintptr_t)dev_halo % ALIGN))
@@ -720,7 +764,7 @@ int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
 }
 
 int gf_slab_set_targets(gf_ctx* c, void* upper_ghost0, void* upper_ghost1, void* lower_top_in) {
-  if (!c) return GF_EINVAL;
+  GF_ENTER(c);
   if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_targets: no halo workspace attached (gf_slab_attach)");
   if ((upper_ghost0 == nullptr) != (upper_ghost1 == nullptr) || (upper_ghost0 == nullptr) != (lower_top_in == nullptr))
     return fail(c, GF_EINVAL, "gf_slab_set_targets: give all three targets or none");
@@ -738,6 +782,7 @@ static int slab_check(gf_ctx* c, int parity, const char* who) {
 }
 
 int gf_slab_pack_top(gf_ctx* c, int parity) {
+  DeviceGuard gf_device_guard_(c);
   int rc = slab_check(c, parity, "gf_slab_pack_top: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
   cudaError_t e = launch_slab_top(c->k, parity, c->fwd_target[parity] ? c->fwd_target[parity] : c->top_out, true);
@@ -747,6 +792,7 @@ int gf_slab_pack_top(gf_ctx* c, int parity) {
 }
 
 int gf_slab_unpack_top(gf_ctx* c, int parity) {
+  DeviceGuard gf_device_guard_(c);
   int rc = slab_check(c, parity, "gf_slab_unpack_top: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
   cudaError_t e = launch_slab_top(c->k, parity, c->top_in, false);
@@ -757,6 +803,7 @@ int gf_slab_unpack_top(gf_ctx* c, int parity) {
 }
 
 int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
+  DeviceGuard gf_device_guard_(c);
   int rc = slab_check(c, parity, "gf_slab_halfsweep_border: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_border: omega outside [1,2)");
@@ -771,6 +818,7 @@ int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
 }
 
 int gf_slab_halfsweep_interior(gf_ctx* c, int parity, double omega) {
+  DeviceGuard gf_device_guard_(c);
   int rc = slab_check(c, parity, "gf_slab_halfsweep_interior: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_slab_halfsweep_interior: omega outside [1,2)");

@@ -3,10 +3,36 @@
 //   ovr_halfsweep            : one parity of the overrelaxation sweep                  (Algorithm 1 l.3-12)
 //   measure_partial / _final : F and theta, two-stage deterministic reduction          (eqs. 1.1-1.3)
 //   reunit                   : Gram-Schmidt reunitarisation of every link
+#include <atomic>
+
 #include "gf_device.cuh"
 #include "gf_internal.h"
 
 namespace gf {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: a process that drives contexts on several
+// GPUs must opt in once on each of them.  One flag per (kernel instantiation, device); racing host threads at worst
+// set the attribute twice.
+struct PerDeviceOnce {
+  std::atomic<unsigned long long> done[2];
+  template <class F>
+  cudaError_t run(F&& f) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 128) return f();
+    std::atomic<unsigned long long>& w = done[dev >> 6];
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (w.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    e = f();
+    if (e == cudaSuccess) w.fetch_or(bit, std::memory_order_release);
+    return e;
+  }
+};
+template <class K>
+static cudaError_t opt_in_smem(PerDeviceOnce& once, K kern, size_t bytes) {
+  return once.run([&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes); });
+}
 
 // ======================================================================================================================
 // canonical <-> internal
@@ -379,12 +405,8 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
   using C = cplx_t<T>;
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false>;
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr, nullptr);
   return cudaGetLastError();
@@ -396,12 +418,8 @@ static cudaError_t halfsweep_series_T(const KernelArgs& a, int parity, double om
   using C = cplx_t<T>;
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, false, true>;
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, a.series, nullptr, nullptr);
   return cudaGetLastError();
@@ -416,12 +434,8 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   if (cb_end <= cb_begin && cb2_end <= cb2_begin) return cudaSuccess;
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   SlabView sv = a.slab;
   sv.cb_begin = cb_begin; sv.cb_end = cb_end;
   sv.cb2_begin = cb2_begin; sv.cb2_end = cb2_end;
@@ -493,12 +507,8 @@ static cudaError_t halfsweep_masked_T(const KernelArgs& a, int parity, double om
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, true>;
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, active, nullptr);
   return cudaGetLastError();
@@ -519,12 +529,8 @@ static cudaError_t halfsweep_defer_T(const KernelArgs& a, int parity, double ome
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, false, true>;
-  static bool attr_set = false;  // per instantiation
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, SlabView{}, 0, nullptr, (C*)acc);
   return cudaGetLastError();

@@ -72,3 +72,18 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".cpp", ".h")):
             assert "paper_1412_1498_b200 import" not in open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1412_1498_b200" not in open(os.path.join(ROOT, "oracle", f)).read()
+
+
+def test_header_compiles_as_c99_and_links_from_c(tmp_path):
+    """include/gf.h is advertised as a C ABI: a C99 translation unit includes it, links libgf.so and walks the error
+    paths that return before any device work."""
+    import subprocess
+
+    libdir = os.path.join(ROOT, "paper_1412_1498_b200")
+    exe = str(tmp_path / "cabi_consumer")
+    subprocess.check_call(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                           os.path.join(ROOT, "tests", "cabi_consumer.c"), "-o", exe, "-L", libdir, "-lgf",
+                           f"-Wl,-rpath,{libdir}"])
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "cabi_consumer: ok" in r.stdout
