@@ -77,7 +77,8 @@ def halfsweep_kernel_name(storage, variant, defer=False):
     """The kernel gf_ovr_sweep launches for this storage format / GF_OPT_SWEEP_VARIANT (csrc/gf_kernels.cu, halfsweep_T)."""
     v = variant or (1 if storage == 8 else 3)
     return {1: "ovr_halfsweep_kernel", 2: "ovr_halfsweep_kernel (L2 bulk prefetch)", 3: "ovr_halfsweep_staged_kernel",
-            4: "ovr_halfsweep_bulk_kernel"}[v] + (" (deferred temporal links)" if defer else "")
+            4: "ovr_halfsweep_staged_kernel<BULK=1> (TMA bulk copies)",
+            5: "ovr_halfsweep_staged_kernel<BULK=2> (forward chunk by TMA bulk copy)"}[v] + (" (deferred temporal links)" if defer else "")
 
 
 def measure_fp_peaks(seconds=0.25):

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace gf {
 
 // ---- scalar traits ------------------------------------------------------------------------------------------------------
@@ -219,19 +221,27 @@ __device__ __forceinline__ void su2_overrelax_series(T r0, T r1, T r2, T r3, T o
 }
 
 // One subgroup step on rows/cols (I,J): K <- gK, G <- gG with g = [[c+i q3, q2+i q1], [-q2+i q1, c-i q3]] embedded.
-// K (and g) are in precision T; G may be kept in a lower precision TG (g is rounded once per step).
+// K is in precision T; G may be kept in a lower precision TG (g is rounded once per step).
+// TS: precision in which g^omega is evaluated from r.  r itself is always formed from K in precision T (the
+// cancellation in the sum of eight links is what is ill-conditioned, not the map r -> g^omega, whose relative
+// condition number is O(1) on the direction r/|r| and omega <= 2 on the angle); with FP32 links TS = float puts
+// sqrt / atan2 / sincos / the division on the FP32 units while K(x) and K <- gK stay FP64.
 // SERIES: g^omega by the truncated series of order `order` instead of the exact power.
-template <int I, int J, bool UPDATE_K, bool SERIES = false, class T, class C, class CG>
-__device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega, int order = 0) {
+// r2min (optional): receives min(*r2min, |r|^2) - the conditioning of this step (see FastPath in gf_kernels.cu).
+template <int I, int J, bool UPDATE_K, bool SERIES = false, class TS = void, class T, class C, class CG>
+__device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega, int order = 0, T* r2min = nullptr) {
   using TG = decltype(G[0].x);
-  const T r0 = K[I * 3 + I].x + K[J * 3 + J].x;
-  const T r1 = -(K[I * 3 + J].y + K[J * 3 + I].y);
-  const T r2 = K[J * 3 + I].x - K[I * 3 + J].x;
-  const T r3 = -(K[I * 3 + I].y - K[J * 3 + J].y);
-  T c, q1, q2, q3;
-  if (SERIES) su2_overrelax_series(r0, r1, r2, r3, omega, order, c, q1, q2, q3);
-  else su2_overrelax(r0, r1, r2, r3, omega, c, q1, q2, q3);
+  using TE = typename std::conditional<std::is_void<TS>::value, T, TS>::type;
+  const TE r0 = (TE)(K[I * 3 + I].x + K[J * 3 + J].x);
+  const TE r1 = (TE)(-(K[I * 3 + J].y + K[J * 3 + I].y));
+  const TE r2 = (TE)(K[J * 3 + I].x - K[I * 3 + J].x);
+  const TE r3 = (TE)(-(K[I * 3 + I].y - K[J * 3 + J].y));
+  if (r2min) *r2min = fmin(*r2min, (T)(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3));
+  TE ce, e1, e2, e3;
+  if (SERIES) su2_overrelax_series(r0, r1, r2, r3, (TE)omega, order, ce, e1, e2, e3);
+  else su2_overrelax(r0, r1, r2, r3, (TE)omega, ce, e1, e2, e3);
   if (UPDATE_K) {
+    const T c = (T)ce, q1 = (T)e1, q2 = (T)e2, q3 = (T)e3;
     const C g00 = mk<T>(c, q3), g01 = mk<T>(q2, q1), g10 = mk<T>(-q2, q1), g11 = mk<T>(c, -q3);
 #pragma unroll
     for (int col = 0; col < 3; ++col) {
@@ -241,7 +251,7 @@ __device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega, int ord
       K[I * 3 + col] = a; K[J * 3 + col] = b;
     }
   }
-  const TG cg = (TG)c, p1 = (TG)q1, p2 = (TG)q2, p3 = (TG)q3;
+  const TG cg = (TG)ce, p1 = (TG)e1, p2 = (TG)e2, p3 = (TG)e3;
   const CG h00 = mk<TG>(cg, p3), h01 = mk<TG>(p2, p1), h10 = mk<TG>(-p2, p1), h11 = mk<TG>(cg, -p3);
 #pragma unroll
   for (int col = 0; col < 3; ++col) {
@@ -254,14 +264,14 @@ __device__ __forceinline__ void su2_step(C (&K)[9], CG (&G)[9], T omega, int ord
 
 // G = g3 g2 g1 for one site from its K (Algorithm 1 l.5-6; subgroup order (0,1),(1,2),(0,2), reading A4; A8)
 // FINAL_K: also carry K through the last step, so that on return K = G K_in (= K(x) of the updated links).
-template <class T, bool FINAL_K = false, bool SERIES = false, class C, class CG>
-__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], CG (&G)[9], T omega, int order = 0) {
+template <class T, bool FINAL_K = false, bool SERIES = false, class TS = void, class C, class CG>
+__device__ __forceinline__ void site_gauge_rotation(C (&K)[9], CG (&G)[9], T omega, int order = 0, T* r2min = nullptr) {
   using TG = decltype(G[0].x);
 #pragma unroll
   for (int e = 0; e < 9; ++e) G[e] = mk<TG>((e % 4 == 0) ? TG(1) : TG(0), TG(0));
-  su2_step<0, 1, true, SERIES>(K, G, omega, order);
-  su2_step<1, 2, true, SERIES>(K, G, omega, order);
-  su2_step<0, 2, FINAL_K, SERIES>(K, G, omega, order);
+  su2_step<0, 1, true, SERIES, TS>(K, G, omega, order, r2min);
+  su2_step<1, 2, true, SERIES, TS>(K, G, omega, order, r2min);
+  su2_step<0, 2, FINAL_K, SERIES, TS>(K, G, omega, order, r2min);
 }
 
 // rows 0..NROW-1 of G.U

@@ -161,6 +161,16 @@ __device__ __forceinline__ T delta_norm2(const C (&A)[9]) {
 // all-FP32 evaluation of the same formulas does).  The links are FP32 inputs, so their sum in FP64 is exact, and
 // each g is rounded to FP32 once; G = g3 g2 g1, loads, stores and the eight 3x3 products stay in the storage precision.
 using RotationType = double;
+// FP32 storage, fast path of the staged kernel: K(x) and the three SU(2) steps in FP32; a site whose smallest |r|^2
+// over the three steps is below FAST_TAU2 is evaluated again in FP64.  Derivation: with e ~ 1e-6 the
+// rounding of an r component formed from an FP32 K (a few sigma of sqrt(8) u |K_ij|), a step's g^omega moves by
+// dg_k <= omega dr_k / |r_k|, and the next step sees K <- g K with dr_{k+1} ~ e + |K| dg_k: the error is amplified by
+// 2 |K| / |r| from step to step.  With every |r_k| >= tau and |K| ~ 6, dg_3 <= (2 e / tau) (1 + 12/tau + 144/tau^2):
+// tau = 4 gives 6.5e-6, which with the ~6e-6 of the FP32 link products stays inside the 2e-5 one-sweep budget (tau = 1,
+// tried first from a bound that ignored the step-to-step amplification, measured 3.5e-5 on 19 sites of config 2).
+// On a Haar-random start E|r|^2 ~ 11, so nearly every warp takes the FP64 branch in the first sweeps; once F > 0.5
+// (|r|^2 ~ 100) almost none does.
+constexpr float FAST_TAU2 = 16.0f;
 
 // Accumulator of K(x) in RotationType: every real of the 2*ND links is converted and added in FP64 (exact for FP32
 // inputs).  Measured alternative for FP32 storage (config 2, ncu): carrying the sum as an unevaluated FP32 pair with
@@ -280,10 +290,40 @@ __device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
 __device__ __forceinline__ void sched_fence() { asm volatile("" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// ---- bulk copies (the TMA unit's 1-D form, cp.async.bulk; SASS UBLKCP) completing on an mbarrier ----------------------------
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");  // visible to the async proxy before the first copy
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned phase) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "GF_MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra GF_MBAR_DONE;\n"
+      "bra GF_MBAR_WAIT;\n"
+      "GF_MBAR_DONE:\n"
+      "}\n" ::"r"(a), "r"(phase)
+      : "memory");
+}
+// bytes: a multiple of 16; both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+               : "memory");
+}
+
 // shared slot of (link l, element e) of this thread: [l][e][THREADS] complex numbers, lane-contiguous (no bank conflicts)
-template <int NELEM, int THREADS, bool FULL, class C>
+template <int NELEM, int STRIDE, bool FULL, class C>
 __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
-  load_link<NELEM, FULL, THREADS>(sm + l * NELEM * THREADS, u);
+  load_link<NELEM, FULL, STRIDE>(sm + l * NELEM * STRIDE, u);
 }
 
 // MEASURE: the launch also leaves, per block, the sum over its sites of sum_ij |Delta_ij(x)|^2 AFTER the update, taken
@@ -296,8 +336,15 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
 // DEFER (Coulomb gauge, gf_defer_*): the temporal links are not touched; instead the site's accumulated rotation
 // A(x) <- G(x) A(x) is kept in `acc` (one matrix per site, layout of one direction of the link field) and applied to
 // them later in one pass (defer_flush_kernel): 6 links + A read and written per site-update instead of 8 links.
+// BULK (GF_OPT_SWEEP_VARIANT 4; plain and MEASURE instantiations): the warp's tile is brought in by the TMA unit instead of
+// 8*NELEM LDGSTS per thread.  Each warp owns a [8 links][NELEM][32] region of shared memory and one mbarrier.  The four
+// forward links of its 32 sites are ONE contiguous chunk of the field (4*NELEM*32 complex numbers): one bulk copy.  The
+// backward links of direction mu are runs of consecutive lanes whose neighbours are consecutive in a tile of the other
+// parity (a whole tile where the row length is a multiple of 32; shorter runs at row ends and periodic wraps); the
+// first lane of a run issues one copy per element.  Runs that are not 16-byte aligned on both sides (FP32 complex is
+// 8 bytes) are fetched by their lanes with cp.async as in the non-bulk kernel.
 template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool MEASURE, bool SLAB, bool SERIES = false,
-          bool MASKED = false, bool DEFER = false>
+          bool MASKED = false, bool DEFER = false, int BULK = 0>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials,
                             SlabView sv, int series = 0, const unsigned char* __restrict__ active = nullptr,
@@ -305,8 +352,15 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   using C = cplx_t<T>;
   using TK = RotationType;
   using CK = cplx_t<TK>;
+  static_assert(!BULK || (!SLAB && !MASKED && !DEFER), "the bulk-copy variant exists for the plain half-sweep only");
+  // shared slot of (link, element): [SLOT][e][STRIDE]; non-bulk: links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu), one column
+  // per thread of the block; bulk: links mu = U_mu(x), 4+mu = U_mu(x-mu), one [8][NELEM][32] region per warp
+  constexpr int STRIDE = BULK ? 32 : THREADS;
+  auto slot_fwd = [](int mu) { return BULK ? mu : 2 * mu; };
+  auto slot_bwd = [](int mu) { return BULK ? 4 + mu : 2 * mu + 1; };
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  C* sm = reinterpret_cast<C*>(smem_raw) + threadIdx.x;
+  C* sm = BULK ? reinterpret_cast<C*>(smem_raw) + (threadIdx.x >> 5) * (8 * NELEM * 32) + (threadIdx.x & 31)
+               : reinterpret_cast<C*>(smem_raw) + threadIdx.x;
   int cb = blockIdx.x * THREADS + threadIdx.x;
   bool live = cb < g.vh;
   if (SLAB) {
@@ -314,60 +368,140 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     cb = second ? sv.cb2_begin + (blockIdx.x - sv.nblocks0) * THREADS + threadIdx.x : sv.cb_begin + cb;
     live = cb < (second ? sv.cb2_end : sv.cb_end);
   }
-  if (!MEASURE && !live) return;
+  if (!MEASURE && !BULK && !live) return;
   if (MASKED && !active[cb / g.s3]) return;  // the slice is finished (its theta_t is below eps)
   double q = 0.0;
+  C* fwd = nullptr;
+  C* bwd[4] = {nullptr, nullptr, nullptr, nullptr};
+  if (BULK) {
+    const unsigned lane = threadIdx.x & 31;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + (size_t)8 * NELEM * THREADS * sizeof(C)) +
+                              (threadIdx.x >> 5);
+    if (lane == 0) mbar_init(bar, 1);
+    const unsigned livem = __ballot_sync(0xffffffffu, live);
+    if (livem != 0) {  // (a whole warp beyond the lattice has nothing to fetch; warp-uniform)
+    if (live) site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
+    // runs of consecutive neighbours per direction; 16-byte alignment decides bulk copy or cp.async for the direction
+    unsigned startm[4], bytes = 0;
+    bool use_bulk[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      const unsigned long long p = (unsigned long long)bwd[mu];
+      const unsigned long long prev = __shfl_up_sync(0xffffffffu, p, 1);
+      const bool prev_live = (livem >> ((lane + 31) & 31)) & 1u;
+      const bool start = live && (lane == 0 || !prev_live || p != prev + sizeof(C));
+      startm[mu] = __ballot_sync(0xffffffffu, start);
+      // the run of this start lane ends before the next start or the first dead lane
+      const unsigned stops = (startm[mu] | ~livem) & ~((2u << lane) - 1u);
+      const unsigned len = (stops ? (unsigned)__ffs((int)stops) - 1u : 32u) - lane;
+      const bool aligned = sizeof(C) == 16 || (((p | (len * sizeof(C)) | (lane * sizeof(C))) & 15u) == 0);
+      use_bulk[mu] = BULK == 1 && __all_sync(0xffffffffu, !start || aligned);  // BULK == 2: forward chunk only
+      if (start && use_bulk[mu]) bytes += len * NELEM * (unsigned)sizeof(C);
+      startm[mu] = start ? len : 0u;  // from here on: this lane's run length (0: not a start lane)
+    }
+    bytes = __reduce_add_sync(0xffffffffu, bytes) + 4u * NELEM * 32u * (unsigned)sizeof(C);
+    __syncwarp();
+    if (lane == 0) {
+      mbar_arrive_expect_tx(bar, bytes);
+      // the forward chunk of the tile (padding lanes of the last tile included: they are part of the layout)
+      bulk_g2s(sm, links + link_offset<NELEM>(g, parity, cb & ~31, 0), 4u * NELEM * 32u * (unsigned)sizeof(C), bar);
+    }
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      if (use_bulk[mu]) {
+        if (startm[mu]) {
+#pragma unroll
+          for (int e = 0; e < NELEM; ++e)
+            bulk_g2s(sm + (slot_bwd(mu) * NELEM + e) * 32, bwd[mu] + e * 32, startm[mu] * (unsigned)sizeof(C), bar);
+        }
+      } else if (live) {
+#pragma unroll
+        for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + (slot_bwd(mu) * NELEM + e) * 32, bwd[mu] + e * 32);
+      }
+    }
+    if (sizeof(C) != 16 || BULK == 2) cp_async_wait_all();
+    mbar_wait(bar, 0);
+    }
+  }
   if (live) {
-    C* fwd;
-    C* bwd[4];
-    site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
+    if (!BULK) site_pointers<T, NELEM>(links, g, parity, cb, fwd, bwd);
     if (SLAB && cb < g.s3) bwd[3] = ghost_link<T, NELEM, C>(sv, parity ^ 1, cb);
 
-    // links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu); DEFER: slot 6 = A(x), the temporal links stay where they are
+    // DEFER: slot 6 = A(x), the temporal links stay where they are
     constexpr int NMU = DEFER ? 3 : 4;
     C* accp = nullptr;
     if (DEFER) accp = acc + (((size_t)parity * g.nblk + (size_t)(cb >> 5)) * NELEM) * 32 + (cb & 31);
+    if (!BULK) {
 #pragma unroll
-    for (int mu = 0; mu < NMU; ++mu) {
+      for (int mu = 0; mu < NMU; ++mu) {
 #pragma unroll
-      for (int e = 0; e < NELEM; ++e) {
-        cp_async<sizeof(C)>(sm + ((2 * mu) * NELEM + e) * THREADS, fwd + (mu * NELEM + e) * 32);
-        cp_async<sizeof(C)>(sm + ((2 * mu + 1) * NELEM + e) * THREADS, bwd[mu] + e * 32);
+        for (int e = 0; e < NELEM; ++e) {
+          cp_async<sizeof(C)>(sm + (slot_fwd(mu) * NELEM + e) * STRIDE, fwd + (mu * NELEM + e) * 32);
+          cp_async<sizeof(C)>(sm + (slot_bwd(mu) * NELEM + e) * STRIDE, bwd[mu] + e * 32);
+        }
       }
+      if (DEFER) {
+#pragma unroll
+        for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + (6 * NELEM + e) * STRIDE, accp + e * 32);
+      }
+      cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
     }
-    if (DEFER) {
-#pragma unroll
-      for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + (6 * NELEM + e) * THREADS, accp + e * 32);
-    }
-    cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
-
-    KSum<T> ks;
-    ks.clear();
-#pragma unroll
-    for (int mu = 0; mu < ND; ++mu) {
-      C u[9];
-      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
-#pragma unroll
-      for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
-      sched_fence();
-      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu + 1, u);
-#pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
-      sched_fence();
-    }
-    CK K[9];
-    ks.finish(K);
 
     C G[9];
-    site_gauge_rotation<TK, MEASURE, SERIES>(K, G, (TK)omega, series);
-    if (MEASURE) q = (double)delta_norm2<TK>(K);
+    // FP32 links, exact power: the site rotation is first evaluated in FP32 (K(x), the three SU(2) steps); where a
+    // step's |r|^2 falls below FAST_TAU2 the direction r/|r| amplifies the rounding of K beyond the parity budget and
+    // the site is evaluated again in FP64 from the links still in shared memory (a rare, divergent branch).
+    bool rotated = false;
+    if constexpr (sizeof(T) == 4 && !SERIES) {
+      C Kf[9];
+#pragma unroll
+      for (int e = 0; e < 9; ++e) Kf[e] = mk<T>(T(0), T(0));
+#pragma unroll
+      for (int mu = 0; mu < ND; ++mu) {
+        C u[9];
+        load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) { Kf[e].x += u[e].x; Kf[e].y += u[e].y; }
+        sched_fence();
+        load_link_smem<NELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int j = 0; j < 3; ++j) { Kf[i * 3 + j].x += u[j * 3 + i].x; Kf[i * 3 + j].y -= u[j * 3 + i].y; }
+        sched_fence();
+      }
+      T r2min = T(3.0e38);
+      site_gauge_rotation<T, MEASURE, false>(Kf, G, omega, 0, &r2min);
+      if (MEASURE) q = (double)delta_norm2<T>(Kf);
+      rotated = r2min >= FAST_TAU2;
+    }
+    if (!rotated) {
+      KSum<T> ks;
+      ks.clear();
+#pragma unroll
+      for (int mu = 0; mu < ND; ++mu) {
+        C u[9];
+        load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
+        sched_fence();
+        load_link_smem<NELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
+        sched_fence();
+      }
+      CK K[9];
+      ks.finish(K);
+      site_gauge_rotation<TK, MEASURE, SERIES>(K, G, (TK)omega, series);
+      if (MEASURE) q = (double)delta_norm2<TK>(K);
+    }
 
 #pragma unroll
     for (int mu = 0; mu < NMU; ++mu) {
       C u[9], w[9];
-      load_link_smem<NELEM, THREADS, true>(sm, 2 * mu, u);
+      load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
       mul_left<LinkRows<NELEM>::value>(G, u, w);                       // U_mu(x) <- G U_mu(x)
       store_link<NELEM>(fwd + mu * NELEM * 32, w);
       if (SLAB && mu == 3 && sv.top_out && cb >= g.vh - g.s3) {  // top slice: the copy that goes to the upper neighbour
@@ -376,7 +510,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
         store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb - (g.vh - g.s3)), w);
       }
       sched_fence();
-      load_link_smem<NELEM, THREADS, false>(sm, 2 * mu + 1, u);
+      load_link_smem<NELEM, STRIDE, false>(sm, slot_bwd(mu), u);
       mul_right_adj<LinkRows<NELEM>::value>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
       store_link<NELEM>(bwd[mu], w);
       if (SLAB && mu == 3 && sv.ret_out && cb < g.s3) {   // bottom slice: the copy that goes back to the lower neighbour
@@ -388,7 +522,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     }
     if (DEFER) {                                          // A(x) <- G A(x)
       C u[9], w[9];
-      load_link_smem<NELEM, THREADS, true>(sm, 6, u);
+      load_link_smem<NELEM, STRIDE, true>(sm, 6, u);
       mul_left<LinkRows<NELEM>::value>(G, u, w);
       store_link<NELEM>(accp, w);
     }
@@ -405,6 +539,19 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
   using C = cplx_t<T>;
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false>;
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
+  const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
+  kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr, nullptr);
+  return cudaGetLastError();
+}
+
+// GF_OPT_SWEEP_VARIANT 4: the tile comes in through bulk copies (TMA unit) completing on one mbarrier per warp
+template <class T, int NELEM, int ND, int THREADS, bool MEASURE, int BULK>
+static cudaError_t halfsweep_bulk_T(const KernelArgs& a, int parity, double omega) {
+  using C = cplx_t<T>;
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C) + 8 * (THREADS / 32);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false, false, false, false, BULK>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
@@ -456,11 +603,24 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
   // 8-real storage: the default is the two-pass kernel (no staging area, so occupancy is set by registers alone, which
   // the dependent chains of the link reconstruction need: 7.6 ms against 10.8 ms staged on the cfg4 lattice)
   const int variant = (a.variant == 0 && NELEM == 4) ? 1 : a.variant;
-  if (variant == 0 || variant == 3) {
+  if (variant == 0 || variant == 3 || variant == 4 || variant == 5) {
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
     constexpr int THREADS = staged_threads<T>();
     if (a.block_threads && a.block_threads != THREADS) return cudaErrorInvalidValue;
-    if (a.series > 0) return halfsweep_series_T<T, NELEM, ND, THREADS>(a, parity, omega);
+    if (a.series > 0) return variant >= 4 ? cudaErrorNotSupported : halfsweep_series_T<T, NELEM, ND, THREADS>(a, parity, omega);
+    if constexpr (NELEM != 4) {
+      if (variant == 4 || variant == 5) {
+        if (fuse_theta) {
+          *qblocks = (a.geo.vh + THREADS - 1) / THREADS;
+          return variant == 4 ? halfsweep_bulk_T<T, NELEM, ND, THREADS, true, 1>(a, parity, omega)
+                              : halfsweep_bulk_T<T, NELEM, ND, THREADS, true, 2>(a, parity, omega);
+        }
+        return variant == 4 ? halfsweep_bulk_T<T, NELEM, ND, THREADS, false, 1>(a, parity, omega)
+                            : halfsweep_bulk_T<T, NELEM, ND, THREADS, false, 2>(a, parity, omega);
+      }
+    } else if (variant == 4 || variant == 5) {
+      return cudaErrorNotSupported;
+    }
     if (fuse_theta) {
       *qblocks = (a.geo.vh + THREADS - 1) / THREADS;
       return halfsweep_staged_T<T, NELEM, ND, THREADS, true>(a, parity, omega);
@@ -630,7 +790,7 @@ cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pac
 }
 
 bool halfsweep_can_fuse_theta(const KernelArgs& a) {
-  return (a.variant == 3 || (a.variant == 0 && a.storage != 8)) && a.series == 0;
+  return (a.variant == 3 || a.variant == 4 || a.variant == 5 || (a.variant == 0 && a.storage != 8)) && a.series == 0;
 }
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
