@@ -136,3 +136,58 @@ def as_complex(links: np.ndarray) -> np.ndarray:
     """(…,3,3,2) real view -> (…,3,3) complex view (no copy)."""
     ct = np.complex128 if links.dtype == np.float64 else np.complex64
     return links.view(ct)[..., 0]
+
+
+# ---- SU(N) fields (general number of colours, host only) ---------------------------------------------------------------
+# The same recipe with N x N matrices, in numpy: U_mu(x) = G(x) exp(i r H_mu(x)) G(x+mu)^dagger, H = sum_a c_a lambda_a
+# over the N^2 - 1 generalised Gell-Mann matrices (Tr lambda_a lambda_b = 2 delta_ab), c_a ~ N(0,1); G(x) Haar SU(N).
+# Random numbers: numpy's PCG64 seeded by (seed, N); drawn in one fixed order, so a field is reproducible as a whole.
+def _gellmann_hermitian(rng, n, N):
+    """n random traceless Hermitian N x N matrices sum_a c_a lambda_a with unit-variance coefficients."""
+    H = np.zeros((n, N, N), dtype=np.complex128)
+    for i in range(N):
+        for j in range(i + 1, N):
+            cs, ca = rng.normal(size=n), rng.normal(size=n)  # symmetric and antisymmetric generator of the pair
+            H[:, i, j] = cs - 1j * ca
+            H[:, j, i] = cs + 1j * ca
+    for k in range(1, N):  # diagonal generators sqrt(2/(k(k+1))) diag(1,..,1,-k,0,..)
+        c = rng.normal(size=n) * np.sqrt(2.0 / (k * (k + 1)))
+        for i in range(k):
+            H[:, i, i] += c
+        H[:, k, k] -= k * c
+    return H
+
+
+def _haar_sun(rng, n, N):
+    z = rng.normal(size=(n, N, N)) + 1j * rng.normal(size=(n, N, N))
+    q, r = np.linalg.qr(z)
+    d = np.diagonal(r, axis1=-2, axis2=-1)
+    q = q * (d / np.abs(d))[:, None, :]
+    det = np.linalg.det(q)
+    return q * np.exp(-1j * np.angle(det) / N)[:, None, None]
+
+
+def make_gauge_sun(dims, ncolors: int, seed: int) -> np.ndarray:
+    """The hidden Haar-random rotation G(x), complex128 (V,N,N)."""
+    _, vol = _dims(dims)
+    return _haar_sun(np.random.default_rng([int(seed), int(ncolors), 1]), vol, int(ncolors))
+
+
+def make_links_sun(dims, ncolors: int, roughness: float, seed: int, dtype=np.float64) -> np.ndarray:
+    """SU(N) links of the whole lattice in the canonical layout, shape (V,4,N,N,2)."""
+    N = int(ncolors)
+    nx, ny, nz, nt = (int(v) for v in dims)
+    _, vol = _dims(dims)
+    G = make_gauge_sun(dims, N, seed).reshape(nt, nz, ny, nx, N, N)
+    rng = np.random.default_rng([int(seed), N, 2])
+    out = np.empty((vol, 4, N, N), dtype=np.complex128)
+    for mu in range(4):
+        H = _gellmann_hermitian(rng, vol, N)
+        w, v = np.linalg.eigh(H)
+        E = (v * np.exp(1j * roughness * w)[:, None, :]) @ np.conj(np.swapaxes(v, -1, -2))  # exp(i r H), det = 1
+        Gup = np.roll(G, -1, axis=3 - mu).reshape(vol, N, N)  # G(x + mu)
+        out[:, mu] = G.reshape(vol, N, N) @ E @ np.conj(np.swapaxes(Gup, -1, -2))
+    res = np.empty((vol, 4, N, N, 2), dtype=np.dtype(dtype))
+    res[..., 0] = out.real
+    res[..., 1] = out.imag
+    return np.ascontiguousarray(res)
