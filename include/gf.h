@@ -72,6 +72,19 @@ size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage)
 int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec, int storage, void* dev_workspace,
               size_t workspace_bytes, void* cuda_stream);
 
+/* General number of colours ("SU(N) with N>2": "iterating over its N(N-1)/2 SU(2)
+ * subgroups"; readings A24, A25 in DESIGN.md).  ncolors = 3 is gf_create with storage = 18; ncolors = 2 and 4 run the
+ * general kernels: all N^2 complex entries of a link are stored, the canonical layout is
+ * links[site][mu][row][col][re,im] with N x N matrices (8 N^2 V elements), the subgroups (i,j), i < j, are visited by
+ * increasing j - i, then i, F is normalised by d N V and theta by N V, and reunitarisation is Gram-Schmidt over the rows
+ * followed by the last row times conj(det).  On such a context gf_set/get_links[_host], gf_ovr_sweep, gf_measure,
+ * gf_fix, gf_get_history, gf_reunitarize and gf_set_reunit_every work as described here; every other call
+ * (gf_set_option, gf_fft_*, gf_slab_*, gf_defer_*, gf_*_slices) returns GF_EUNSUPPORTED.  Other ncolors:
+ * GF_EUNSUPPORTED (gf_workspace_bytes_sun: 0). */
+size_t gf_workspace_bytes_sun(int ncolors, int nx, int ny, int nz, int nt, int prec);
+int gf_create_sun(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt, int gauge, int prec, void* dev_workspace,
+                  size_t workspace_bytes, void* cuda_stream);
+
 /* Canonical layout (device) -> internal layout.  With storage = 12 only rows 0 and 1 are kept.  Resets the sweep
  * counter used by the reunitarisation cadence.  Async. */
 int gf_set_links(gf_ctx* ctx, const void* dev_links);

@@ -24,7 +24,8 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_fft_workspace_bytes", "gf_fft_attach", "gf_fft_step", "gf_fix_fft",
            "gf_measure_slices", "gf_fix_slices", "gf_defer_bytes", "gf_defer_attach", "gf_defer_flush",
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
-           "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma"]
+           "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma", "gf_workspace_bytes_sun",
+           "gf_create_sun"]
 
 
 def _load() -> ctypes.CDLL:
@@ -33,6 +34,10 @@ def _load() -> ctypes.CDLL:
     lib.gf_workspace_bytes.argtypes = [c_int] * 6
     lib.gf_create.restype = c_int
     lib.gf_create.argtypes = [POINTER(c_void_p)] + [c_int] * 7 + [c_void_p, c_size_t, c_void_p]
+    lib.gf_workspace_bytes_sun.restype = c_size_t
+    lib.gf_workspace_bytes_sun.argtypes = [c_int] * 6
+    lib.gf_create_sun.restype = c_int
+    lib.gf_create_sun.argtypes = [POINTER(c_void_p)] + [c_int] * 7 + [c_void_p, c_size_t, c_void_p]
     for name in ("gf_set_links", "gf_get_links", "gf_set_links_host", "gf_get_links_host"):
         getattr(lib, name).restype = c_int
         getattr(lib, name).argtypes = [c_void_p, c_void_p]
@@ -113,6 +118,18 @@ def gf_create(nx, ny, nz, nt, gauge, prec, storage, dev_workspace: int, workspac
     h = c_void_p()
     rc = lib.gf_create(byref(h), nx, ny, nz, nt, gauge, prec, storage, c_void_p(dev_workspace), workspace_bytes,
                        c_void_p(cuda_stream))
+    return rc, h
+
+
+def gf_workspace_bytes_sun(ncolors, nx, ny, nz, nt, prec) -> int:
+    return int(lib.gf_workspace_bytes_sun(ncolors, nx, ny, nz, nt, prec))
+
+
+def gf_create_sun(ncolors, nx, ny, nz, nt, gauge, prec, dev_workspace: int, workspace_bytes: int, cuda_stream: int):
+    """Returns (rc, ctx_handle)."""
+    h = c_void_p()
+    rc = lib.gf_create_sun(byref(h), ncolors, nx, ny, nz, nt, gauge, prec, c_void_p(dev_workspace), workspace_bytes,
+                           c_void_p(cuda_stream))
     return rc, h
 
 
@@ -280,26 +297,34 @@ _PREC = {"f64": GF_FP64, "f32": GF_FP32}
 class GaugeFixer:
     """Owns a gf_ctx and the torch workspace tensor behind it.  All methods marshal arguments and check return codes."""
 
-    def __init__(self, dims, gauge="landau", prec="f64", storage=18, device="cuda:0", stream=None):
+    def __init__(self, dims, gauge="landau", prec="f64", storage=18, device="cuda:0", stream=None, ncolors=3):
         import torch
 
         self.torch = torch
         self.dims = tuple(int(d) for d in dims)
         self.gauge, self.prec, self.storage = gauge, prec, int(storage)
+        self.ncolors = int(ncolors)  # 3: gf_create; 2 or 4: gf_create_sun (all N^2 entries stored)
         self.device = torch.device(device)
         self.dtype = torch.float64 if prec == "f64" else torch.float32
         self.volume = 1
         for d in self.dims:
             self.volume *= d
-        nbytes = gf_workspace_bytes(*self.dims, _PREC[prec], self.storage)
+        if self.ncolors == 3:
+            nbytes = gf_workspace_bytes(*self.dims, _PREC[prec], self.storage)
+        else:
+            nbytes = gf_workspace_bytes_sun(self.ncolors, *self.dims, _PREC[prec])
         if nbytes == 0:
             # let gf_create produce the precise error code
             nbytes = 256
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self.workspace = self._alloc(nbytes)
-            rc, self.ctx = gf_create(*self.dims, _GAUGE[gauge], _PREC[prec], self.storage, self.workspace.data_ptr(),
-                                     nbytes, self.stream.cuda_stream)
+            if self.ncolors == 3:
+                rc, self.ctx = gf_create(*self.dims, _GAUGE[gauge], _PREC[prec], self.storage, self.workspace.data_ptr(),
+                                         nbytes, self.stream.cuda_stream)
+            else:
+                rc, self.ctx = gf_create_sun(self.ncolors, *self.dims, _GAUGE[gauge], _PREC[prec],
+                                             self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
         if rc != GF_OK:
             self.ctx = None
             raise GFError(rc)
@@ -317,17 +342,17 @@ class GaugeFixer:
             raise GFError(rc, gf_last_error(self.ctx))
 
     def new_links_buffer(self):
-        """An uninitialised device tensor in the canonical layout (V,4,3,3,2)."""
-        return self.torch.empty((self.volume, 4, 3, 3, 2), dtype=self.dtype, device=self.device)
+        """An uninitialised device tensor in the canonical layout (V,4,N,N,2)."""
+        return self.torch.empty((self.volume, 4, self.ncolors, self.ncolors, 2), dtype=self.dtype, device=self.device)
 
     def set_links(self, links):
-        assert links.is_cuda and links.is_contiguous() and links.dtype == self.dtype and links.numel() == self.volume * 72
+        assert links.is_cuda and links.is_contiguous() and links.dtype == self.dtype and links.numel() == self.volume * 8 * self.ncolors ** 2
         self._check(gf_set_links(self.ctx, links.data_ptr()))
 
     def get_links(self, out=None):
         if out is None:
             out = self.new_links_buffer()
-        assert out.is_cuda and out.is_contiguous() and out.dtype == self.dtype and out.numel() == self.volume * 72
+        assert out.is_cuda and out.is_contiguous() and out.dtype == self.dtype and out.numel() == self.volume * 8 * self.ncolors ** 2
         self._check(gf_get_links(self.ctx, out.data_ptr()))
         return out
 

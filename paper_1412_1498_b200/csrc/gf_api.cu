@@ -41,6 +41,7 @@ Geo make_geo(int nx, int ny, int nz, int nt) {
   return g;
 }
 
+// storage = reals per stored link: 18 / 12 / 8 for SU(3), 2 N^2 for the general SU(N) kernels
 Sizes sizes_of(const Geo& g, int prec, int storage) {
   Sizes s;
   const size_t csize = prec == GF_FP64 ? 16 : 8;
@@ -119,6 +120,11 @@ int fail(gf_ctx* c, int code, const char* msg) {
   return code;
 }
 size_t elem_size(const gf_ctx* c) { return c->k.prec == GF_FP64 ? sizeof(double) : sizeof(float); }
+bool is_sun(const gf_ctx* c) { return c->k.ncolors != 3; }  // the general SU(N) kernels (gf_sun.cu)
+cudaError_t reorder(const gf_ctx* c, bool in, void* canon, long long lex_begin, long long lex_end, const void* chunk_base) {
+  return is_sun(c) ? launch_reorder_sun(c->k, in, canon, lex_begin, lex_end, chunk_base)
+                   : launch_reorder(c->k, in, canon, lex_begin, lex_end, chunk_base);
+}
 long long volume(const gf_ctx* c) { return 2LL * c->k.geo.vh; }
 }  // namespace
 
@@ -132,16 +138,41 @@ size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage)
   return sizes_of(make_geo(nx, ny, nz, nt), prec, storage).total;
 }
 
+size_t gf_workspace_bytes_sun(int ncolors, int nx, int ny, int nz, int nt, int prec) {
+  if (ncolors == 3) return gf_workspace_bytes(nx, ny, nz, nt, prec, 18);
+  int err;
+  if (!sun_supported(ncolors) || !valid_lattice(nx, ny, nz, nt, &err) || (prec != GF_FP64 && prec != GF_FP32)) return 0;
+  return sizes_of(make_geo(nx, ny, nz, nt), prec, 2 * ncolors * ncolors).total;
+}
+
+static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt, int gauge, int prec, int storage,
+                      void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
+
 int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec, int storage, void* dev_workspace,
               size_t workspace_bytes, void* cuda_stream) {
   if (!out) return GF_EINVAL;
   *out = nullptr;
+  if (storage != 18 && storage != 12 && storage != 8) return GF_EUNSUPPORTED;
+  if (storage == 8 && prec != GF_FP64) return GF_EUNSUPPORTED;  // 1/N amplification of rounding: FP64 only (reading A23)
+  return create_ctx(out, 3, nx, ny, nz, nt, gauge, prec, storage, dev_workspace, workspace_bytes, cuda_stream);
+}
+
+int gf_create_sun(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt, int gauge, int prec, void* dev_workspace,
+                  size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return GF_EINVAL;
+  *out = nullptr;
+  if (ncolors == 3) return create_ctx(out, 3, nx, ny, nz, nt, gauge, prec, 18, dev_workspace, workspace_bytes, cuda_stream);
+  if (!sun_supported(ncolors)) return GF_EUNSUPPORTED;
+  return create_ctx(out, ncolors, nx, ny, nz, nt, gauge, prec, 2 * ncolors * ncolors, dev_workspace, workspace_bytes,
+                    cuda_stream);
+}
+
+static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt, int gauge, int prec, int storage,
+                      void* dev_workspace, size_t workspace_bytes, void* cuda_stream) {
   int err;
   if (!valid_lattice(nx, ny, nz, nt, &err)) return err;
   if (gauge != GF_LANDAU && gauge != GF_COULOMB) return GF_EUNSUPPORTED;
   if (prec != GF_FP64 && prec != GF_FP32) return GF_EUNSUPPORTED;
-  if (storage != 18 && storage != 12 && storage != 8) return GF_EUNSUPPORTED;
-  if (storage == 8 && prec != GF_FP64) return GF_EUNSUPPORTED;  // 1/N amplification of rounding: FP64 only (reading A23)
   if (!dev_workspace) return GF_EINVAL;
   const Geo g = make_geo(nx, ny, nz, nt);
   const Sizes sz = sizes_of(g, prec, storage);
@@ -153,6 +184,7 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   c->k.stream = (cudaStream_t)cuda_stream;
   c->k.prec = prec; c->k.storage = storage; c->k.gauge = gauge;
   c->k.variant = 0; c->k.block_threads = 0; c->k.series = 0;
+  c->k.ncolors = ncolors;
   c->sz = sz;
   char* base = (char*)dev_workspace;
   c->k.links = base;
@@ -232,7 +264,7 @@ size_t gf_defer_bytes(const gf_ctx* c) { return c ? defer_bytes(c) : 0; }
 
 int gf_defer_attach(gf_ctx* c, void* dev_acc, size_t bytes) {
   GF_ENTER(c);
-  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8)
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8 || is_sun(c))
     return fail(c, GF_EUNSUPPORTED, "gf_defer_attach: Coulomb gauge on a whole lattice only, 18- or 12-real storage");
   if (!dev_acc) {  // detach: bring the temporal links up to date first
     int rc = defer_flush(c);
@@ -258,7 +290,7 @@ int gf_defer_flush(gf_ctx* c) {
 int gf_set_links(gf_ctx* c, const void* dev_links) {
   GF_ENTER(c);
   if (!dev_links) return fail(c, GF_EINVAL, "gf_set_links: null links");
-  cudaError_t e = launch_reorder(c->k, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
+  cudaError_t e = reorder(c, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
   if (e == cudaSuccess && c->defer_acc && c->defer_dirty) e = launch_defer(c->k, c->defer_acc, false);  // A = 1
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links");
   c->launches += 1;
@@ -273,7 +305,7 @@ int gf_get_links(gf_ctx* c, void* dev_links_out) {
   if (!dev_links_out) return fail(c, GF_EINVAL, "gf_get_links: null output");
   int rc = defer_flush(c);
   if (rc != GF_OK) return rc;
-  cudaError_t e = launch_reorder(c->k, false, dev_links_out, 0, volume(c), nullptr);
+  cudaError_t e = reorder(c, false, dev_links_out, 0, volume(c), nullptr);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_get_links");
   c->launches += 1;
   return GF_OK;
@@ -283,7 +315,7 @@ int gf_get_links(gf_ctx* c, void* dev_links_out) {
 // stream, the reorder kernels on the context's stream, ordered by events per buffer, so that (with pinned host
 // memory) the copy of chunk i+1 runs beside the reorder kernel of chunk i.
 static int links_host(gf_ctx* c, void* host, bool in) {
-  const size_t link_bytes = 18 * elem_size(c);
+  const size_t link_bytes = 2 * (size_t)c->k.ncolors * c->k.ncolors * elem_size(c);
   const long long sites_per_chunk = (long long)(STAGING_BYTES / (4 * link_bytes));
   const long long V = volume(c);
   cudaStream_t main = c->k.stream, copy = c->copy_stream;
@@ -302,11 +334,11 @@ static int links_host(gf_ctx* c, void* host, bool in) {
       if (e == cudaSuccess) e = cudaMemcpyAsync(st, h, bytes, cudaMemcpyHostToDevice, copy);
       if (e == cudaSuccess) e = cudaEventRecord(c->staging_full[b], copy);
       if (e == cudaSuccess) e = cudaStreamWaitEvent(main, c->staging_full[b], 0);
-      if (e == cudaSuccess) e = launch_reorder(c->k, true, nullptr, s0, s1, st);
+      if (e == cudaSuccess) e = reorder(c, true, nullptr, s0, s1, st);
       if (e == cudaSuccess) e = cudaEventRecord(c->staging_free[b], main);
     } else {
       if (i >= 2) e = cudaStreamWaitEvent(main, c->staging_free[b], 0);  // the copy of chunk i-2 has left it
-      if (e == cudaSuccess) e = launch_reorder(c->k, false, nullptr, s0, s1, st);
+      if (e == cudaSuccess) e = reorder(c, false, nullptr, s0, s1, st);
       if (e == cudaSuccess) e = cudaEventRecord(c->staging_full[b], main);
       if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, c->staging_full[b], 0);
       if (e == cudaSuccess) e = cudaMemcpyAsync(h, st, bytes, cudaMemcpyDeviceToHost, copy);
@@ -346,7 +378,7 @@ int gf_reunitarize(gf_ctx* c) {
   int rc = defer_flush(c);  // every link is projected as it would stand after an in-place update
   if (rc != GF_OK) return rc;
   c->qblocks = 0;
-  cudaError_t e = launch_reunit(c->k);
+  cudaError_t e = is_sun(c) ? launch_reunit_sun(c->k) : launch_reunit(c->k);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_reunitarize");
   c->launches += 1;
   return GF_OK;
@@ -361,6 +393,7 @@ int gf_set_reunit_every(gf_ctx* c, int k) {
 
 int gf_set_option(gf_ctx* c, int key, int value) {
   GF_ENTER(c);
+  if (is_sun(c)) return fail(c, GF_EUNSUPPORTED, "gf_set_option: no options on an SU(N != 3) context");
   switch (key) {
     case GF_OPT_SWEEP_VARIANT:
       if (value < 0 || value > 5) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
@@ -401,6 +434,21 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_ovr_sweep: omega outside [1,2)");
   if (c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_ovr_sweep: the context is a slab, use gf_slab_halfsweep_*");
   if (n > 0) c->qblocks = 0;
+  if (is_sun(c)) {  // general SU(N): the N(N-1)/2 subgroups per site, no fused theta terms
+    for (int i = 0; i < n; ++i) {
+      for (int parity = 0; parity < 2; ++parity) {  // even first
+        cudaError_t e = launch_halfsweep_sun(c->k, parity, omega);
+        if (e != cudaSuccess) return fail_cuda(c, e, "gf_ovr_sweep (SU(N))");
+        c->launches += 1;
+      }
+      c->sweeps_total += 1;
+      if (c->reunit_every > 0 && c->sweeps_total % c->reunit_every == 0) {
+        int rc = gf_reunitarize(c);
+        if (rc != GF_OK) return rc;
+      }
+    }
+    return GF_OK;
+  }
   if (c->defer_acc) {  // Coulomb gauge, temporal links deferred: 6 links + A(x) per site-update
     for (int i = 0; i < n; ++i) {
       for (int parity = 0; parity < 2; ++parity) {
@@ -439,10 +487,10 @@ int gf_ovr_sweep(gf_ctx* c, int n, double omega) {
 int gf_measure(gf_ctx* c, double* F, double* theta) {
   GF_ENTER(c);
   if (!F || !theta) return fail(c, GF_EINVAL, "gf_measure: null out-param");
-  cudaError_t e = launch_measure(c->k, c->qblocks);
+  cudaError_t e = is_sun(c) ? launch_measure_sun(c->k) : launch_measure(c->k, c->qblocks);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_measure");
-  c->launches += measure_launches(c->k.geo, c->qblocks);
+  c->launches += is_sun(c) ? 2 : measure_launches(c->k.geo, c->qblocks);
   *F = c->host_result[0];
   *theta = c->host_result[1];
   if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_measure: non-finite F or theta");
@@ -485,7 +533,7 @@ int gf_fix(gf_ctx* c, double omega, double eps, int max_sweeps, int check_every,
 
 // ---- Coulomb gauge, every time slice its own stop test (reading A22) -------------------------------------------------------
 static int slices_check(gf_ctx* c, const char* who) {
-  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, who);
+  if (c->k.gauge != GF_COULOMB || c->k.slab.ghost || c->k.storage == 8 || is_sun(c)) return fail(c, GF_EUNSUPPORTED, who);
   if (!c->host_slices) {
     cudaError_t e = cudaHostAlloc((void**)&c->host_slices, 2 * sizeof(double) * c->k.geo.n[3], cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->dev_slices, c->host_slices, 0);
@@ -592,7 +640,8 @@ int gf_get_history(gf_ctx* c, double* hist, int cap, int* n) {
 
 // ---- Algorithm 2: steepest descent with Fourier acceleration -------------------------------------
 static int fft_plan(gf_ctx* c) {
-  if (c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not built for 8-real storage");
+  if (c->k.storage == 8 && !is_sun(c)) return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not built for 8-real storage");
+  if (is_sun(c)) return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is built for SU(3) only");
   if (c->k.slab.ghost)  // no multi-GPU steepest descent (no distributed 4-D transform)
     return fail(c, GF_EUNSUPPORTED, "Algorithm 2 is not available on a slab context");
   if (c->fft) return GF_OK;
@@ -749,7 +798,7 @@ size_t gf_slab_halo_bytes(const gf_ctx* c) { return c ? c->halo_bytes : 0; }
 int gf_slab_attach(gf_ctx* c, void* dev_halo, size_t bytes) {
   GF_ENTER(c);
   if (!dev_halo) return fail(c, GF_EINVAL, "gf_slab_attach: null workspace");
-  if (c->k.storage == 8) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: not built for 8-real storage");
+  if (c->k.storage == 8 || is_sun(c)) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: SU(3) with 18- or 12-real storage only");
   if (bytes < 4 * c->halo_bytes || ((uintptr_t)dev_halo % ALIGN))
     return fail(c, GF_ENOMEM, "gf_slab_attach: workspace too small or misaligned");
   if (c->fft_w) return fail(c, GF_EUNSUPPORTED, "gf_slab_attach: Algorithm 2 is attached to this context");

@@ -328,4 +328,30 @@ __device__ __forceinline__ void reunitarize(C (&u)[9]) {
   rebuild_row2(u);
 }
 
+// deterministic block sums (warp shuffles, then one shared-memory hop between warps; FP64 in both precisions)
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum of (f, q) over the THREADS threads of the block; valid in thread 0.  Every thread of the block must call it.
+template <int THREADS>
+__device__ __forceinline__ void block_sum2(double& f, double& q) {
+  static_assert(THREADS % 32 == 0 && THREADS <= 1024, "whole warps");
+  constexpr int NW = THREADS / 32;
+  f = warp_sum(f);
+  q = warp_sum(q);
+  if (NW == 1) return;
+  __shared__ double sf[NW], sq[NW];
+  if ((threadIdx.x & 31) == 0) { sf[threadIdx.x >> 5] = f; sq[threadIdx.x >> 5] = q; }
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    f = threadIdx.x < NW ? sf[threadIdx.x] : 0.0;
+    q = threadIdx.x < NW ? sq[threadIdx.x] : 0.0;
+    f = warp_sum(f);
+    q = warp_sum(q);
+  }
+}
+
 }  // namespace gf

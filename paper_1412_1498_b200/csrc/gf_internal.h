@@ -31,6 +31,7 @@ struct KernelArgs {
   int variant;  // half-sweep kernel variant (GF_OPT_SWEEP_VARIANT)
   int block_threads;
   int series;   // GF_OPT_OVR_SERIES: 0 = exact g^omega, N > 0 = truncated binomial series of order N
+  int ncolors;  // 3 (everything above), or 2 / 4: the general SU(N) kernels of gf_sun.cu, N^2 complex numbers per link
   SlabView slab;
 };
 
@@ -62,6 +63,15 @@ cudaError_t launch_halfsweep_masked(const KernelArgs& a, int parity, double omeg
 cudaError_t launch_halfsweep_defer(const KernelArgs& a, int parity, double omega, void* acc);
 cudaError_t launch_defer(const KernelArgs& a, void* acc, bool flush);  // flush: U_t <- A U_t A(x+t)^dag; then A <- 1
 int measure_launches(const Geo& g, int nq);  // kernels launch_measure issues: 1 (small grids) or 2
+cudaError_t launch_measure_tail(const KernelArgs& a, int n, int nf, double norm_f, double norm_q);
+
+// ---- general SU(N) (gf_sun.cu): N = 2, 4, full storage ---------------------------------------------------
+bool sun_supported(int ncolors);
+cudaError_t launch_reorder_sun(const KernelArgs& a, bool in, void* canon, long long lex_begin, long long lex_end,
+                               const void* chunk_base);
+cudaError_t launch_halfsweep_sun(const KernelArgs& a, int parity, double omega);
+cudaError_t launch_measure_sun(const KernelArgs& a);  // 2 launches
+cudaError_t launch_reunit_sun(const KernelArgs& a);
 
 // ---- Algorithm 2 (gf_fftsd.cu): steepest descent with Fourier acceleration ------------------------------------------------
 struct FftPlans;  // the cuFFT plans of one context

@@ -96,34 +96,6 @@ cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long 
                          : reorder_T<float, 6>(a, in, canon, lex_begin, lex_end, chunk_base);
 }
 
-// ======================================================================================================================
-// deterministic block sums (warp shuffles, then one shared-memory hop between warps; FP64 in both precisions)
-// ======================================================================================================================
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
-// Sum of (f, q) over the THREADS threads of the block; valid in thread 0.  Every thread of the block must call it.
-template <int THREADS>
-__device__ __forceinline__ void block_sum2(double& f, double& q) {
-  static_assert(THREADS % 32 == 0 && THREADS <= 1024, "whole warps");
-  constexpr int NW = THREADS / 32;
-  f = warp_sum(f);
-  q = warp_sum(q);
-  if (NW == 1) return;
-  __shared__ double sf[NW], sq[NW];
-  if ((threadIdx.x & 31) == 0) { sf[threadIdx.x >> 5] = f; sq[threadIdx.x >> 5] = q; }
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    f = threadIdx.x < NW ? sf[threadIdx.x] : 0.0;
-    q = threadIdx.x < NW ? sq[threadIdx.x] : 0.0;
-    f = warp_sum(f);
-    q = warp_sum(q);
-  }
-}
-
 // sum_ij |Delta_ij|^2 for Delta = (A - A^dag) - (1/3) Tr(A - A^dag)  (eqs. 1.2-1.3, reading A2).  The sign of A drops
 // out, so A may be sum_nu [U_nu(x-nu) - U_nu(x)] or K(x) of eq. 1.5 (A - A^dag = -(K - K^dag)).
 template <class T, class C>
@@ -923,6 +895,13 @@ static cudaError_t measure_T(const KernelArgs& a, int nq) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess || single) return e;
   measure_tail_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, nblk, tail);
+  return cudaGetLastError();
+}
+
+// second stage alone: F = norm_f * sum of the first nf partials' f, theta = norm_q * sum of all n partials' q -> a.result
+cudaError_t launch_measure_tail(const KernelArgs& a, int n, int nf, double norm_f, double norm_q) {
+  const MeasureTail tail{nullptr, nf, nullptr, 0, norm_f, norm_q, (double*)a.result};
+  measure_tail_kernel<<<1, 1024, 0, a.stream>>>((const double2*)a.partials, n, tail);
   return cudaGetLastError();
 }
 
