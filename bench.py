@@ -36,7 +36,7 @@ if ROOT not in sys.path:
 
 METRIC = "ovr_site_updates_per_s"
 UNIT = "site-updates/s"
-LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48, ("f64", 8): 64}
+LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 48, ("f64", 8): 64, ("f32", 8): 32}
 # nominal flop per site-update (add = mul = 1, FMA = 2; reconstruct + K + 3 subgroup steps + 8
 # products), split into the part the kernels run in FP64 in BOTH storage precisions (K(x) and the three SU(2) steps,
 # DESIGN.md §2 "Precision of the site rotation") and the part that runs in the storage precision.
@@ -75,7 +75,7 @@ def load_peaks():
 
 def halfsweep_kernel_name(storage, variant, defer=False):
     """The kernel gf_ovr_sweep launches for this storage format / GF_OPT_SWEEP_VARIANT (csrc/gf_kernels.cu, halfsweep_T)."""
-    v = variant or (1 if storage == 8 else 3)
+    v = variant or 3
     return {1: "ovr_halfsweep_kernel", 2: "ovr_halfsweep_kernel (L2 bulk prefetch)", 3: "ovr_halfsweep_staged_kernel",
             4: "ovr_halfsweep_staged_kernel<BULK=1> (TMA bulk copies)",
             5: "ovr_halfsweep_staged_kernel<BULK=2> (forward chunk by TMA bulk copy)"}[v] + (" (deferred temporal links)" if defer else "")
@@ -312,6 +312,8 @@ def run_ours(args):
         cfg["storage"] = args.storage
     if args.gauge:
         cfg["gauge"] = args.gauge
+    if args.prec:
+        cfg["prec"] = args.prec
     dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
     V = gi.volume(dims)
     L = LINK_BYTES[(prec, storage)]
@@ -321,6 +323,8 @@ def run_ours(args):
     fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
     if args.defer:
         fx.defer_temporal_links()
+    if storage == 8:  # a study on a rough synthetic field: a few of its 1.3e8 links lie outside the format's domain
+        fx.set_option(gf.GF_OPT_DOMAIN8_CHECK, 0)
     if args.variant:
         fx.set_option(gf.GF_OPT_SWEEP_VARIANT, args.variant)
     if args.block:
@@ -378,7 +382,7 @@ def run_ours(args):
     ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
     achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
     kernel = halfsweep_kernel_name(storage, args.variant, args.defer)
-    traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer) else (None, None)
+    traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer or args.prec) else (None, None)
     # flops leg: the FMA-chain peaks measured now, on this GPU, under the clocks it runs at after
     # the timed region (gf_peak_fma); the site rotation is FP64 in both storage precisions, the link products are in
     # the storage precision
@@ -527,7 +531,7 @@ def run_ours(args):
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": prec, "data": "synthetic",
         "config": {"workload": workload_name(cfg) + (" (deferred temporal links)" if args.defer else "")
-                   + (" [study: not the config's own storage / gauge]" if args.storage or args.gauge else ""),
+                   + (" [study: not the config's own storage / gauge / precision]" if args.storage or args.gauge or args.prec else ""),
                    "step": f"{n_sw} sweeps + 1 F/theta measurement",
                    "sites": V, "l2": "inputs exceed L2 (field %.2f GB vs 126 MB)" % (4 * V * L / 1e9)
                    if 4 * V * L > 4 * 126e6 else "field fits L2: not an HBM measurement", "parallelism": "replicas only",
@@ -723,6 +727,7 @@ def main():
                     help="T-slab sharded sweep with K slabs per rank (secondary line; default 0 = single context / replicas)")
     ap.add_argument("--storage", type=int, default=0, help="kernel study: 18, 12 or 8 (FP64) instead of the config's storage")
     ap.add_argument("--gauge", default="", choices=["", "landau", "coulomb"], help="kernel study: another gauge on the config's lattice")
+    ap.add_argument("--prec", default="", choices=["", "f64", "f32"], help="kernel study: another precision on the config's lattice")
     ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
     ap.add_argument("--peaks", action="store_true", help="print the measured FP64 / FP32 FMA-chain peaks and exit")

@@ -44,11 +44,16 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 enum { GF_LANDAU = 0, GF_COULOMB = 1 }; /* PAPER.md:35 */
 enum { GF_FP64 = 0, GF_FP32 = 1 };      /* PAPER.md:140 (SP/DP) */
 /* storage: 18 (full 3x3), 12 (rows 0,1 stored; row 2 = conj(row0 x row1) rebuilt at every load) or 8 reals per link,
- * PAPER.md:128, 144, 174.  8 (GF_FP64 only; reading A23 in DESIGN.md): a2, a3, b1 and the phases of a1 and c1 are kept,
- * the rest follows from unitarity and det = 1 with a division by N = |a2|^2 + |a3|^2 - undefined for block-diagonal
- * links (N = 0, e.g. the unit field) and less accurate the smaller N is.  With storage = 8 the library offers
- * gf_set/get_links[_host], gf_ovr_sweep, gf_measure, gf_fix, gf_reunitarize; the gf_fft_*, gf_slab_*, gf_defer_*,
- * gf_*_slices calls and GF_OPT_OVR_SERIES return GF_EUNSUPPORTED. */
+ * PAPER.md:128, 144, 174.  8 (reading A23 in DESIGN.md): a2, a3, b1 and the phases of a1 and c1 (each as tan(phase/2))
+ * are kept, the rest follows from unitarity and det = 1 with a division by N = |a2|^2 + |a3|^2.
+ * VALIDITY DOMAIN of storage = 8: undefined for block-diagonal links (N = 0: the unit field, a cold start) and
+ * rounding is amplified by 1/N.  Whenever a link with N < 1e-6 (GF_FP64; error ~1e-10) or N < 1e-3 (GF_FP32; error
+ * ~6e-5) is stored - by gf_set_links or by a sweep - a flag is raised and the next gf_measure, gf_fix or
+ * gf_*_links_host returns GF_ENUMERIC with the reason in gf_last_error (the flag is then cleared; it is kept per
+ * device, not per context).  Smooth fields close to Landau gauge have N ~ |U - 1|^2 and leave the domain: use 12 or
+ * 18 there.  With storage = 8 the library offers gf_set/get_links[_host], gf_ovr_sweep, gf_measure, gf_fix,
+ * gf_reunitarize; the gf_fft_*, gf_slab_*, gf_defer_*, gf_*_slices calls and GF_OPT_OVR_SERIES return
+ * GF_EUNSUPPORTED. */
 
 enum {
   GF_OK = 0,
@@ -150,9 +155,11 @@ int gf_set_reunit_every(gf_ctx* ctx, int k);
 
 /* Tuning knobs for benchmarking kernel variants; the defaults are the fastest measured.  GF_EINVAL on unknown keys. */
 enum {
-  GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (= 3); 1 = two-pass; 2 = two-pass + L2 bulk prefetch;
-                               3 = staged through shared memory with cp.async; see DESIGN.md.  All variants give
-                               bit-identical links. */
+  GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (= 3); 1 = two-pass; 2 = two-pass + L2
+                               bulk prefetch; 3 = staged through shared memory with cp.async; 4 = staged, the tile
+                               fetched by bulk copies of the TMA unit (cp.async.bulk on an mbarrier); 5 = staged, only
+                               the contiguous forward chunk by bulk copy; see DESIGN.md.  {3,4,5} give bit-identical
+                               links, so do {1,2}; in FP64 all five do. */
   GF_OPT_BLOCK_THREADS = 2, /* threads per block of the half-sweep kernel (0 = default; a value the chosen variant
                                has no instantiation for makes the next sweep fail with GF_ECUDA) */
   GF_OPT_FUSE_MEASURE = 3,  /* 1 (default): the last odd half-sweep of every gf_ovr_sweep call also leaves the odd
@@ -167,10 +174,12 @@ enum {
                                (<= 256) and an (x,y) plane fits shared memory, the transforms, the Fourier factor and
                                the inverse transforms run as hand-written passes (5 over the fields in Landau gauge,
                                3 in Coulomb gauge), without cuFFT; other lattices, or 0: the cuFFT path */
-  GF_OPT_OVR_SERIES = 7     /* 0 (default): g^omega of every SU(2) subgroup step is the exact power (reading A6);
+  GF_OPT_OVR_SERIES = 7,    /* 0 (default): g^omega of every SU(2) subgroup step is the exact power (reading A6);
                                N = 1..16: the binomial series sum_{n<=N} binom(omega,n) (g-1)^n, normalised back to
                                SU(2) - the way ref. [1] of the paper evaluates g^omega (reading A21).
                                Default sweep variant only; GF_EUNSUPPORTED on a slab context. */
+  GF_OPT_DOMAIN8_CHECK = 8  /* 1 (default): storage = 8 reports links outside its validity domain (above); 0: the
+                               flag is ignored (kernel studies on rough fields only) */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 

@@ -71,6 +71,7 @@ struct gf_ctx {
   double* dev_slices;   // its device pointer
   int reunit_every;
   int fuse_measure;  // GF_OPT_FUSE_MEASURE
+  int domain8_check;  // GF_OPT_DOMAIN8_CHECK
   int qblocks;       // > 0: k.qpartials[0..qblocks) hold the odd sites' theta terms of the links as they stand
   long long sweeps_total;  // sweeps since the last gf_set_links (reunitarisation cadence)
   long long launches;
@@ -134,7 +135,6 @@ size_t gf_workspace_bytes(int nx, int ny, int nz, int nt, int prec, int storage)
   int err;
   if (!valid_lattice(nx, ny, nz, nt, &err)) return 0;
   if ((prec != GF_FP64 && prec != GF_FP32) || (storage != 18 && storage != 12 && storage != 8)) return 0;
-  if (storage == 8 && prec != GF_FP64) return 0;
   return sizes_of(make_geo(nx, ny, nz, nt), prec, storage).total;
 }
 
@@ -153,7 +153,6 @@ int gf_create(gf_ctx** out, int nx, int ny, int nz, int nt, int gauge, int prec,
   if (!out) return GF_EINVAL;
   *out = nullptr;
   if (storage != 18 && storage != 12 && storage != 8) return GF_EUNSUPPORTED;
-  if (storage == 8 && prec != GF_FP64) return GF_EUNSUPPORTED;  // 1/N amplification of rounding: FP64 only (reading A23)
   return create_ctx(out, 3, nx, ny, nz, nt, gauge, prec, storage, dev_workspace, workspace_bytes, cuda_stream);
 }
 
@@ -194,7 +193,7 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->k.counter = base + sz.links + sz.partials + sz.qpartials;  // the workspace's result slot holds the counter
   c->staging[0] = base + sz.links + sz.partials + sz.qpartials + sz.result;
   c->staging[1] = c->staging[0] + sz.staging;
-  c->fuse_measure = 1; c->qblocks = 0;
+  c->fuse_measure = 1; c->qblocks = 0; c->domain8_check = 1;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0; c->fft_own = 1; c->own_table = nullptr;
@@ -314,6 +313,20 @@ int gf_get_links(gf_ctx* c, void* dev_links_out) {
 // Host <-> device through the two staging buffers: chunk i uses buffer i & 1.  The copies run on the context's own copy
 // stream, the reorder kernels on the context's stream, ordered by events per buffer, so that (with pinned host
 // memory) the copy of chunk i+1 runs beside the reorder kernel of chunk i.
+// 8-real storage: a link stored since the last check had N = |a2|^2 + |a3|^2 below the validity threshold (reading A23)
+static int domain8_check(gf_ctx* c, const char* who) {
+  if (c->k.storage != 8 || c->k.ncolors != 3 || !c->domain8_check) return GF_OK;
+  unsigned flag = 0;
+  cudaError_t e = take_domain_flag(&flag);
+  if (e != cudaSuccess) return fail_cuda(c, e, who);
+  if (flag) {
+    snprintf(c->err, sizeof(c->err), "%s: 8-real storage met a link with |a2|^2+|a3|^2 below %g: outside the domain of "
+             "the parametrisation (nearly block-diagonal link); use storage 12 or 18", who, c->k.prec == GF_FP64 ? 1e-6 : 1e-3);
+    return GF_ENUMERIC;
+  }
+  return GF_OK;
+}
+
 static int links_host(gf_ctx* c, void* host, bool in) {
   const size_t link_bytes = 2 * (size_t)c->k.ncolors * c->k.ncolors * elem_size(c);
   const long long sites_per_chunk = (long long)(STAGING_BYTES / (4 * link_bytes));
@@ -349,7 +362,7 @@ static int links_host(gf_ctx* c, void* host, bool in) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(copy);
   if (e == cudaSuccess) e = cudaStreamSynchronize(main);
   if (e != cudaSuccess) return fail_cuda(c, e, in ? "gf_set_links_host" : "gf_get_links_host");
-  return GF_OK;
+  return domain8_check(c, in ? "gf_set_links_host" : "gf_get_links_host");
 }
 
 int gf_set_links_host(gf_ctx* c, const void* host_links) {
@@ -418,6 +431,9 @@ int gf_set_option(gf_ctx* c, int key, int value) {
         return fail(c, GF_EUNSUPPORTED, "gf_set_option: no series variant on a slab context or with 8-real storage");
       c->k.series = value;
       c->qblocks = 0;
+      return GF_OK;
+    case GF_OPT_DOMAIN8_CHECK:
+      c->domain8_check = value != 0;
       return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
@@ -493,6 +509,7 @@ int gf_measure(gf_ctx* c, double* F, double* theta) {
   c->launches += is_sun(c) ? 2 : measure_launches(c->k.geo, c->qblocks);
   *F = c->host_result[0];
   *theta = c->host_result[1];
+  if (int rc = domain8_check(c, "gf_measure"); rc != GF_OK) return rc;
   if (!std::isfinite(*F) || !std::isfinite(*theta)) return fail(c, GF_ENUMERIC, "gf_measure: non-finite F or theta");
   return GF_OK;
 }

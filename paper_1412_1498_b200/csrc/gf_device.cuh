@@ -93,26 +93,44 @@ __device__ __forceinline__ int cb_down(const Geo& g, const Site& s, int cb, int 
 }
 
 // ---- 8-real storage (NELEM = 4; "Elems = 4", 144, 174; reading A23) --------------------------------------------
-// Stored: a2, a3, b1 and (arg a1, arg c1) for the rows a, b, c of the link.  With N = |a2|^2 + |a3|^2:
+// Stored: a2, a3, b1 and the two phases arg a1, arg c1 for the rows a, b, c of the link.  With N = |a2|^2 + |a3|^2:
 //   |a1| = sqrt(1 - N), |c1| = sqrt(N - |b1|^2)  (row a and column 0 have unit norm);
 //   (b2, b3) = alpha (a2, a3) + beta (-conj a3, conj a2), alpha = -conj(a1) b1 / N, beta = conj(c1) / N;  c = conj(a x b).
-// Undefined for N = 0 (block-diagonal links); rounding is amplified by 1/N near it.
+// A phase theta is kept as its stereographic coordinate t = tan(theta/2), a rational chart of the unit circle:
+//   e^{i theta} = ((1 - t^2) + 2 i t) / (1 + t^2),      t = y / (|z| + x)  (x >= 0)  or  (|z| - x) / y  (x < 0),
+// so that a load costs divisions instead of two sincos and a store a square root and a division instead of atan2
+// (d theta = 2 dt / (1 + t^2): a relative rounding of t moves theta by at most one rounding, also for |t| >> 1).
+// Undefined for N = 0 (block-diagonal links); rounding is amplified by 1/N near it: a store with N below
+// Domain8<T>::n_min raises gf_domain_flag, which gf_measure / gf_get_links_host report as GF_ENUMERIC.
 __device__ __forceinline__ double hypot2_(double x, double y) { return x * x + y * y; }
 __device__ __forceinline__ float hypot2_(float x, float y) { return x * x + y * y; }
-__device__ __forceinline__ void sincos8_(double a, double* s, double* c) { sincos(a, s, c); }
-__device__ __forceinline__ void sincos8_(float a, float* s, float* c) { sincosf(a, s, c); }
+template <class T> struct Domain8;
+template <> struct Domain8<double> { static constexpr double n_min = 1e-6, t_max = 1e75; };
+template <> struct Domain8<float> { static constexpr float n_min = 1e-3f, t_max = 1e9f; };
+static __device__ unsigned gf_domain_flag = 0;  // one per translation unit; only gf_kernels.cu stores 8-real links
 
-template <class T, class C>
+// t = tan(arg(z) / 2) for z = x + i y (0 for z = 0)
+template <class T>
+__device__ __forceinline__ T phase_to_t(T x, T y) {
+  const T m = sqrt(x * x + y * y);
+  const bool right = x >= T(0);
+  const T num = right ? y : m - x, den = right ? m + x : y;
+  T t = den != T(0) ? num / den : (num != T(0) ? Domain8<T>::t_max : T(0));
+  return fmin(fmax(t, -Domain8<T>::t_max), Domain8<T>::t_max);
+}
+
+template <class T, class C, bool ROW2 = true>
 __device__ __forceinline__ void decode8(const C a2, const C a3, const C b1, const C phases, C (&u)[9]) {
   const T N = hypot2_(a2.x, a2.y) + hypot2_(a3.x, a3.y);
-  T sn, cs;
-  sincos8_(phases.x, &sn, &cs);
-  const T ra = sqrt(fmax(T(0), T(1) - N));
-  const C a1 = mk<T>(ra * cs, ra * sn);
-  sincos8_(phases.y, &sn, &cs);
-  const T rc = sqrt(fmax(T(0), N - hypot2_(b1.x, b1.y)));
-  const C c1 = mk<T>(rc * cs, rc * sn);
-  const T invN = T(1) / N;
+  const T ta = phases.x, tc = phases.y;
+  const T da = T(1) + ta * ta, dc = T(1) + tc * tc;
+  // one division for 1/da, 1/dc and 1/N
+  const T inv = T(1) / (da * dc * N);
+  const T inv_da = inv * dc * N, inv_dc = inv * da * N, invN = inv * da * dc;
+  const T ra = sqrt(fmax(T(0), T(1) - N)) * inv_da;
+  const C a1 = mk<T>(ra * (T(1) - ta * ta), ra * (ta + ta));
+  const T rc = sqrt(fmax(T(0), N - hypot2_(b1.x, b1.y))) * inv_dc;
+  const C c1 = mk<T>(rc * (T(1) - tc * tc), rc * (tc + tc));
   // alpha = -conj(a1) b1 / N, beta = conj(c1) / N
   const C alpha = mk<T>(-(a1.x * b1.x + a1.y * b1.y) * invN, -(a1.x * b1.y - a1.y * b1.x) * invN);
   const C beta = mk<T>(c1.x * invN, -c1.y * invN);
@@ -122,7 +140,7 @@ __device__ __forceinline__ void decode8(const C a2, const C a3, const C b1, cons
                alpha.x * a2.y + alpha.y * a2.x - (beta.y * a3.x - beta.x * a3.y));
   u[5] = mk<T>(alpha.x * a3.x - alpha.y * a3.y + (beta.x * a2.x + beta.y * a2.y),
                alpha.x * a3.y + alpha.y * a3.x + (beta.y * a2.x - beta.x * a2.y));
-  rebuild_row2(u);
+  if (ROW2) rebuild_row2(u);
 }
 
 // rows of a product that a store of this storage format needs: 18 reals 3, 12 reals 2, 8 reals 3 (it reads c1)
@@ -146,7 +164,8 @@ __device__ __forceinline__ void store_link(C* __restrict__ p, const C (&u)[9]) {
   if constexpr (NELEM == 4) {
     using T = decltype(u[0].x);
     p[0] = u[1]; p[32] = u[2]; p[64] = u[3];
-    p[96] = mk<T>(atan2(u[0].y, u[0].x), atan2(u[6].y, u[6].x));
+    p[96] = mk<T>(phase_to_t(u[0].x, u[0].y), phase_to_t(u[6].x, u[6].y));
+    if (hypot2_(u[1].x, u[1].y) + hypot2_(u[2].x, u[2].y) < Domain8<T>::n_min) atomicOr(&gf_domain_flag, 1u);
   } else {
 #pragma unroll
     for (int e = 0; e < NELEM; ++e) p[e * 32] = u[e];

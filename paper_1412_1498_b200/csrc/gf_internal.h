@@ -54,6 +54,7 @@ int halfsweep_max_qblocks(const Geo& g);
 // the even sites are visited (every link read once); nq = 0: all sites are visited.
 cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);
+cudaError_t take_domain_flag(unsigned* out);  // 8-real storage: a stored link had N below the validity threshold
 int measure_num_partials(const Geo& g);
 // Coulomb gauge with a stop test per time slice (gf_measure_slices / gf_fix_slices)
 int measure_slices_num_partials(const Geo& g);  // double2 entries launch_measure_slices needs in a.partials

@@ -89,7 +89,9 @@ static cudaError_t reorder_T(const KernelArgs& a, bool in, void* canon, long lon
 
 cudaError_t launch_reorder(const KernelArgs& a, bool in, void* canon, long long lex_begin, long long lex_end,
                            const void* chunk_base) {
-  if (a.storage == 8) return reorder_T<double, 4>(a, in, canon, lex_begin, lex_end, chunk_base);  // FP64 only
+  if (a.storage == 8)
+    return a.prec == 0 ? reorder_T<double, 4>(a, in, canon, lex_begin, lex_end, chunk_base)
+                       : reorder_T<float, 4>(a, in, canon, lex_begin, lex_end, chunk_base);
   if (a.prec == 0) return a.storage == 18 ? reorder_T<double, 9>(a, in, canon, lex_begin, lex_end, chunk_base)
                                           : reorder_T<double, 6>(a, in, canon, lex_begin, lex_end, chunk_base);
   return a.storage == 18 ? reorder_T<float, 9>(a, in, canon, lex_begin, lex_end, chunk_base)
@@ -328,6 +330,11 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   // shared slot of (link, element): [SLOT][e][STRIDE]; non-bulk: links 2*mu = U_mu(x), 2*mu+1 = U_mu(x-mu), one column
   // per thread of the block; bulk: links mu = U_mu(x), 4+mu = U_mu(x-mu), one [8][NELEM][32] region per warp
   constexpr int STRIDE = BULK ? 32 : THREADS;
+  // 8-real storage: the four stored complex numbers of a link land in the upper four of a six-element slot and are
+  // decoded ONCE, in place, into rows 0 and 1; from there on the site works as with 12-real storage (row 2 rebuilt at
+  // each use), so a site-update costs 8 reconstructions instead of 16 and has the 12-real kernel's shared-memory footprint
+  constexpr int SELEM = NELEM == 4 ? 6 : NELEM;
+  constexpr int SOFF = SELEM - NELEM;
   auto slot_fwd = [](int mu) { return BULK ? mu : 2 * mu; };
   auto slot_bwd = [](int mu) { return BULK ? 4 + mu : 2 * mu + 1; };
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -408,8 +415,8 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       for (int mu = 0; mu < NMU; ++mu) {
 #pragma unroll
         for (int e = 0; e < NELEM; ++e) {
-          cp_async<sizeof(C)>(sm + (slot_fwd(mu) * NELEM + e) * STRIDE, fwd + (mu * NELEM + e) * 32);
-          cp_async<sizeof(C)>(sm + (slot_bwd(mu) * NELEM + e) * STRIDE, bwd[mu] + e * 32);
+          cp_async<sizeof(C)>(sm + (slot_fwd(mu) * SELEM + SOFF + e) * STRIDE, fwd + (mu * NELEM + e) * 32);
+          cp_async<sizeof(C)>(sm + (slot_bwd(mu) * SELEM + SOFF + e) * STRIDE, bwd[mu] + e * 32);
         }
       }
       if (DEFER) {
@@ -417,6 +424,17 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
         for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + (6 * NELEM + e) * STRIDE, accp + e * 32);
       }
       cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
+      if constexpr (NELEM == 4) {
+#pragma unroll
+        for (int l = 0; l < 8; ++l) {
+          C* s8 = sm + l * SELEM * STRIDE;
+          C u[9];
+          decode8<T, C, false>(s8[2 * STRIDE], s8[3 * STRIDE], s8[4 * STRIDE], s8[5 * STRIDE], u);
+#pragma unroll
+          for (int e = 0; e < 6; ++e) s8[e * STRIDE] = u[e];
+          sched_fence();
+        }
+      }
     }
 
     C G[9];
@@ -431,11 +449,11 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
 #pragma unroll
       for (int mu = 0; mu < ND; ++mu) {
         C u[9];
-        load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+        load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
 #pragma unroll
         for (int e = 0; e < 9; ++e) { Kf[e].x += u[e].x; Kf[e].y += u[e].y; }
         sched_fence();
-        load_link_smem<NELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+        load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
 #pragma unroll
         for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -453,11 +471,11 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
 #pragma unroll
       for (int mu = 0; mu < ND; ++mu) {
         C u[9];
-        load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+        load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
 #pragma unroll
         for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
         sched_fence();
-        load_link_smem<NELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+        load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
 #pragma unroll
         for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -473,7 +491,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
 #pragma unroll
     for (int mu = 0; mu < NMU; ++mu) {
       C u[9], w[9];
-      load_link_smem<NELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+      load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
       mul_left<LinkRows<NELEM>::value>(G, u, w);                       // U_mu(x) <- G U_mu(x)
       store_link<NELEM>(fwd + mu * NELEM * 32, w);
       if (SLAB && mu == 3 && sv.top_out && cb >= g.vh - g.s3) {  // top slice: the copy that goes to the upper neighbour
@@ -482,7 +500,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
         store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb - (g.vh - g.s3)), w);
       }
       sched_fence();
-      load_link_smem<NELEM, STRIDE, false>(sm, slot_bwd(mu), u);
+      load_link_smem<SELEM, STRIDE, NELEM == 4>(sm, slot_bwd(mu), u);  // (an 8-real store needs c1: all three rows)
       mul_right_adj<LinkRows<NELEM>::value>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
       store_link<NELEM>(bwd[mu], w);
       if (SLAB && mu == 3 && sv.ret_out && cb < g.s3) {   // bottom slice: the copy that goes back to the lower neighbour
@@ -494,7 +512,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     }
     if (DEFER) {                                          // A(x) <- G A(x)
       C u[9], w[9];
-      load_link_smem<NELEM, STRIDE, true>(sm, 6, u);
+      load_link_smem<SELEM, STRIDE, true>(sm, 6, u);
       mul_left<LinkRows<NELEM>::value>(G, u, w);
       store_link<NELEM>(accp, w);
     }
@@ -509,7 +527,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
 template <class T, int NELEM, int ND, int THREADS, bool MEASURE>
 static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = (size_t)8 * (NELEM == 4 ? 6 : NELEM) * THREADS * sizeof(C);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -572,9 +590,7 @@ template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
   using C = cplx_t<T>;
   *qblocks = 0;
-  // 8-real storage: the default is the two-pass kernel (no staging area, so occupancy is set by registers alone, which
-  // the dependent chains of the link reconstruction need: 7.6 ms against 10.8 ms staged on the cfg4 lattice)
-  const int variant = (a.variant == 0 && NELEM == 4) ? 1 : a.variant;
+  const int variant = a.variant;
   if (variant == 0 || variant == 3 || variant == 4 || variant == 5) {
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
     constexpr int THREADS = staged_threads<T>();
@@ -626,9 +642,13 @@ static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bo
   } while (0)
 
 cudaError_t launch_halfsweep(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
-  if (a.storage == 8)  // FP64 only (gf_create)
-    return a.gauge == 1 ? halfsweep_T<double, 4, 3>(a, parity, omega, fuse_theta, qblocks)
-                        : halfsweep_T<double, 4, 4>(a, parity, omega, fuse_theta, qblocks);
+  if (a.storage == 8) {
+    if (a.prec == 0)
+      return a.gauge == 1 ? halfsweep_T<double, 4, 3>(a, parity, omega, fuse_theta, qblocks)
+                          : halfsweep_T<double, 4, 4>(a, parity, omega, fuse_theta, qblocks);
+    return a.gauge == 1 ? halfsweep_T<float, 4, 3>(a, parity, omega, fuse_theta, qblocks)
+                        : halfsweep_T<float, 4, 4>(a, parity, omega, fuse_theta, qblocks);
+  }
   GF_DISPATCH(halfsweep_T, a, parity, omega, fuse_theta, qblocks);
 }
 
@@ -762,7 +782,7 @@ cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pac
 }
 
 bool halfsweep_can_fuse_theta(const KernelArgs& a) {
-  return (a.variant == 3 || a.variant == 4 || a.variant == 5 || (a.variant == 0 && a.storage != 8)) && a.series == 0;
+  return (a.variant == 0 || a.variant == 3 || a.variant == 4 || a.variant == 5) && a.series == 0;
 }
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
@@ -906,7 +926,10 @@ cudaError_t launch_measure_tail(const KernelArgs& a, int n, int nf, double norm_
 }
 
 cudaError_t launch_measure(const KernelArgs& a, int nq) {
-  if (a.storage == 8) return a.gauge == 1 ? measure_T<double, 4, 3>(a, nq) : measure_T<double, 4, 4>(a, nq);
+  if (a.storage == 8) {
+    if (a.prec == 0) return a.gauge == 1 ? measure_T<double, 4, 3>(a, nq) : measure_T<double, 4, 4>(a, nq);
+    return a.gauge == 1 ? measure_T<float, 4, 3>(a, nq) : measure_T<float, 4, 4>(a, nq);
+  }
   GF_DISPATCH(measure_T, a, nq);
 }
 
@@ -965,17 +988,15 @@ cudaError_t launch_measure_slices(const KernelArgs& a, double* out) {
 // ======================================================================================================================
 // One thread per stored link: the internal array is a sequence of (block, mu) tiles of NELEM*32 complex numbers.
 template <class T, int NELEM>
-__global__ void __launch_bounds__(256) reunit_kernel(cplx_t<T>* __restrict__ links, long long ntiles) {
+__global__ void __launch_bounds__(256) reunit_kernel(cplx_t<T>* __restrict__ links, long long ntiles, int nblk, int vh) {
   using C = cplx_t<T>;
   const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long tile = tid >> 5;
+  const long long tile = tid >> 5;  // (parity * nblk + blk) * 4 + mu
   if (tile >= ntiles) return;
+  if (((tile >> 2) % nblk) * 32 + (tid & 31) >= vh) return;  // padding lanes of a parity's last block hold no link
   C* p = links + (size_t)tile * NELEM * 32 + (tid & 31);
   C u[9];
-  if (NELEM == 4 && p[0].x == T(0) && p[0].y == T(0) && p[32].x == T(0) && p[32].y == T(0)) return;  // padding lane
   load_link<NELEM, false>(p, u);
-  // padding lanes of the last block hold zeros: leave them alone (0/0)
-  if (u[0].x == T(0) && u[0].y == T(0) && u[1].x == T(0) && u[1].y == T(0) && u[2].x == T(0) && u[2].y == T(0)) return;
   reunitarize<T>(u);
   store_link<NELEM>(p, u);
 }
@@ -984,12 +1005,23 @@ template <class T, int NELEM>
 static cudaError_t reunit_T(const KernelArgs& a) {
   const long long ntiles = 2LL * a.geo.nblk * 4;
   const unsigned blocks = (unsigned)((ntiles * 32 + 255) / 256);
-  reunit_kernel<T, NELEM><<<blocks, 256, 0, a.stream>>>((cplx_t<T>*)a.links, ntiles);
+  reunit_kernel<T, NELEM><<<blocks, 256, 0, a.stream>>>((cplx_t<T>*)a.links, ntiles, a.geo.nblk, a.geo.vh);
   return cudaGetLastError();
 }
 
+// 8-real storage: has any store since the last call seen a link outside the validity domain (N < Domain8::n_min)?
+// Reads and clears the flag of the current device; the caller has synchronised the stream.
+cudaError_t take_domain_flag(unsigned* out) {
+  cudaError_t e = cudaMemcpyFromSymbol(out, gf_domain_flag, sizeof(unsigned));
+  if (e == cudaSuccess && *out) {
+    const unsigned zero = 0;
+    e = cudaMemcpyToSymbol(gf_domain_flag, &zero, sizeof(unsigned));
+  }
+  return e;
+}
+
 cudaError_t launch_reunit(const KernelArgs& a) {
-  if (a.storage == 8) return reunit_T<double, 4>(a);
+  if (a.storage == 8) return a.prec == 0 ? reunit_T<double, 4>(a) : reunit_T<float, 4>(a);
   if (a.prec == 0) return a.storage == 18 ? reunit_T<double, 9>(a) : reunit_T<double, 6>(a);
   return a.storage == 18 ? reunit_T<float, 9>(a) : reunit_T<float, 6>(a);
 }

@@ -495,35 +495,72 @@ def test_deferred_links_whole_run_with_reunitarisation_and_errors(gf, torch):
     fx.close()
 
 
-# ---- 8-real storage (reading A23): FP64 only; tolerance scaled by the conditioning 1/N of the reconstruction --------------
+# ---- 8-real storage (reading A23); tolerance scaled by the conditioning 1/N of the reconstruction ---------------------------
 @pytest.mark.parametrize("dims", [(8, 8, 8, 8), (6, 4, 2, 2), (10, 6, 4, 4), (2, 2, 2, 2)])
 @pytest.mark.parametrize("gauge", ["landau", "coulomb"])
-def test_8_real_storage_against_oracle(gf, torch, dims, gauge):
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_8_real_storage_against_oracle(gf, torch, dims, gauge, prec):
     omega = 1.7
-    U = gi.make_links(dims, 0.5, 84)
-    Uo = U.copy()
+    f64 = prec == "f64"
+    u = 1.1e-16 if f64 else 6e-8
+    U = gi.make_links(dims, 0.5, 84, dtype=np.float64 if f64 else np.float32)
+    Uo = np.ascontiguousarray(U.astype(np.float64))  # reading A18: the FP64 oracle on the rounded input
     oracle.project8(Uo, dims)
-    fx = gf.GaugeFixer(dims, gauge=gauge, prec="f64", storage=8)
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=8)
     fx.set_links(torch.from_numpy(U).cuda())
-    back = fx.get_links().cpu().numpy()
+    back = fx.get_links().cpu().numpy().astype(np.float64)
     F0, th0 = fx.measure()
     Fo0, tho0 = oracle.measure(Uo, dims, gauge)
-    Uc = U[..., 0] + 1j * U[..., 1]
+    Uc = U[..., 0].astype(np.float64) + 1j * U[..., 1]
     Nmin = (np.abs(Uc[:, :, 0, 1]) ** 2 + np.abs(Uc[:, :, 0, 2]) ** 2).min()
-    assert np.abs(back - Uo).max() <= 1e-14 / Nmin             # storing and reading back = the oracle's round trip
-    assert abs(F0 - Fo0) <= 1e-12 and abs(th0 / tho0 - 1) <= 1e-10
+    assert np.abs(back - Uo).max() <= 100 * u / Nmin           # storing and reading back = the oracle's round trip
+    assert abs(F0 - Fo0) <= (1e-12 if f64 else 1e-5) and abs(th0 / tho0 - 1) <= (1e-10 if f64 else 1e-4)
     fx.ovr_sweep(1, omega)
-    got = fx.get_links().cpu().numpy()
+    got = fx.get_links().cpu().numpy().astype(np.float64)
     F, th = fx.measure()
     fx.reunitarize()
-    after = fx.get_links().cpu().numpy()
+    after = fx.get_links().cpu().numpy().astype(np.float64)
     fx.close()
     oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=8)
     Fo, tho = oracle.measure(Uo, dims, gauge)
-    assert np.abs(got - Uo).max() <= max(1e-12, 1e-13 / Nmin)  # the one-sweep bound, widened where 1/N demands it
-    assert abs(F - Fo) <= 1e-10 * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
-    assert np.abs(after - got).max() <= 1e-12 / Nmin           # the links were unitary: reunitarisation changes nothing
-    assert sum(fx_bytes for fx_bytes in [gf.gf_workspace_bytes(*dims, gf.GF_FP64, 8)]) < gf.gf_workspace_bytes(*dims, gf.GF_FP64, 12)
+    # the one-sweep bound, widened where 1/N demands it (1000 u / N: 1e-13 / N in FP64, 6e-5 / N ... in FP32)
+    assert np.abs(got - Uo).max() <= max(1e-12 if f64 else 2e-5, 1000 * u / Nmin)
+    assert abs(F - Fo) <= (1e-10 if f64 else 1e-5) * abs(Fo) and tho / 1.5 <= th <= tho * 1.5
+    assert np.abs(after - got).max() <= 1e4 * u / Nmin         # the links were unitary: reunitarisation changes nothing
+    assert gf.gf_workspace_bytes(*dims, int(not f64), 8) < gf.gf_workspace_bytes(*dims, int(not f64), 12)
+
+
+def test_8_real_storage_reports_links_outside_its_domain(gf, torch):
+    """A cold start (unit links: N = 0), a pure gauge and a nearly fixed smooth field are where 8-real storage is
+    undefined or inaccurate: the store raises a flag and the next synchronising call says GF_ENUMERIC
+    instead of returning garbage."""
+    dims = (4, 4, 4, 4)
+    V = 256
+    unit = np.zeros((V, 4, 3, 3, 2))
+    unit[:, :, 0, 0, 0] = unit[:, :, 1, 1, 0] = unit[:, :, 2, 2, 0] = 1.0
+    fx = gf.GaugeFixer(dims, prec="f64", storage=8)
+    fx.set_links(torch.from_numpy(unit).cuda())
+    rc, F, th = gf.gf_measure(fx.ctx)
+    assert rc == gf.GF_ENUMERIC and "8-real" in gf.gf_last_error(fx.ctx)
+    # a rough field is inside the domain: the flag was cleared by the report
+    U = gi.make_links(dims, 0.5, 3)
+    fx.set_links(torch.from_numpy(U).cuda())
+    rc, F, th = gf.gf_measure(fx.ctx)
+    assert rc == gf.GF_OK and np.isfinite(F) and np.isfinite(th)
+    # a smooth field driven towards Landau gauge from a cold-ish start: links near 1, N ~ roughness^2
+    Us = gi.make_links(dims, 1e-4, 4)
+    G = gi.make_gauge(dims, 4)  # undo the hidden rotation: the field is then exp(i r H), r = 1e-4
+    Uc = Us[..., 0] + 1j * Us[..., 1]
+    nx, ny, nz, nt = dims
+    Gg = G.reshape(nt, nz, ny, nx, 3, 3)
+    for mu in range(4):
+        Gup = np.roll(Gg, -1, axis=3 - mu).reshape(V, 3, 3)
+        Uc[:, mu] = np.conj(np.swapaxes(G, -1, -2)) @ Uc[:, mu] @ Gup
+    Us = np.ascontiguousarray(np.stack([Uc.real, Uc.imag], axis=-1))
+    fx.set_links(torch.from_numpy(Us).cuda())
+    rc, F, th = gf.gf_measure(fx.ctx)
+    assert rc == gf.GF_ENUMERIC
+    fx.close()
 
 
 def test_8_real_storage_fix_and_unsupported_calls(gf, torch):
@@ -544,6 +581,4 @@ def test_8_real_storage_fix_and_unsupported_calls(gf, torch):
     halo = torch.zeros(4 * B, dtype=torch.uint8, device="cuda")
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
     fx.close()
-    assert gf.gf_workspace_bytes(8, 8, 8, 8, gf.GF_FP32, 8) == 0
-    with pytest.raises(gf.GFError):
-        gf.GaugeFixer(dims, gauge="landau", prec="f32", storage=8)
+    assert gf.gf_workspace_bytes(8, 8, 8, 8, gf.GF_FP32, 8) > 0
