@@ -619,7 +619,9 @@ def run_fftsd(args):
 
 def run_sharded(args):
     """--sharded K: the overrelaxation sweep over T-slabs (paper_1412_1498_b200.sharded; SURVEY.md §8(f) NEXT-2,
-    PAPER.md:132-134).  Every rank holds the config's lattice as K slabs; the global lattice is world x taller (fixed
+    PAPER.md:132-134).  The paper's weak-scaling point (32^4 per GPU) is
+        python bench.py --gpus N --sharded 1 --config cfg2
+    (unmeasured on more than one GPU: this pool leases one).  Every rank holds the config's lattice as K slabs; the global lattice is world x taller (fixed
     local volume per GPU, the paper's weak-scaling set-up).  Secondary line: with one rank the halo
     messages are device-to-device copies and the number is the cost of the border / interior split on one GPU."""
     import torch
@@ -637,6 +639,9 @@ def run_sharded(args):
     if world > 1:
         import torch.distributed as dist
 
+        # NCCL's initialisation lines stay on (stderr), so that a reader of the log can count the ranks and see the transport
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = get_cfg(args.config)
     dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
@@ -692,7 +697,7 @@ def run_sharded(args):
                            "step": f"{n_sw} sweeps + 1 F/theta measurement",
                            "parallelism": f"T-slabs: {n_slabs} slabs over {world} rank(s), {K} per rank",
                            "halo": f"2 messages of {halo // len(sh.engines)} B per slab and half-sweep "
-                                   f"({'stored by the border kernel into the neighbour slab' if sh.direct else 'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
+                                   f"({'stored by the border kernel into the neighbour slab' if sh.direct else 'stored by the border kernel into the CUDA-IPC mapped workspace of the neighbour rank; one 1-element NCCL all-reduce per half-sweep orders the ranks' if sh.ipc else 'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
                            "l2": "inputs exceed L2" if 4 * V * L > 126e6 else "field fits L2 in part",
                            "final_F": F, "final_theta": th},
                 "roofline": {"bound": "hbm", "kernel": "ovr_halfsweep_staged_kernel (border + interior launches)",

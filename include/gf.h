@@ -249,6 +249,31 @@ int gf_fix_fft(gf_ctx* ctx, double alpha, double eps, int max_iters, int check_e
  * slab's unpack before a neighbour's next border kernel.  Pass the three pointers of the neighbours' workspaces (upper:
  * offset 0 and B, lower: offset 3B), or three nulls to go back to top_out.  gf_slab_pack_top then writes to the upper
  * neighbour's ghost[parity] too. */
+/* Between PROCESSES (one per GPU) the neighbours' workspaces are mapped with CUDA IPC and handed to
+ * gf_slab_set_peer_targets: as gf_slab_set_targets, but the "ret" message of the even half-sweep goes to
+ * lower_top_in_even (the lower neighbour's workspace + 3B) and that of the odd half-sweep to lower_top_in_odd (its
+ * workspace + 2B, the top_out slot, unused when messages are delivered directly), and gf_slab_unpack_top(1-p) reads the
+ * buffer half-sweep p filled.  With top_in double-buffered ONE synchronisation of neighbouring ranks per half-sweep is
+ * enough: between the border kernels (all messages stored) and gf_slab_unpack_top; a rank's next border kernel only
+ * writes buffers whose last readers ran before that point.
+ *   gf_ipc_export: a 64-byte CUDA IPC handle of the allocation dev_ptr lies in, and dev_ptr's offset in it (host out).
+ *   gf_ipc_open:   maps that allocation in this process; *dev_ptr = its base + offset.  gf_ipc_close unmaps it.
+ * Errors: GF_EINVAL (null), GF_ECUDA (not a cudaMalloc allocation, same process, no peer access). */
+int gf_slab_set_peer_targets(gf_ctx* ctx, void* upper_ghost0, void* upper_ghost1, void* lower_top_in_even,
+                             void* lower_top_in_odd);
+int gf_ipc_export(const void* dev_ptr, unsigned char* handle64, size_t* offset);
+int gf_ipc_open(const unsigned char* handle64, size_t offset, void** dev_ptr);
+int gf_ipc_close(void* dev_ptr, size_t offset);
+
+/* The driver's decisions of Algorithm 1 for callers that run it over several contexts:
+ *   gf_combine_slabs: global F and theta from the gf_measure values of n_slabs equal slabs (host arrays, slab order):
+ *     their means, added in slab order so that every rank gets the same bits.  GF_ENUMERIC if not finite.
+ *   gf_fix_plan: *n_next = the number of sweeps to do before the next measurement - 0 when theta < eps or
+ *     sweeps_done >= max_sweeps (stop), else min(check_every, max_sweeps - sweeps_done); validates omega in [1,2),
+ *     check_every >= 1, max_sweeps >= 0, eps >= 0 as gf_fix does (GF_EINVAL). */
+int gf_combine_slabs(const double* F_slab, const double* theta_slab, int n_slabs, double* F, double* theta);
+int gf_fix_plan(double omega, double eps, int max_sweeps, int check_every, int sweeps_done, double theta, int* n_next);
+
 size_t gf_slab_halo_bytes(const gf_ctx* ctx);
 int gf_slab_set_targets(gf_ctx* ctx, void* upper_ghost0, void* upper_ghost1, void* lower_top_in);
 int gf_slab_attach(gf_ctx* ctx, void* dev_halo, size_t halo_workspace_bytes);

@@ -25,7 +25,8 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_measure_slices", "gf_fix_slices", "gf_defer_bytes", "gf_defer_attach", "gf_defer_flush",
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma", "gf_workspace_bytes_sun",
-           "gf_create_sun"]
+           "gf_create_sun", "gf_slab_set_peer_targets", "gf_ipc_export", "gf_ipc_open", "gf_ipc_close", "gf_combine_slabs",
+           "gf_fix_plan"]
 
 
 def _load() -> ctypes.CDLL:
@@ -85,6 +86,18 @@ def _load() -> ctypes.CDLL:
     for name in ("gf_slab_halfsweep_border", "gf_slab_halfsweep_interior"):
         getattr(lib, name).restype = c_int
         getattr(lib, name).argtypes = [c_void_p, c_int, c_double]
+    lib.gf_slab_set_peer_targets.restype = c_int
+    lib.gf_slab_set_peer_targets.argtypes = [c_void_p] * 5
+    lib.gf_ipc_export.restype = c_int
+    lib.gf_ipc_export.argtypes = [c_void_p, c_char_p, POINTER(c_size_t)]
+    lib.gf_ipc_open.restype = c_int
+    lib.gf_ipc_open.argtypes = [c_char_p, c_size_t, POINTER(c_void_p)]
+    lib.gf_ipc_close.restype = c_int
+    lib.gf_ipc_close.argtypes = [c_void_p, c_size_t]
+    lib.gf_combine_slabs.restype = c_int
+    lib.gf_combine_slabs.argtypes = [POINTER(c_double), POINTER(c_double), c_int, POINTER(c_double), POINTER(c_double)]
+    lib.gf_fix_plan.restype = c_int
+    lib.gf_fix_plan.argtypes = [c_double, c_double, c_int, c_int, c_int, c_double, POINTER(c_int)]
     lib.gf_peak_fma.restype = c_int
     lib.gf_peak_fma.argtypes = [c_int, c_double, c_void_p, c_void_p, POINTER(c_double)]
     lib.gf_kernel_launches.restype = c_longlong
@@ -248,6 +261,46 @@ def gf_slab_attach(ctx, dev_halo: int, halo_workspace_bytes: int) -> int:
 def gf_slab_set_targets(ctx, upper_ghost0: int, upper_ghost1: int, lower_top_in: int) -> int:
     return lib.gf_slab_set_targets(ctx, c_void_p(upper_ghost0 or None), c_void_p(upper_ghost1 or None),
                                    c_void_p(lower_top_in or None))
+
+
+def gf_slab_set_peer_targets(ctx, upper_ghost0: int, upper_ghost1: int, lower_top_in_even: int, lower_top_in_odd: int) -> int:
+    return lib.gf_slab_set_peer_targets(ctx, c_void_p(upper_ghost0), c_void_p(upper_ghost1), c_void_p(lower_top_in_even),
+                                        c_void_p(lower_top_in_odd))
+
+
+def gf_ipc_export(dev_ptr: int):
+    """Returns (rc, 64-byte handle, offset)."""
+    buf = ctypes.create_string_buffer(64)
+    off = c_size_t()
+    rc = lib.gf_ipc_export(c_void_p(dev_ptr), buf, byref(off))
+    return rc, buf.raw, off.value
+
+
+def gf_ipc_open(handle: bytes, offset: int):
+    """Returns (rc, device pointer)."""
+    p = c_void_p()
+    rc = lib.gf_ipc_open(handle, offset, byref(p))
+    return rc, (p.value or 0)
+
+
+def gf_ipc_close(dev_ptr: int, offset: int) -> int:
+    return lib.gf_ipc_close(c_void_p(dev_ptr), offset)
+
+
+def gf_combine_slabs(F_slab, theta_slab):
+    """Returns (rc, F, theta)."""
+    n = len(F_slab)
+    Fa, ta = (c_double * n)(*F_slab), (c_double * n)(*theta_slab)
+    F, th = c_double(), c_double()
+    rc = lib.gf_combine_slabs(Fa, ta, n, byref(F), byref(th))
+    return rc, F.value, th.value
+
+
+def gf_fix_plan(omega, eps, max_sweeps, check_every, sweeps_done, theta):
+    """Returns (rc, n_next)."""
+    n = c_int()
+    rc = lib.gf_fix_plan(omega, eps, max_sweeps, check_every, sweeps_done, theta, byref(n))
+    return rc, n.value
 
 
 def gf_slab_pack_top(ctx, parity: int) -> int:

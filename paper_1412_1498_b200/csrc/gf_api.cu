@@ -92,6 +92,8 @@ struct gf_ctx {
   char* top_in;       // ghost links coming back from the upper neighbour
   char* fwd_target[2];  // gf_slab_set_targets: the upper neighbour's ghost[0], ghost[1] (peer-mapped), or null
   char* ret_target;     //                      the lower neighbour's top_in, or null
+  char* ret_target_odd; // gf_slab_set_peer_targets: where the odd half-sweep's "ret" message goes (even: ret_target)
+  bool alt_top_in;      // gf_slab_set_peer_targets: unpack_top(1-p) reads top_in (p = 0) or the top_out slot (p = 1)
   char err[256];
 };
 
@@ -201,7 +203,8 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr, nullptr};
   c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
   c->top_out = c->top_in = nullptr;
-  c->fwd_target[0] = c->fwd_target[1] = c->ret_target = nullptr;
+  c->fwd_target[0] = c->fwd_target[1] = c->ret_target = c->ret_target_odd = nullptr;
+  c->alt_top_in = false;
   c->host_result = nullptr;
   c->host_slices = c->dev_slices = nullptr;
   c->defer_acc = nullptr; c->defer_dirty = false;
@@ -836,7 +839,83 @@ int gf_slab_set_targets(gf_ctx* c, void* upper_ghost0, void* upper_ghost1, void*
     return fail(c, GF_EINVAL, "gf_slab_set_targets: give all three targets or none");
   c->fwd_target[0] = (char*)upper_ghost0;
   c->fwd_target[1] = (char*)upper_ghost1;
-  c->ret_target = (char*)lower_top_in;
+  c->ret_target = c->ret_target_odd = (char*)lower_top_in;
+  c->alt_top_in = false;
+  return GF_OK;
+}
+
+int gf_slab_set_peer_targets(gf_ctx* c, void* upper_ghost0, void* upper_ghost1, void* lower_top_in_even,
+                             void* lower_top_in_odd) {
+  GF_ENTER(c);
+  if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_peer_targets: no halo workspace attached (gf_slab_attach)");
+  if (!upper_ghost0 || !upper_ghost1 || !lower_top_in_even || !lower_top_in_odd)
+    return fail(c, GF_EINVAL, "gf_slab_set_peer_targets: null target");
+  c->fwd_target[0] = (char*)upper_ghost0;
+  c->fwd_target[1] = (char*)upper_ghost1;
+  c->ret_target = (char*)lower_top_in_even;
+  c->ret_target_odd = (char*)lower_top_in_odd;
+  c->alt_top_in = true;
+  return GF_OK;
+}
+
+// ---- device memory of another process (CUDA IPC), for gf_slab_set_peer_targets between ranks --------------------------------
+int gf_ipc_export(const void* dev_ptr, unsigned char* handle64, size_t* offset) {
+  if (!dev_ptr || !handle64 || !offset) return GF_EINVAL;
+  // the handle names the whole allocation dev_ptr lies in (torch hands out pieces of larger cudaMalloc segments):
+  // find its base through the driver's cuMemGetAddressRange, looked up at run time (no link dependency on libcuda)
+  typedef int (*range_fn)(unsigned long long*, size_t*, unsigned long long);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn ||
+      q != cudaDriverEntryPointSuccess)
+    return GF_ECUDA;
+  unsigned long long base = 0;
+  size_t size = 0;
+  if (((range_fn)fn)(&base, &size, (unsigned long long)(uintptr_t)dev_ptr) != 0) return GF_ECUDA;
+  cudaIpcMemHandle_t h;
+  static_assert(sizeof(h) == 64, "cudaIpcMemHandle_t is 64 bytes");
+  if (cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base) != cudaSuccess) { cudaGetLastError(); return GF_ECUDA; }
+  memcpy(handle64, &h, 64);
+  *offset = (size_t)((uintptr_t)dev_ptr - (uintptr_t)base);
+  return GF_OK;
+}
+
+int gf_ipc_open(const unsigned char* handle64, size_t offset, void** dev_ptr) {
+  if (!handle64 || !dev_ptr) return GF_EINVAL;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle64, 64);
+  void* base = nullptr;
+  if (cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return GF_ECUDA; }
+  *dev_ptr = (char*)base + offset;
+  return GF_OK;
+}
+
+int gf_ipc_close(void* dev_ptr, size_t offset) {
+  if (!dev_ptr) return GF_EINVAL;
+  if (cudaIpcCloseMemHandle((char*)dev_ptr - offset) != cudaSuccess) { cudaGetLastError(); return GF_ECUDA; }
+  return GF_OK;
+}
+
+// ---- the driver's decisions, for callers that run Algorithm 1 over several contexts (slabs) -------------------------------
+int gf_combine_slabs(const double* F_slab, const double* theta_slab, int n_slabs, double* F, double* theta) {
+  if (!F_slab || !theta_slab || !F || !theta || n_slabs < 1) return GF_EINVAL;
+  double f = 0.0, t = 0.0;
+  for (int s = 0; s < n_slabs; ++s) {  // slab order: every rank adds the same numbers in the same order
+    f += F_slab[s];
+    t += theta_slab[s];
+  }
+  *F = f / n_slabs;  // slabs have equal volumes: the global normalisation d Nc V is n_slabs times a slab's
+  *theta = t / n_slabs;
+  return (std::isfinite(*F) && std::isfinite(*theta)) ? GF_OK : GF_ENUMERIC;
+}
+
+int gf_fix_plan(double omega, double eps, int max_sweeps, int check_every, int sweeps_done, double theta, int* n_next) {
+  if (!n_next) return GF_EINVAL;
+  *n_next = 0;
+  if (check_every < 1 || max_sweeps < 0 || sweeps_done < 0 || !(eps >= 0.0)) return GF_EINVAL;
+  if (!(omega >= 1.0 && omega < 2.0)) return GF_EINVAL;
+  if (theta < eps || sweeps_done >= max_sweeps) return GF_OK;  // Algorithm 1 l.2: stop
+  *n_next = check_every < max_sweeps - sweeps_done ? check_every : max_sweeps - sweeps_done;
   return GF_OK;
 }
 
@@ -861,7 +940,9 @@ int gf_slab_unpack_top(gf_ctx* c, int parity) {
   DeviceGuard gf_device_guard_(c);
   int rc = slab_check(c, parity, "gf_slab_unpack_top: parity must be 0 or 1");
   if (rc != GF_OK) return rc;
-  cudaError_t e = launch_slab_top(c->k, parity, c->top_in, false);
+  // with peer targets the odd half-sweep's "ret" message arrived in the top_out slot (top_in is double-buffered, so that
+  // one cross-rank synchronisation per half-sweep is enough); unpack_top(1 - p) follows half-sweep p
+  cudaError_t e = launch_slab_top(c->k, parity, (c->alt_top_in && parity == 0) ? c->top_out : c->top_in, false);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_unpack_top");
   c->launches += 1;
   c->qblocks = 0;
@@ -876,7 +957,8 @@ int gf_slab_halfsweep_border(gf_ctx* c, int parity, double omega) {
   const Geo& g = c->k.geo;
   // one launch: bottom slice, top slice; the top-slice sites also write their updated U_t(x) into top_out
   cudaError_t e = launch_halfsweep_slab(c->k, parity, omega, 0, g.s3, g.vh - g.s3, g.vh,
-                                        c->fwd_target[parity] ? c->fwd_target[parity] : c->top_out, c->ret_target);
+                                        c->fwd_target[parity] ? c->fwd_target[parity] : c->top_out,
+                                        parity ? c->ret_target_odd : c->ret_target);
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_halfsweep_border");
   c->launches += 1;
   c->qblocks = 0;

@@ -5,10 +5,17 @@ libgf context with a halo workspace attached; all arithmetic (border / interior 
 the top-slice temporal links, F and theta) runs in libgf's kernels.  This module is the plumbing between them: which
 buffer goes to which neighbour and when, on which stream, over which transport
 
-  * slabs owned by the same process: device-to-device copies,
-  * slabs owned by different processes (one process per GPU): torch.distributed send / recv (NCCL on GPUs),
+  * direct delivery (default on GPUs): the border kernel of a slab stores its two halo messages straight into the
+    neighbours' workspaces - plain pointers for slabs of the same process (gf_slab_set_targets), CUDA-IPC mappings of the
+    other ranks' workspaces between processes on one node (gf_ipc_export / gf_ipc_open, gf_slab_set_peer_targets), i.e.
+    stores over NVLink from inside the update kernel; what is left per half-sweep is one ordering point between ranks
+    (a one-element all-reduce queued on the streams with NCCL; stream synchronisation + barrier with gloo),
+  * transport (direct=False, or where the mappings cannot be made): device-to-device copies between slabs of one
+    process, torch.distributed send / recv between ranks,
 
-and the driver loop of Algorithm 1 around it (the one data-path collective: an all-gather of each slab's F and theta).
+and the driver loop of Algorithm 1 around it, whose decisions (stop test, sweeps to the next measurement, the global
+F and theta from the slabs' values) are taken by libgf (gf_fix_plan, gf_combine_slabs); the one data-path collective is
+an all-gather of each slab's F and theta.
 
 Per half-sweep of parity p (include/gf.h steps 1-4), for every local slab s with lower neighbour s-1 and upper s+1:
     border(p)    -> ghost[1-p] updated in place, top_out = top-slice U_t of the parity-p sites
@@ -53,6 +60,12 @@ class GpuSlabEngine:
         """Device tensors of the neighbours' halo workspaces the border kernel stores into (None x 3: back to top_out)."""
         ptr = [t.data_ptr() if t is not None else 0 for t in (upper_ghost0, upper_ghost1, lower_top_in)]
         self.fx._check(_b.gf_slab_set_targets(self.fx.ctx, *ptr))
+
+    def set_peer_targets(self, upper_base: int, lower_base: int):
+        """Device addresses of the upper and lower neighbours' halo workspaces (own process or CUDA-IPC mappings)."""
+        B = self.halo_bytes
+        self.fx._check(_b.gf_slab_set_peer_targets(self.fx.ctx, upper_base, upper_base + B, lower_base + 3 * B,
+                                                   lower_base + 2 * B))
 
     def pack_top(self, parity):
         self.fx._check(_b.gf_slab_pack_top(self.fx.ctx, int(parity)))
@@ -125,10 +138,12 @@ class ShardedGaugeFixer:
     dims: the GLOBAL lattice (nx, ny, nz, nt).  With torch.distributed initialised every rank constructs the same object
     and owns n_slabs / world_size consecutive slabs; without it (or with group=False) all slabs live in this process.
     engine_factory(local_dims, slab_index) builds one slab (default: GpuSlabEngine on `device`).
-    direct: the border kernels store the halo messages straight into the neighbours' buffers (gf_slab_set_targets)
-    instead of handing them to the transport; possible when every neighbour's halo workspace is addressable from the
-    slab's device, i.e. today when all slabs live in this process (default then).  Between processes the buffers would
-    have to be mapped with CUDA IPC first; that is not built, the transport path is used.
+    direct: the border kernels store the halo messages straight into the neighbours' buffers instead of handing them to
+    the transport.  None (default): yes wherever the slabs are libgf contexts on GPUs - within one process by plain
+    pointers, between the processes of one node through CUDA-IPC mappings of the neighbours' workspaces ("ipc"; if the
+    mappings cannot be made, e.g. the allocator uses virtual-memory segments, a warning is issued and the transport is
+    used).  False: always the transport.  (device=None with an engine_factory is the seam tests/_slab_oracle.py uses to
+    drive this schedule with CPU slabs.)
     """
 
     def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
@@ -165,19 +180,86 @@ class ShardedGaugeFixer:
         if self.on_gpu:
             with torch.cuda.device(self.device):
                 self.comm_stream = torch.cuda.Stream(self.device)
-        can_direct = self.world == 1 and self.on_gpu and all(hasattr(e, "set_targets") for e in self.engines.values())
-        if direct and not can_direct:
-            raise ValueError("direct delivery needs all slabs in this process, on GPUs")
-        self.direct = can_direct if direct is None else bool(direct)
+        gpu_slabs = self.on_gpu and all(hasattr(e, "set_targets") for e in self.engines.values())
+        can_direct = self.world == 1 and gpu_slabs
+        if direct and not gpu_slabs:
+            raise ValueError("direct delivery needs libgf slabs on GPUs")
+        self.direct = can_direct if direct is None else (bool(direct) and self.world == 1)
+        self.ipc = False
+        self._ipc_mapped = {}
         if self.direct:
             for s, e in self.engines.items():
                 up, lo = self.engines[(s + 1) % self.n_slabs], self.engines[(s - 1) % self.n_slabs]
                 e.set_targets(up.ghost[0], up.ghost[1], lo.top_in)
+        elif self.world > 1 and gpu_slabs and direct is not False:
+            self.ipc = self._map_neighbours()
+            if not self.ipc:
+                import warnings
+
+                warnings.warn("ShardedGaugeFixer: CUDA IPC mapping of the neighbours' halo workspaces failed; halo messages "
+                              "go through torch.distributed send/recv")
         self._after_unpack = {}
         self.reunit_every = 0
         self.sweeps_total = 0
         self.messages_sent = 0  # remote (torch.distributed) messages posted by this rank
         self.copies = 0         # local device-to-device copies
+
+    # ---- direct delivery between processes -----------------------------------------------------------------------------------
+    def _map_neighbours(self):
+        """Exchange CUDA-IPC handles of every slab's halo workspace, map the ones of this rank's remote neighbours and
+        give every local slab its two neighbours' addresses.  All ranks agree on the outcome."""
+        torch, dist = self.torch, self.dist
+        mine, ok = {}, True
+        for s, e in self.engines.items():
+            rc, handle, off = _b.gf_ipc_export(e.halo.data_ptr())
+            ok = ok and rc == _b.GF_OK
+            mine[s] = (handle, off)
+        gathered = [None] * self.world
+        dist.all_gather_object(gathered, (ok, mine), group=self.group)
+        if not all(g[0] for g in gathered):
+            return False
+        table = {}
+        for _, d in gathered:
+            table.update(d)
+
+        def base(slab):
+            if slab in self.engines:
+                return self.engines[slab].halo.data_ptr()
+            handle, off = table[slab]
+            if handle not in self._ipc_mapped:  # several slabs of a rank may sit in one allocation: map it once
+                with torch.cuda.device(self.device):
+                    rc, ptr = _b.gf_ipc_open(handle, 0)
+                self._ipc_mapped[handle] = ptr if rc == _b.GF_OK else None
+            return None if self._ipc_mapped[handle] is None else self._ipc_mapped[handle] + off
+
+        bases = {s: (base((s + 1) % self.n_slabs), base((s - 1) % self.n_slabs)) for s in self.slabs}
+        good = all(u is not None and l is not None for u, l in bases.values())
+        flags = [None] * self.world
+        dist.all_gather_object(flags, good, group=self.group)
+        if not all(flags):
+            return False
+        for s, (u, l) in bases.items():
+            self.engines[s].set_peer_targets(u, l)
+        self._token = torch.zeros(1, dtype=torch.float32, device=self.device)
+        return True
+
+    def _rank_sync(self):
+        """One ordering point between all ranks' streams: what every rank queued before it is complete before anything
+        queued after it starts.  NCCL: a one-element all-reduce on the transport stream between the compute streams (no
+        host wait); other backends: stream synchronisation and a barrier."""
+        torch, dist = self.torch, self.dist
+        if dist.get_backend(self.group) == "nccl":
+            for s in self.slabs:
+                self.comm_stream.wait_event(self.engines[s].mark())
+            with torch.cuda.stream(self.comm_stream):
+                dist.all_reduce(self._token, group=self.group)
+            done = torch.cuda.Event()
+            done.record(self.comm_stream)
+            for s in self.slabs:
+                self.engines[s].wait(done)
+        else:
+            self.synchronize()
+            dist.barrier(group=self.group)
 
     # ---- transport ------------------------------------------------------------------------------------------------------
     def _buffer(self, kind, end, slab, p):
@@ -238,13 +320,17 @@ class ShardedGaugeFixer:
         """Fill both ghost buffers of every slab from its lower neighbour's top slice (after set_links, reunitarize)."""
         if self.direct:  # pack_top writes into the upper neighbour's ghost buffer: wait for whatever it still runs
             self._join_neighbours({s: self.engines[s].mark() for s in self.slabs})
+        if self.ipc:
+            self._rank_sync()
         for q in (0, 1):
             for s in self.slabs:
                 self.engines[s].pack_top(q)
             if self.direct:
                 self._join_neighbours({s: self.engines[s].mark() for s in self.slabs})
-            else:
+            elif not self.ipc:
                 self._exchange(q, kinds=("fwd",))
+        if self.ipc:
+            self._rank_sync()
 
     # ---- links in / out ---------------------------------------------------------------------------------------------------
     def set_links(self, links_by_slab):
@@ -278,6 +364,18 @@ class ShardedGaugeFixer:
                 self.engines[s].unpack_top(1 - p)
             self._after_unpack = {s: self.engines[s].mark() for s in self.slabs}
             return
+        if self.ipc:
+            # Between processes: the border kernels store both messages in the neighbours' mapped workspaces (top_in is
+            # double-buffered by parity, gf_slab_set_peer_targets), then ONE ordering point between the ranks; the next
+            # border kernel only writes buffers whose last readers ran before it.
+            for s in self.slabs:
+                self.engines[s].border(p, omega)
+            self._rank_sync()
+            for s in self.slabs:
+                self.engines[s].interior(p, omega)
+            for s in self.slabs:
+                self.engines[s].unpack_top(1 - p)
+            return
         for s in self.slabs:
             self.engines[s].border(p, omega)
         # the transport starts as soon as the border kernels are done, beside the interior kernels queued behind them
@@ -298,8 +396,8 @@ class ShardedGaugeFixer:
 
     def ovr_sweep(self, n, omega):
         """n sweeps, even half-sweep first; reunitarisation cadence as gf_ovr_sweep."""
-        if not (1.0 <= omega < 2.0):
-            raise ValueError("omega outside [1,2)")
+        if _b.gf_fix_plan(float(omega), 0.0, int(n), 1, 0, 1.0)[0] != _b.GF_OK:
+            raise ValueError("omega outside [1,2) or n < 0")
         for _ in range(int(n)):
             self.half_sweep(0, omega)
             self.half_sweep(1, omega)
@@ -318,21 +416,28 @@ class ShardedGaugeFixer:
             parts = [torch.empty_like(buf) for _ in range(self.world)]
             self.dist.all_gather(parts, buf, group=self.group)
             local = torch.cat(parts).cpu()
-        F = theta = 0.0
-        for row in local.tolist():
-            F += row[0]
-            theta += row[1]
-        return F / self.n_slabs, theta / self.n_slabs
+        rows = local.tolist()
+        rc, F, theta = _b.gf_combine_slabs([r[0] for r in rows], [r[1] for r in rows])
+        if rc != _b.GF_OK:
+            raise _b.GFError(rc, "global F / theta from the slabs' values")
+        return F, theta
 
     def fix(self, omega, eps, max_sweeps, check_every):
         """Algorithm 1 with a measurement cadence (as gf_fix).  Returns (sweeps_done, [(sweep, F, theta), ...])."""
-        if check_every < 1 or max_sweeps < 0 or not eps >= 0.0:
-            raise ValueError("need check_every >= 1, max_sweeps >= 0, eps >= 0")
+        def plan(done, theta):  # Algorithm 1 l.2 and the cadence: decided by libgf, as in gf_fix
+            rc, n = _b.gf_fix_plan(float(omega), float(eps), int(max_sweeps), int(check_every), done, theta)
+            if rc != _b.GF_OK:
+                raise ValueError("need omega in [1,2), check_every >= 1, max_sweeps >= 0, eps >= 0")
+            return n
+
+        plan(0, 1.0)
         done = 0
         F, th = self.measure()
         history = [(0, F, th)]
-        while not th < eps and done < max_sweeps:
-            n = min(check_every, max_sweeps - done)
+        while True:
+            n = plan(done, th)
+            if n == 0:
+                break
             self.ovr_sweep(n, omega)
             done += n
             F, th = self.measure()
@@ -349,6 +454,14 @@ class ShardedGaugeFixer:
             self.comm_stream.synchronize()
 
     def close(self):
+        if self._ipc_mapped:
+            self.synchronize()
+            if self.dist is not None:
+                self.dist.barrier(group=self.group)  # no rank unmaps while a neighbour's kernels may still store into it
+            for ptr in self._ipc_mapped.values():
+                if ptr:
+                    _b.gf_ipc_close(ptr, 0)
+            self._ipc_mapped = {}
         for e in self.engines.values():
             e.close()
         self.engines = {}

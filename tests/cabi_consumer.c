@@ -22,7 +22,8 @@ int main(void) {
   bytes = gf_workspace_bytes(8, 8, 8, 8, GF_FP64, 18);
   CHECK(bytes >= (size_t)4 * 4096 * 144);
   CHECK(gf_workspace_bytes(7, 8, 8, 8, GF_FP64, 18) == 0); /* odd extent */
-  CHECK(gf_workspace_bytes(8, 8, 8, 8, GF_FP32, 8) == 0);  /* 8-real storage is FP64 only */
+  CHECK(gf_workspace_bytes(8, 8, 8, 8, GF_FP32, 10) == 0); /* storage must be 18, 12 or 8 */
+  CHECK(gf_workspace_bytes_sun(5, 8, 8, 8, 8, GF_FP64) == 0 && gf_workspace_bytes_sun(4, 8, 8, 8, 8, GF_FP64) > 0);
 
   CHECK(gf_create(NULL, 8, 8, 8, 8, GF_LANDAU, GF_FP64, 18, NULL, 0, NULL) == GF_EINVAL);
   CHECK(gf_create(&ctx, 8, 8, 8, 9, GF_LANDAU, GF_FP64, 18, NULL, 0, NULL) == GF_EODD && ctx == NULL);
@@ -36,6 +37,13 @@ int main(void) {
   CHECK(gf_fix(NULL, 1.7, 1e-12, 10, 1, &done) == GF_EINVAL);
   CHECK(gf_reunitarize(NULL) == GF_EINVAL);
   CHECK(gf_peak_fma(GF_FP64, 0.0, NULL, NULL, &tflops) == GF_EINVAL);
+  CHECK(gf_fix_plan(1.7, 1e-12, 100, 10, 95, 1.0, &done) == GF_OK && done == 5);
+  CHECK(gf_fix_plan(1.7, 1e-12, 100, 10, 40, 1e-13, &done) == GF_OK && done == 0);
+  CHECK(gf_fix_plan(2.0, 1e-12, 100, 10, 0, 1.0, &done) == GF_EINVAL);
+  {
+    const double Fs[2] = {0.25, 0.75}, ts[2] = {2.0, 4.0};
+    CHECK(gf_combine_slabs(Fs, ts, 2, &F, &theta) == GF_OK && F == 0.5 && theta == 3.0);
+  }
   CHECK(gf_kernel_launches(NULL) == 0);
   CHECK(strcmp(gf_strerror(GF_OK), "ok") == 0);
   CHECK(strlen(gf_strerror(GF_EODD)) > 0 && strlen(gf_last_error(NULL)) == 0);

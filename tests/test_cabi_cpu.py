@@ -28,7 +28,7 @@ def test_workspace_bytes():
         assert 4 * V * L + (128 << 20) <= n <= 4 * V * L + (128 << 20) + (8 << 20)
     assert gf.gf_workspace_bytes(7, 8, 8, 8, 0, 18) == 0
     assert gf.gf_workspace_bytes(8, 8, 8, 8, 0, 10) == 0
-    assert gf.gf_workspace_bytes(8, 8, 8, 8, 1, 8) == 0  # 8-real storage is FP64 only
+    assert 0 < gf.gf_workspace_bytes(8, 8, 8, 8, 1, 8) < gf.gf_workspace_bytes(8, 8, 8, 8, 1, 12)  # 8-real, FP32
     assert 0 < gf.gf_workspace_bytes(8, 8, 8, 8, 0, 8) < gf.gf_workspace_bytes(8, 8, 8, 8, 0, 12)
     assert gf.gf_workspace_bytes(8, 8, 8, 8, 2, 18) == 0
 
@@ -40,7 +40,7 @@ def test_create_rejects_bad_arguments_before_touching_the_device():
     assert gf.gf_create(8, 8, 8, 8, 2, 0, 18, 256, big, 0)[0] == gf.GF_EUNSUPPORTED
     assert gf.gf_create(8, 8, 8, 8, 0, 3, 18, 256, big, 0)[0] == gf.GF_EUNSUPPORTED
     assert gf.gf_create(8, 8, 8, 8, 0, 0, 10, 256, big, 0)[0] == gf.GF_EUNSUPPORTED  # storage must be 18, 12 or 8
-    assert gf.gf_create(8, 8, 8, 8, 0, 1, 8, 256, big, 0)[0] == gf.GF_EUNSUPPORTED   # 8-real storage is FP64 only
+    assert gf.gf_create(8, 8, 8, 8, 0, 1, 9, 256, big, 0)[0] == gf.GF_EUNSUPPORTED   # storage must be 18, 12 or 8
     assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 0, big, 0)[0] == gf.GF_EINVAL
     assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 256, 1024, 0)[0] == gf.GF_ENOMEM
     assert gf.gf_create(8, 8, 8, 8, 0, 0, 18, 264, big, 0)[0] == gf.GF_ENOMEM        # misaligned
