@@ -78,7 +78,8 @@ def halfsweep_kernel_name(storage, variant, defer=False):
     v = variant or 3
     return {1: "ovr_halfsweep_kernel", 2: "ovr_halfsweep_kernel (L2 bulk prefetch)", 3: "ovr_halfsweep_staged_kernel",
             4: "ovr_halfsweep_staged_kernel<BULK=1> (TMA bulk copies)",
-            5: "ovr_halfsweep_staged_kernel<BULK=2> (forward chunk by TMA bulk copy)"}[v] + (" (deferred temporal links)" if defer else "")
+            5: "ovr_halfsweep_staged_kernel<BULK=2> (forward chunk by TMA bulk copy)",
+            6: "ovr_halfsweep_pair8_kernel (two lanes per site)"}[v] + (" (deferred temporal links)" if defer else "")
 
 
 def measure_fp_peaks(seconds=0.25):

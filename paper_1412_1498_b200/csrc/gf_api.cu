@@ -412,7 +412,7 @@ int gf_set_option(gf_ctx* c, int key, int value) {
   if (is_sun(c)) return fail(c, GF_EUNSUPPORTED, "gf_set_option: no options on an SU(N != 3) context");
   switch (key) {
     case GF_OPT_SWEEP_VARIANT:
-      if (value < 0 || value > 5) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
+      if (value < 0 || value > 6) return fail(c, GF_EINVAL, "gf_set_option: bad variant");
       c->k.variant = value;
       return GF_OK;
     case GF_OPT_FUSE_MEASURE:

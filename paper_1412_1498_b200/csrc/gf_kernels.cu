@@ -247,6 +247,37 @@ ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) 
   }
 }
 
+// An 8-real store needs five of the nine elements of a product: a1, a2, a3 (row 0), b1 and c1 (column 0).
+template <class C>
+__device__ __forceinline__ void mul_left_8(const C (&G)[9], const C (&u)[9], C (&w)[9]) {
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {  // row 0 of G.U
+    C z = cmul(G[0], u[j]); cfma(z, G[1], u[3 + j]); cfma(z, G[2], u[6 + j]);
+    w[j] = z;
+  }
+#pragma unroll
+  for (int i = 1; i < 3; ++i) {  // column 0 of rows 1, 2
+    C z = cmul(G[i * 3], u[0]); cfma(z, G[i * 3 + 1], u[3]); cfma(z, G[i * 3 + 2], u[6]);
+    w[i * 3] = z;
+  }
+}
+template <class C>
+__device__ __forceinline__ void mul_right_adj_8(const C (&u)[9], const C (&G)[9], C (&w)[9]) {
+  using T = decltype(w[0].x);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {  // row 0 of U.G^dagger
+    C z = mk<T>(T(0), T(0));
+    cfma_cj(z, u[0], G[j * 3]); cfma_cj(z, u[1], G[j * 3 + 1]); cfma_cj(z, u[2], G[j * 3 + 2]);
+    w[j] = z;
+  }
+#pragma unroll
+  for (int i = 1; i < 3; ++i) {  // column 0 of rows 1, 2
+    C z = mk<T>(T(0), T(0));
+    cfma_cj(z, u[i * 3], G[0]); cfma_cj(z, u[i * 3 + 1], G[1]); cfma_cj(z, u[i * 3 + 2], G[2]);
+    w[i * 3] = z;
+  }
+}
+
 // ---- staged through shared memory with cp.async ---------------------------------------------------------
 template <class T> constexpr int staged_threads() { return sizeof(T) == 8 ? 64 : 128; }
 // FP32 storage: 4 blocks of 128 threads per SM (shared memory allows 4), i.e. at most 128 registers for the FP64 rotation
@@ -425,13 +456,17 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       }
       cp_async_wait_all();  // a thread reads only what it copied itself: no block barrier needed
       if constexpr (NELEM == 4) {
+        // two links at a time: their reconstructions are independent dependent chains (division, square roots), and a
+        // thread has only its own instruction-level parallelism to hide them (8 warps per SM)
 #pragma unroll
-        for (int l = 0; l < 8; ++l) {
+        for (int l = 0; l < 8; l += 2) {
           C* s8 = sm + l * SELEM * STRIDE;
-          C u[9];
+          C* t8 = s8 + SELEM * STRIDE;
+          C u[9], v[9];
           decode8<T, C, false>(s8[2 * STRIDE], s8[3 * STRIDE], s8[4 * STRIDE], s8[5 * STRIDE], u);
+          decode8<T, C, false>(t8[2 * STRIDE], t8[3 * STRIDE], t8[4 * STRIDE], t8[5 * STRIDE], v);
 #pragma unroll
-          for (int e = 0; e < 6; ++e) s8[e * STRIDE] = u[e];
+          for (int e = 0; e < 6; ++e) { s8[e * STRIDE] = u[e]; t8[e * STRIDE] = v[e]; }
           sched_fence();
         }
       }
@@ -492,16 +527,18 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     for (int mu = 0; mu < NMU; ++mu) {
       C u[9], w[9];
       load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
-      mul_left<LinkRows<NELEM>::value>(G, u, w);                       // U_mu(x) <- G U_mu(x)
+      if constexpr (NELEM == 4) mul_left_8(G, u, w);                   // (the five elements an 8-real store needs)
+      else mul_left<LinkRows<NELEM>::value>(G, u, w);                  // U_mu(x) <- G U_mu(x)
       store_link<NELEM>(fwd + mu * NELEM * 32, w);
       if (SLAB && mu == 3 && sv.top_out && cb >= g.vh - g.s3) {  // top slice: the copy that goes to the upper neighbour
         SlabView out = sv;
         out.ghost = sv.top_out;
         store_link<NELEM>(ghost_link<T, NELEM, C>(out, 0, cb - (g.vh - g.s3)), w);
       }
-      sched_fence();
+      if (NELEM != 4) sched_fence();  // (8-real: the two encodings of a direction overlap)
       load_link_smem<SELEM, STRIDE, NELEM == 4>(sm, slot_bwd(mu), u);  // (an 8-real store needs c1: all three rows)
-      mul_right_adj<LinkRows<NELEM>::value>(u, G, w);                  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+      if constexpr (NELEM == 4) mul_right_adj_8(u, G, w);
+      else mul_right_adj<LinkRows<NELEM>::value>(u, G, w);             // U_mu(x-mu) <- U_mu(x-mu) G^dagger
       store_link<NELEM>(bwd[mu], w);
       if (SLAB && mu == 3 && sv.ret_out && cb < g.s3) {   // bottom slice: the copy that goes back to the lower neighbour
         SlabView out = sv;
@@ -533,6 +570,123 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + THREADS - 1) / THREADS);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials, SlabView{}, 0, nullptr, nullptr);
+  return cudaGetLastError();
+}
+
+
+// ---- 8-real storage, two lanes per site (GF_OPT_SWEEP_VARIANT 6) ------------------------------------------------------------
+// With one thread per site the 8-real kernel is bound by the dependent-issue latency of 8 warps per SM (shared memory
+// sets the occupancy; profiles/r2_8real_cfg3_ncu.txt).  Here two WARPS share 32 sites (a lane pair inside one warp would
+// diverge at every step - measured: slower than one thread per site): warp 2k (h = 0) owns the four forward links of its
+// 32 sites, warp 2k+1 (h = 1) the four backward links.  Each lane copies, decodes (once, in place, into rows 0 and 1) and
+// later updates its own four links; the two partial sums of K(x) are exchanged through shared memory (K = own + other:
+// the same bits in both lanes, addition being commutative), and both lanes run the three SU(2) steps.  About 0.6 of the
+// instructions per lane and twice the lanes per site.
+template <class T> struct PairSites { static constexpr int value = sizeof(T) == 8 ? 64 : 128; };
+
+template <class T, int ND, bool MEASURE>
+__global__ void __launch_bounds__(2 * PairSites<T>::value, sizeof(T) == 8 ? 3 : 2)
+ovr_halfsweep_pair8_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
+  using C = cplx_t<T>;
+  using CK = cplx_t<RotationType>;
+  constexpr int SITES = PairSites<T>::value;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, h = warp & 1;
+  const int i = (warp >> 1) * 32 + (threadIdx.x & 31);
+  // slot of (link l, element e) of site i: [l][e][SITES]; this lane's links are l = 4 h + mu
+  C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)(4 * h) * 6 * SITES + i;
+  // exchange area behind the link slots: [h][real 0..17][SITES] doubles
+  double* xch = reinterpret_cast<double*>(smem_raw + (size_t)8 * 6 * SITES * sizeof(C));
+  const int cb = blockIdx.x * SITES + i;
+  const bool live = cb < g.vh;
+  const Site s = site_of(g, parity, live ? cb : 0);
+  // this lane's link in direction mu: U_mu(x) (h = 0) or U_mu(x - mu) (h = 1)
+  auto link_ptr = [&](int mu) -> C* {
+    return h == 0 ? links + link_offset<4>(g, parity, cb, mu) : links + link_offset<4>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
+  };
+  CK K[9];
+#pragma unroll
+  for (int e = 0; e < 9; ++e) K[e] = make_double2(0.0, 0.0);
+  // The loops over the lane's four links are NOT unrolled: the fully unrolled one-thread-per-site kernels are
+  // 90-115 KB of straight-line code that every warp streams through once, and with a dozen warps per SM at different
+  // places in it the instruction caches miss ("no instruction" stalls, profiles/r2_8real_cfg3_ncu.txt).
+  if (live) {
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+      const C* p = link_ptr(mu);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) cp_async<sizeof(C)>(sm + (mu * 6 + 2 + e) * SITES, p + e * 32);
+    }
+    cp_async_wait_all();  // a lane reads only what it copied itself
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu += 2) {  // two reconstructions at a time (independent dependent chains)
+      C* s8 = sm + mu * 6 * SITES;
+      C* t8 = s8 + 6 * SITES;
+      C u[9], v[9];
+      decode8<T, C, false>(s8[2 * SITES], s8[3 * SITES], s8[4 * SITES], s8[5 * SITES], u);
+      decode8<T, C, false>(t8[2 * SITES], t8[3 * SITES], t8[4 * SITES], t8[5 * SITES], v);
+#pragma unroll
+      for (int e = 0; e < 6; ++e) { s8[e * SITES] = u[e]; t8[e * SITES] = v[e]; }
+    }
+    // this lane's half of K(x) = sum_{mu<ND} [U_mu(x) + U_mu(x-mu)^dagger]   (eq. 1.5), FP64 in both precisions
+#pragma unroll 1
+    for (int mu = 0; mu < ND; ++mu) {
+      C u[9];
+      load_link<6, true, SITES>(sm + mu * 6 * SITES, u);
+      if (h == 0) {
+#pragma unroll
+        for (int e = 0; e < 9; ++e) { K[e].x += (double)u[e].x; K[e].y += (double)u[e].y; }
+      } else {
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) { K[r * 3 + c].x += (double)u[c * 3 + r].x; K[r * 3 + c].y -= (double)u[c * 3 + r].y; }
+      }
+    }
+  }
+  // the partner warp's half (every thread of the block reaches the barrier)
+#pragma unroll
+  for (int e = 0; e < 9; ++e) {
+    xch[(h * 18 + 2 * e) * SITES + i] = K[e].x;
+    xch[(h * 18 + 2 * e + 1) * SITES + i] = K[e].y;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int e = 0; e < 9; ++e) {
+    K[e].x += xch[((1 - h) * 18 + 2 * e) * SITES + i];
+    K[e].y += xch[((1 - h) * 18 + 2 * e + 1) * SITES + i];
+  }
+  double q = 0.0;
+  if (live) {
+    C G[9];
+    site_gauge_rotation<RotationType, MEASURE, false>(K, G, (RotationType)omega, 0);
+    if (MEASURE && h == 0) q = (double)delta_norm2<RotationType>(K);
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+      C u[9], w[9];
+      load_link<6, true, SITES>(sm + mu * 6 * SITES, u);
+      if (h == 0) mul_left_8(G, u, w);        // U_mu(x) <- G U_mu(x)
+      else mul_right_adj_8(u, G, w);          // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+      store_link<4>(link_ptr(mu), w);
+    }
+  }
+  if (MEASURE) {
+    double f = 0.0;
+    block_sum2<2 * SITES>(f, q);
+    if (threadIdx.x == 0) qpartials[blockIdx.x] = q;
+  }
+}
+
+template <class T, int ND, bool MEASURE>
+static cudaError_t halfsweep_pair8_T(const KernelArgs& a, int parity, double omega) {
+  using C = cplx_t<T>;
+  constexpr int SITES = PairSites<T>::value;
+  constexpr size_t SMEM = (size_t)8 * 6 * SITES * sizeof(C) + (size_t)2 * 18 * SITES * sizeof(double);
+  auto kern = ovr_halfsweep_pair8_kernel<T, ND, MEASURE>;
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
+  const unsigned blocks = (unsigned)((a.geo.vh + SITES - 1) / SITES);
+  kern<<<blocks, 2 * SITES, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, (double*)a.qpartials);
   return cudaGetLastError();
 }
 
@@ -590,7 +744,20 @@ template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
   using C = cplx_t<T>;
   *qblocks = 0;
+  // 8-real storage: variant 6 = two warps per 32 sites (measured: no faster than one thread per site)
   const int variant = a.variant;
+  if (variant == 6) {
+    if constexpr (NELEM == 4) {
+      if (a.series > 0 || a.block_threads) return cudaErrorNotSupported;
+      if (fuse_theta) {
+        *qblocks = (a.geo.vh + PairSites<T>::value - 1) / PairSites<T>::value;
+        return halfsweep_pair8_T<T, ND, true>(a, parity, omega);
+      }
+      return halfsweep_pair8_T<T, ND, false>(a, parity, omega);
+    } else {
+      return cudaErrorNotSupported;
+    }
+  }
   if (variant == 0 || variant == 3 || variant == 4 || variant == 5) {
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM
     constexpr int THREADS = staged_threads<T>();
@@ -782,7 +949,7 @@ cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pac
 }
 
 bool halfsweep_can_fuse_theta(const KernelArgs& a) {
-  return (a.variant == 0 || a.variant == 3 || a.variant == 4 || a.variant == 5) && a.series == 0;
+  return (a.variant == 0 || a.variant == 3 || a.variant == 4 || a.variant == 5 || a.variant == 6) && a.series == 0;
 }
 int halfsweep_max_qblocks(const Geo& g) { return (g.vh + 31) / 32; }
 
