@@ -43,7 +43,7 @@ class GpuSlabEngine:
         self.stream = self.fx.stream
         B = _b.gf_slab_halo_bytes(self.fx.ctx)
         self.halo_bytes = B
-        with torch.cuda.device(self.device):
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):  # tied to the stream its kernels run on
             self.halo = torch.zeros(4 * B, dtype=torch.uint8, device=self.device)
         self.fx._check(_b.gf_slab_attach(self.fx.ctx, self.halo.data_ptr(), 4 * B))
         self.ghost = [self.halo[0:B], self.halo[B:2 * B]]
@@ -142,8 +142,8 @@ class ShardedGaugeFixer:
     the transport.  None (default): yes wherever the slabs are libgf contexts on GPUs - within one process by plain
     pointers, between the processes of one node through CUDA-IPC mappings of the neighbours' workspaces ("ipc"; if the
     mappings cannot be made, e.g. the allocator uses virtual-memory segments, a warning is issued and the transport is
-    used).  False: always the transport.  (device=None with an engine_factory is the seam tests/_slab_oracle.py uses to
-    drive this schedule with CPU slabs.)
+    used).  False: always the transport.  (device=None with an engine_factory is the seam the CPU schedule test uses to
+    drive this schedule with host-side slabs.)
     """
 
     def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
