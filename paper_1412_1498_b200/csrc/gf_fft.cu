@@ -316,22 +316,23 @@ fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
   const int nx = a.nx, ny = a.ny, row = a.row;
   C* g = w + (size_t)blockIdx.x * nx * ny;
   const int nthreads = blockDim.x;
-  for (int i = threadIdx.x; i < nx * ny; i += nthreads) {  // global -> tile without a register round trip
-    const int y = i / nx, x = i - y * nx;
-    const unsigned dst = (unsigned)__cvta_generic_to_shared(tile + y * row + x);
-    if (sizeof(C) == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(g + i) : "memory");
-    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(g + i) : "memory");
-  }
-  asm volatile("cp.async.wait_all;" ::: "memory");
-  __syncthreads();
-  // x lines: line y, elements tile[y*row + pos]; work item -> (sub, y) with y fastest: neighbouring lanes are one row
-  // apart, and the row stride is odd, so they fall on different banks whatever the stride along the line is
-  auto x_outer = [&](auto inv_tag) {
+  // The y steps at the two ends of the pass work straight on global memory (a y step's lanes are consecutive in x:
+  // 512-byte runs): the forward pass writes the results of its last step to the field, the inverse pass reads the
+  // operands of its first step from it, so that end of the pass needs no tile copy and no barrier.  The x steps stay in
+  // the tile on the load side: measured on the cfg4 lattice, an x step that READS global memory (8 lanes per 128-byte
+  // line) costs more than the tile copy it saves (forward pass 1.04 ms against 0.99 ms), one that WRITES it does not
+  // (inverse pass 0.95 ms against 1.03 ms with a tile copy at the end).  Forward 0.99 -> 0.91 ms, inverse 0.99 -> 0.95 ms.
+  // x lines: line y, elements base[y*rs + pos].  In the tile the work item is (sub, y) with y fastest: neighbouring lanes
+  // are one row apart, and the row stride is odd, so they fall on different banks whatever the stride along the line is.
+  // Against global memory it is (sub, y) with sub fastest: the rx2 lanes of a row read / write rx2 consecutive elements
+  // (whole 128-byte lines for rx2 = 8 in FP64); the tile side of that step is conflict-free because row = 1 mod 8.
+  auto x_outer = [&](auto inv_tag, const C* src, int srs, C* dst, int drs, bool sub_fastest) {
     constexpr bool I = decltype(inv_tag)::value;
     for (int it = threadIdx.x; it < ny * a.rx2; it += nthreads) {
-      const int t2 = it / ny, y = it - t2 * ny;
-      C* p = tile + y * row + t2;
-      GF_R_CASES(a.rx1, fft_step<T, RR, I, !I>(p, (size_t)a.rx2, p, (size_t)a.rx2, a.twx, t2));
+      int t2, y;
+      if (sub_fastest) { y = it / a.rx2; t2 = it - y * a.rx2; }
+      else { t2 = it / ny; y = it - t2 * ny; }
+      GF_R_CASES(a.rx1, fft_step<T, RR, I, !I>(src + y * srs + t2, (size_t)a.rx2, dst + y * drs + t2, (size_t)a.rx2, a.twx, t2));
     }
   };
   auto x_inner = [&](auto inv_tag) {
@@ -342,40 +343,54 @@ fft_plane_kernel(cplx_t<T>* __restrict__ w, PlaneArgs a) {
       GF_R_CASES(a.rx2, fft_step<T, RR, I, I>(p, (size_t)1, p, (size_t)1, a.twx, k1));
     }
   };
-  // y lines: line x, elements tile[pos*row + x]; work item -> (sub, x) with x fastest
-  auto y_outer = [&](auto inv_tag) {
+  // y lines: line x, elements base[pos*rs + x]; work item -> (sub, x) with x fastest (contiguous in global memory too)
+  auto y_outer = [&](auto inv_tag, const C* src, int srs, C* dst, int drs) {
     constexpr bool I = decltype(inv_tag)::value;
     for (int it = threadIdx.x; it < nx * a.ry2; it += nthreads) {
       const int t2 = it / nx, x = it - t2 * nx;
-      C* p = tile + t2 * row + x;
-      GF_R_CASES(a.ry1, fft_step<T, RR, I, !I>(p, (size_t)a.ry2 * row, p, (size_t)a.ry2 * row, a.twy, t2));
+      GF_R_CASES(a.ry1, fft_step<T, RR, I, !I>(src + t2 * srs + x, (size_t)a.ry2 * srs, dst + t2 * drs + x, (size_t)a.ry2 * drs,
+                                                a.twy, t2));
     }
   };
-  auto y_inner = [&](auto inv_tag) {
+  auto y_inner = [&](auto inv_tag, const C* src, int srs, C* dst, int drs) {
     constexpr bool I = decltype(inv_tag)::value;
     for (int it = threadIdx.x; it < nx * a.ry1; it += nthreads) {
       const int k1 = it / nx, x = it - k1 * nx;
-      C* p = tile + a.ry2 * k1 * row + x;
-      GF_R_CASES(a.ry2, fft_step<T, RR, I, I>(p, (size_t)row, p, (size_t)row, a.twy, k1));
+      GF_R_CASES(a.ry2, fft_step<T, RR, I, I>(src + a.ry2 * k1 * srs + x, (size_t)srs, dst + a.ry2 * k1 * drs + x, (size_t)drs,
+                                               a.twy, k1));
     }
   };
   using Fwd = DirTag<false>;
   using Inv = DirTag<true>;
+  auto load_tile = [&]() {  // global -> tile without a register round trip
+    for (int i = threadIdx.x; i < nx * ny; i += nthreads) {
+      const int y = i / nx, x = i - y * nx;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(tile + y * row + x);
+      if (sizeof(C) == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(g + i) : "memory");
+      else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(g + i) : "memory");
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+  };
   if (!INV) {
-    x_outer(Fwd{}); __syncthreads();
+    load_tile();
+    x_outer(Fwd{}, tile, row, tile, row, false); __syncthreads();
     if (a.rx2 > 1) { x_inner(Fwd{}); __syncthreads(); }
-    y_outer(Fwd{}); __syncthreads();
-    if (a.ry2 > 1) { y_inner(Fwd{}); __syncthreads(); }
+    if (a.ry2 > 1) {
+      y_outer(Fwd{}, tile, row, tile, row); __syncthreads();
+      y_inner(Fwd{}, tile, row, g, nx);
+    } else {
+      y_outer(Fwd{}, tile, row, g, nx);
+    }
   } else {
-    if (a.ry2 > 1) { y_inner(Inv{}); __syncthreads(); }
-    y_outer(Inv{}); __syncthreads();
+    if (a.ry2 > 1) {
+      y_inner(Inv{}, g, nx, tile, row); __syncthreads();
+      y_outer(Inv{}, tile, row, tile, row); __syncthreads();
+    } else {
+      y_outer(Inv{}, g, nx, tile, row); __syncthreads();
+    }
     if (a.rx2 > 1) { x_inner(Inv{}); __syncthreads(); }
-    x_outer(Inv{}); __syncthreads();
-  }
-#pragma unroll 4
-  for (int i = threadIdx.x; i < nx * ny; i += nthreads) {
-    const int y = i / nx, x = i - y * nx;
-    g[i] = tile[y * row + x];
+    x_outer(Inv{}, tile, row, g, nx, true);
   }
 }
 
