@@ -186,13 +186,23 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) 
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+
+// Serpentine block order: the odd half-sweep walks the lattice from the far end back, the even one (and the measure pass)
+// from the near end, so a pass starts on the links the previous pass touched last, while they are still in the 126 MB
+// L2.  A field of a few L2 sizes (config 2: 201 MB) then finds most of its links there instead of streaming through an
+// LRU cache that has just dropped them; fields far larger than L2 (configs 3, 4) are unaffected.  Which block takes
+// which sites does not change any result (same-parity updates are independent).
+__device__ __forceinline__ unsigned serpentine_block(int parity) {
+  return (parity & 1) ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+}
+
 template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool PREFETCH>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) {
   using C = cplx_t<T>;
   using TK = RotationType;  // K(x), the SU(2) steps and G(x) are always FP64 (see RotationType)
   using CK = cplx_t<TK>;
-  int cb = blockIdx.x * THREADS + threadIdx.x;
+  int cb = serpentine_block(parity) * THREADS + threadIdx.x;
   const bool live = cb < g.vh;
   if (!PREFETCH && !live) return;
   if (!live) cb = g.vh - 1;  // keep the warp converged for the shuffles below; the lane does no loads or stores
@@ -371,11 +381,12 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C* sm = BULK ? reinterpret_cast<C*>(smem_raw) + (threadIdx.x >> 5) * (8 * NELEM * 32) + (threadIdx.x & 31)
                : reinterpret_cast<C*>(smem_raw) + threadIdx.x;
-  int cb = blockIdx.x * THREADS + threadIdx.x;
+  const unsigned bid = SLAB ? blockIdx.x : serpentine_block(parity);  // (a slab launch covers two given ranges)
+  int cb = bid * THREADS + threadIdx.x;
   bool live = cb < g.vh;
   if (SLAB) {
     const bool second = (int)blockIdx.x >= sv.nblocks0;
-    cb = second ? sv.cb2_begin + (blockIdx.x - sv.nblocks0) * THREADS + threadIdx.x : sv.cb_begin + cb;
+    cb = second ? sv.cb2_begin + (blockIdx.x - sv.nblocks0) * THREADS + threadIdx.x : sv.cb_begin + (int)(blockIdx.x * THREADS + threadIdx.x);
     live = cb < (second ? sv.cb2_end : sv.cb_end);
   }
   if (!MEASURE && !BULK && !live) return;
@@ -557,7 +568,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   if (MEASURE) {
     double f = 0.0;
     block_sum2<THREADS>(f, q);
-    if (threadIdx.x == 0) qpartials[blockIdx.x] = q;
+    if (threadIdx.x == 0) qpartials[bid] = q;
   }
 }
 
@@ -597,7 +608,8 @@ ovr_halfsweep_pair8_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T o
   C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)(4 * h) * 6 * SITES + i;
   // exchange area behind the link slots: [h][real 0..17][SITES] doubles
   double* xch = reinterpret_cast<double*>(smem_raw + (size_t)8 * 6 * SITES * sizeof(C));
-  const int cb = blockIdx.x * SITES + i;
+  const unsigned bid = serpentine_block(parity);
+  const int cb = bid * SITES + i;
   const bool live = cb < g.vh;
   const Site s = site_of(g, parity, live ? cb : 0);
   // this lane's link in direction mu: U_mu(x) (h = 0) or U_mu(x - mu) (h = 1)
@@ -673,7 +685,7 @@ ovr_halfsweep_pair8_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T o
   if (MEASURE) {
     double f = 0.0;
     block_sum2<2 * SITES>(f, q);
-    if (threadIdx.x == 0) qpartials[blockIdx.x] = q;
+    if (threadIdx.x == 0) qpartials[bid] = q;
   }
 }
 

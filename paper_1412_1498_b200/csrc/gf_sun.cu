@@ -135,7 +135,8 @@ __global__ void __launch_bounds__(SUN_THREADS) halfsweep_sun_kernel(cplx_t<T>* _
                                                                     double omega) {
   using C = cplx_t<T>;
   constexpr int NN = N * N;
-  const int cb = blockIdx.x * SUN_THREADS + threadIdx.x;
+  // serpentine block order (see gf_kernels.cu): the odd half-sweep starts where the even one ended, in L2
+  const int cb = ((parity & 1) ? gridDim.x - 1u - blockIdx.x : blockIdx.x) * SUN_THREADS + threadIdx.x;
   if (cb >= g.vh) return;
   const Site s = site_of(g, parity, cb);
   C* fwd = links + link_offset<NN>(g, parity, cb, 0);
