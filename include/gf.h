@@ -158,8 +158,8 @@ enum {
   GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (= 3); 1 = two-pass; 2 = two-pass + L2
                                bulk prefetch; 3 = staged through shared memory with cp.async; 4 = staged, the tile
                                fetched by bulk copies of the TMA unit (cp.async.bulk on an mbarrier); 5 = staged, only
-                               the contiguous forward chunk by bulk copy; 6 = storage 8 only: two warps per 32 sites (forward /
-                               backward links); see DESIGN.md.  {3,4,5} give bit-identical
+                               the contiguous forward chunk by bulk copy; 6 = two warps per 32 sites (forward / backward links; a study, never
+                               the default); see DESIGN.md.  {3,4,5} give bit-identical
                                links, so do {1,2}; in FP64 all five do. */
   GF_OPT_BLOCK_THREADS = 2, /* threads per block of the half-sweep kernel (0 = default; a value the chosen variant
                                has no instantiation for makes the next sweep fail with GF_ECUDA) */

@@ -189,8 +189,11 @@ __device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
 //   r0 = Re(M00+M11), r1 = -Im(M01+M10), r2 = Re(M10-M01), r3 = -Im(M00-M11);   a = r/|r|;
 //   phi = atan2(|a_vec|, a0);  g^omega = (cos(omega phi); a_vec sin(omega phi)/|a_vec|).
 // |r| cancels in both phi and the direction of a_vec, so it is never formed: phi = atan2(S, r0), S = |r_vec|.
+#ifndef GF_SU2_INLINE
+#define GF_SU2_INLINE __forceinline__
+#endif
 template <class T>
-__device__ __forceinline__ void su2_overrelax(T r0, T r1, T r2, T r3, T omega, T& c, T& q1, T& q2, T& q3) {
+__device__ GF_SU2_INLINE void su2_overrelax(T r0, T r1, T r2, T r3, T omega, T& c, T& q1, T& q2, T& q3) {
   const T S2 = r1 * r1 + r2 * r2 + r3 * r3;
   const T S = sqrt_(S2);
   if (S <= tiny_of<T>() * fabs(r0)) {  // reading A7 (includes |r| = 0 and phi = pi: g = 1)

@@ -341,6 +341,66 @@ __device__ __forceinline__ void load_link_smem(const C* sm, int l, C (&u)[9]) {
   load_link<NELEM, FULL, STRIDE>(sm + l * NELEM * STRIDE, u);
 }
 
+// G(x) of one site from its eight links in shared memory (slot_fwd(mu) / slot_bwd(mu): the slots of U_mu(x) / U_mu(x-mu),
+// SELEM elements each, element stride STRIDE); with MEASURE also q = sum_ij |Delta_ij|^2 of the updated links.
+// K(x) is summed in the order mu = 0 forward, mu = 0 backward, mu = 1 forward, ... in every kernel that calls this, so
+// they all produce the same bits.
+template <class T, int SELEM, int ND, int STRIDE, bool MEASURE, bool SERIES, class SlotF, class SlotB, class C>
+__device__ __forceinline__ void site_rotation_from_slots(const C* sm, SlotF slot_fwd, SlotB slot_bwd, T omega, int series,
+                                                         C (&G)[9], double& q) {
+  using TK = RotationType;
+  using CK = cplx_t<TK>;
+  // FP32 links, exact power: the site rotation is first evaluated in FP32 (K(x), the three SU(2) steps); where a
+  // step's |r|^2 falls below FAST_TAU2 the direction r/|r| amplifies the rounding of K beyond the parity budget and
+  // the site is evaluated again in FP64 from the links still in shared memory (a rare, divergent branch).
+  bool rotated = false;
+  if constexpr (sizeof(T) == 4 && !SERIES) {
+    C Kf[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) Kf[e] = mk<T>(T(0), T(0));
+#pragma unroll
+    for (int mu = 0; mu < ND; ++mu) {
+      C u[9];
+      load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+#pragma unroll
+      for (int e = 0; e < 9; ++e) { Kf[e].x += u[e].x; Kf[e].y += u[e].y; }
+      sched_fence();
+      load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) { Kf[i * 3 + j].x += u[j * 3 + i].x; Kf[i * 3 + j].y -= u[j * 3 + i].y; }
+      sched_fence();
+    }
+    T r2min = T(3.0e38);
+    site_gauge_rotation<T, MEASURE, false>(Kf, G, omega, 0, &r2min);
+    if (MEASURE) q = (double)delta_norm2<T>(Kf);
+    rotated = r2min >= FAST_TAU2;
+  }
+  if (!rotated) {
+    KSum<T> ks;
+    ks.clear();
+#pragma unroll
+    for (int mu = 0; mu < ND; ++mu) {
+      C u[9];
+      load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
+#pragma unroll
+      for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
+      sched_fence();
+      load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
+      sched_fence();
+    }
+    CK K[9];
+    ks.finish(K);
+    site_gauge_rotation<TK, MEASURE, SERIES>(K, G, (TK)omega, series);
+    if (MEASURE) q = (double)delta_norm2<TK>(K);
+  }
+}
+
 // MEASURE: the launch also leaves, per block, the sum over its sites of sum_ij |Delta_ij(x)|^2 AFTER the update, taken
 // from K_final(x) = G(x) K(x), which is K(x) of the updated links (the site's own update is the last one to touch
 // them in this half-sweep).  After the odd half-sweep these are the odd sites' terms of theta of the finished sweep.
@@ -484,55 +544,7 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     }
 
     C G[9];
-    // FP32 links, exact power: the site rotation is first evaluated in FP32 (K(x), the three SU(2) steps); where a
-    // step's |r|^2 falls below FAST_TAU2 the direction r/|r| amplifies the rounding of K beyond the parity budget and
-    // the site is evaluated again in FP64 from the links still in shared memory (a rare, divergent branch).
-    bool rotated = false;
-    if constexpr (sizeof(T) == 4 && !SERIES) {
-      C Kf[9];
-#pragma unroll
-      for (int e = 0; e < 9; ++e) Kf[e] = mk<T>(T(0), T(0));
-#pragma unroll
-      for (int mu = 0; mu < ND; ++mu) {
-        C u[9];
-        load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
-#pragma unroll
-        for (int e = 0; e < 9; ++e) { Kf[e].x += u[e].x; Kf[e].y += u[e].y; }
-        sched_fence();
-        load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int j = 0; j < 3; ++j) { Kf[i * 3 + j].x += u[j * 3 + i].x; Kf[i * 3 + j].y -= u[j * 3 + i].y; }
-        sched_fence();
-      }
-      T r2min = T(3.0e38);
-      site_gauge_rotation<T, MEASURE, false>(Kf, G, omega, 0, &r2min);
-      if (MEASURE) q = (double)delta_norm2<T>(Kf);
-      rotated = r2min >= FAST_TAU2;
-    }
-    if (!rotated) {
-      KSum<T> ks;
-      ks.clear();
-#pragma unroll
-      for (int mu = 0; mu < ND; ++mu) {
-        C u[9];
-        load_link_smem<SELEM, STRIDE, true>(sm, slot_fwd(mu), u);
-#pragma unroll
-        for (int e = 0; e < 9; ++e) ks.add(e, u[e].x, u[e].y);
-        sched_fence();
-        load_link_smem<SELEM, STRIDE, true>(sm, slot_bwd(mu), u);
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int j = 0; j < 3; ++j) ks.add(i * 3 + j, u[j * 3 + i].x, -u[j * 3 + i].y);
-        sched_fence();
-      }
-      CK K[9];
-      ks.finish(K);
-      site_gauge_rotation<TK, MEASURE, SERIES>(K, G, (TK)omega, series);
-      if (MEASURE) q = (double)delta_norm2<TK>(K);
-    }
+    site_rotation_from_slots<T, SELEM, ND, STRIDE, MEASURE, SERIES>(sm, slot_fwd, slot_bwd, omega, series, G, q);
 
 #pragma unroll
     for (int mu = 0; mu < NMU; ++mu) {
@@ -585,101 +597,83 @@ static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double om
 }
 
 
-// ---- 8-real storage, two lanes per site (GF_OPT_SWEEP_VARIANT 6) ------------------------------------------------------------
-// With one thread per site the 8-real kernel is bound by the dependent-issue latency of 8 warps per SM (shared memory
-// sets the occupancy; profiles/r2_8real_cfg3_ncu.txt).  Here two WARPS share 32 sites (a lane pair inside one warp would
-// diverge at every step - measured: slower than one thread per site): warp 2k (h = 0) owns the four forward links of its
-// 32 sites, warp 2k+1 (h = 1) the four backward links.  Each lane copies, decodes (once, in place, into rows 0 and 1) and
-// later updates its own four links; the two partial sums of K(x) are exchanged through shared memory (K = own + other:
-// the same bits in both lanes, addition being commutative), and both lanes run the three SU(2) steps.  About 0.6 of the
-// instructions per lane and twice the lanes per site.
-template <class T> struct PairSites { static constexpr int value = sizeof(T) == 8 ? 64 : 128; };
+// ---- two lanes per site (GF_OPT_SWEEP_VARIANT 6) -----------------------------------------------------------------------------
+// A study of what bounds the kernels that are not HBM-bound (8-real storage; the L2-resident configs 0 and 1).  Two WARPS
+// share 32 sites (a lane pair inside one warp would diverge at every step): warp 2k (h = 0) copies in, updates and
+// stores the four forward links of its 32 sites, warp 2k+1 (h = 1) the four backward links; both sum K(x) over all
+// eight links (in the order every other kernel uses, so the links come out bit-identical) and both run the three SU(2)
+// steps.  Same shared memory per site, twice the warps, about 0.75 of the instructions per lane.  8-real storage: each
+// lane reconstructs its own four links.  Measured: no faster anywhere - cfg0 8.5 us and cfg1 23 us per
+// half-sweep with either kernel, 8-real 5.6 against 5.4 ms, cfg2 90 against 63 us - so it is not the default for anything.
+template <class T> struct SplitSites { static constexpr int value = sizeof(T) == 8 ? 64 : 128; };
 
-template <class T, int ND, bool MEASURE>
-__global__ void __launch_bounds__(2 * PairSites<T>::value, sizeof(T) == 8 ? 3 : 2)
-ovr_halfsweep_pair8_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
+template <class T, int NELEM, int ND, bool MEASURE>
+__global__ void __launch_bounds__(2 * SplitSites<T>::value, sizeof(T) == 8 ? 3 : 2)
+ovr_halfsweep_split_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega, double* __restrict__ qpartials) {
   using C = cplx_t<T>;
-  using CK = cplx_t<RotationType>;
-  constexpr int SITES = PairSites<T>::value;
+  constexpr int SITES = SplitSites<T>::value;
+  constexpr int SELEM = NELEM == 4 ? 6 : NELEM;
+  constexpr int SOFF = SELEM - NELEM;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, h = warp & 1;
   const int i = (warp >> 1) * 32 + (threadIdx.x & 31);
-  // slot of (link l, element e) of site i: [l][e][SITES]; this lane's links are l = 4 h + mu
-  C* sm = reinterpret_cast<C*>(smem_raw) + (size_t)(4 * h) * 6 * SITES + i;
-  // exchange area behind the link slots: [h][real 0..17][SITES] doubles
-  double* xch = reinterpret_cast<double*>(smem_raw + (size_t)8 * 6 * SITES * sizeof(C));
+  // slot of (link l, element e) of site i: [l][e][SITES], l = 2 mu (forward), 2 mu + 1 (backward)
+  C* sm = reinterpret_cast<C*>(smem_raw) + i;
+  auto slot_fwd = [](int mu) { return 2 * mu; };
+  auto slot_bwd = [](int mu) { return 2 * mu + 1; };
   const unsigned bid = serpentine_block(parity);
   const int cb = bid * SITES + i;
   const bool live = cb < g.vh;
-  const Site s = site_of(g, parity, live ? cb : 0);
-  // this lane's link in direction mu: U_mu(x) (h = 0) or U_mu(x - mu) (h = 1)
-  auto link_ptr = [&](int mu) -> C* {
-    return h == 0 ? links + link_offset<4>(g, parity, cb, mu) : links + link_offset<4>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
-  };
-  CK K[9];
-#pragma unroll
-  for (int e = 0; e < 9; ++e) K[e] = make_double2(0.0, 0.0);
-  // The loops over the lane's four links are NOT unrolled: the fully unrolled one-thread-per-site kernels are
-  // 90-115 KB of straight-line code that every warp streams through once, and with a dozen warps per SM at different
-  // places in it the instruction caches miss ("no instruction" stalls, profiles/r2_8real_cfg3_ncu.txt).
+  C* ptr[4] = {nullptr, nullptr, nullptr, nullptr};  // this lane's four links in the field
   if (live) {
-#pragma unroll 1
-    for (int mu = 0; mu < 4; ++mu) {
-      const C* p = link_ptr(mu);
+    if (h == 0) {
+      C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
 #pragma unroll
-      for (int e = 0; e < 4; ++e) cp_async<sizeof(C)>(sm + (mu * 6 + 2 + e) * SITES, p + e * 32);
+      for (int mu = 0; mu < 4; ++mu) ptr[mu] = fwd + mu * NELEM * 32;
+    } else {
+      const Site s = site_of(g, parity, cb);
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) ptr[mu] = links + link_offset<NELEM>(g, parity ^ 1, cb_down(g, s, cb, mu), mu);
     }
-    cp_async_wait_all();  // a lane reads only what it copied itself
-#pragma unroll 1
-    for (int mu = 0; mu < 4; mu += 2) {  // two reconstructions at a time (independent dependent chains)
-      C* s8 = sm + mu * 6 * SITES;
-      C* t8 = s8 + 6 * SITES;
-      C u[9], v[9];
-      decode8<T, C, false>(s8[2 * SITES], s8[3 * SITES], s8[4 * SITES], s8[5 * SITES], u);
-      decode8<T, C, false>(t8[2 * SITES], t8[3 * SITES], t8[4 * SITES], t8[5 * SITES], v);
 #pragma unroll
-      for (int e = 0; e < 6; ++e) { s8[e * SITES] = u[e]; t8[e * SITES] = v[e]; }
-    }
-    // this lane's half of K(x) = sum_{mu<ND} [U_mu(x) + U_mu(x-mu)^dagger]   (eq. 1.5), FP64 in both precisions
-#pragma unroll 1
-    for (int mu = 0; mu < ND; ++mu) {
-      C u[9];
-      load_link<6, true, SITES>(sm + mu * 6 * SITES, u);
-      if (h == 0) {
+    for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
-        for (int e = 0; e < 9; ++e) { K[e].x += (double)u[e].x; K[e].y += (double)u[e].y; }
-      } else {
+      for (int e = 0; e < NELEM; ++e) cp_async<sizeof(C)>(sm + ((2 * mu + h) * SELEM + SOFF + e) * SITES, ptr[mu] + e * 32);
+    cp_async_wait_all();
+    if constexpr (NELEM == 4) {
 #pragma unroll
-        for (int r = 0; r < 3; ++r)
+      for (int mu = 0; mu < 4; mu += 2) {  // two reconstructions at a time (independent dependent chains)
+        C* s8 = sm + (2 * mu + h) * SELEM * SITES;
+        C* t8 = s8 + 2 * SELEM * SITES;
+        C u[9], v[9];
+        decode8<T, C, false>(s8[2 * SITES], s8[3 * SITES], s8[4 * SITES], s8[5 * SITES], u);
+        decode8<T, C, false>(t8[2 * SITES], t8[3 * SITES], t8[4 * SITES], t8[5 * SITES], v);
 #pragma unroll
-          for (int c = 0; c < 3; ++c) { K[r * 3 + c].x += (double)u[c * 3 + r].x; K[r * 3 + c].y -= (double)u[c * 3 + r].y; }
+        for (int e = 0; e < 6; ++e) { s8[e * SITES] = u[e]; t8[e * SITES] = v[e]; }
+        sched_fence();
       }
     }
   }
-  // the partner warp's half (every thread of the block reaches the barrier)
-#pragma unroll
-  for (int e = 0; e < 9; ++e) {
-    xch[(h * 18 + 2 * e) * SITES + i] = K[e].x;
-    xch[(h * 18 + 2 * e + 1) * SITES + i] = K[e].y;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int e = 0; e < 9; ++e) {
-    K[e].x += xch[((1 - h) * 18 + 2 * e) * SITES + i];
-    K[e].y += xch[((1 - h) * 18 + 2 * e + 1) * SITES + i];
-  }
+  __syncthreads();  // the partner warp's four links are in place
   double q = 0.0;
   if (live) {
     C G[9];
-    site_gauge_rotation<RotationType, MEASURE, false>(K, G, (RotationType)omega, 0);
-    if (MEASURE && h == 0) q = (double)delta_norm2<RotationType>(K);
-#pragma unroll 1
+    site_rotation_from_slots<T, SELEM, ND, SITES, MEASURE, false>(sm, slot_fwd, slot_bwd, omega, 0, G, q);
+    if (h == 1) q = 0.0;  // the site's theta term is counted once
+#pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
       C u[9], w[9];
-      load_link<6, true, SITES>(sm + mu * 6 * SITES, u);
-      if (h == 0) mul_left_8(G, u, w);        // U_mu(x) <- G U_mu(x)
-      else mul_right_adj_8(u, G, w);          // U_mu(x-mu) <- U_mu(x-mu) G^dagger
-      store_link<4>(link_ptr(mu), w);
+      if (h == 0) {
+        load_link_smem<SELEM, SITES, true>(sm, slot_fwd(mu), u);
+        if constexpr (NELEM == 4) mul_left_8(G, u, w);
+        else mul_left<LinkRows<NELEM>::value>(G, u, w);              // U_mu(x) <- G U_mu(x)
+      } else {
+        load_link_smem<SELEM, SITES, NELEM == 4>(sm, slot_bwd(mu), u);
+        if constexpr (NELEM == 4) mul_right_adj_8(u, G, w);
+        else mul_right_adj<LinkRows<NELEM>::value>(u, G, w);         // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+      }
+      store_link<NELEM>(ptr[mu], w);
+      sched_fence();
     }
   }
   if (MEASURE) {
@@ -689,12 +683,12 @@ ovr_halfsweep_pair8_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T o
   }
 }
 
-template <class T, int ND, bool MEASURE>
-static cudaError_t halfsweep_pair8_T(const KernelArgs& a, int parity, double omega) {
+template <class T, int NELEM, int ND, bool MEASURE>
+static cudaError_t halfsweep_split_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
-  constexpr int SITES = PairSites<T>::value;
-  constexpr size_t SMEM = (size_t)8 * 6 * SITES * sizeof(C) + (size_t)2 * 18 * SITES * sizeof(double);
-  auto kern = ovr_halfsweep_pair8_kernel<T, ND, MEASURE>;
+  constexpr int SITES = SplitSites<T>::value;
+  constexpr size_t SMEM = (size_t)8 * (NELEM == 4 ? 6 : NELEM) * SITES * sizeof(C);
+  auto kern = ovr_halfsweep_split_kernel<T, NELEM, ND, MEASURE>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
   const unsigned blocks = (unsigned)((a.geo.vh + SITES - 1) / SITES);
@@ -756,19 +750,14 @@ template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_T(const KernelArgs& a, int parity, double omega, bool fuse_theta, int* qblocks) {
   using C = cplx_t<T>;
   *qblocks = 0;
-  // 8-real storage: variant 6 = two warps per 32 sites (measured: no faster than one thread per site)
-  const int variant = a.variant;
+  const int variant = a.variant;  // 0: one thread per site, staged (= 3)
   if (variant == 6) {
-    if constexpr (NELEM == 4) {
-      if (a.series > 0 || a.block_threads) return cudaErrorNotSupported;
-      if (fuse_theta) {
-        *qblocks = (a.geo.vh + PairSites<T>::value - 1) / PairSites<T>::value;
-        return halfsweep_pair8_T<T, ND, true>(a, parity, omega);
-      }
-      return halfsweep_pair8_T<T, ND, false>(a, parity, omega);
-    } else {
-      return cudaErrorNotSupported;
+    if (a.series > 0 || a.block_threads) return cudaErrorNotSupported;
+    if (fuse_theta) {
+      *qblocks = (a.geo.vh + SplitSites<T>::value - 1) / SplitSites<T>::value;
+      return halfsweep_split_T<T, NELEM, ND, true>(a, parity, omega);
     }
+    return halfsweep_split_T<T, NELEM, ND, false>(a, parity, omega);
   }
   if (variant == 0 || variant == 3 || variant == 4 || variant == 5) {
     // 8*L bytes of shared memory per thread: FP64/18 1152 B -> 192 threads per SM, FP32/12 384 B -> 512 threads per SM

@@ -220,8 +220,8 @@ def test_argument_errors(gf, torch):
 @pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
 def test_halfsweep_variants_agree_bit_for_bit_and_match_oracle(gf, torch, dims, gauge, prec, storage):
     """GF_OPT_SWEEP_VARIANT 1 (two-pass), 2 (two-pass + L2 bulk prefetch), 3 (staged, the default), 4 (staged, the tile
-    fetched by bulk copies of the TMA unit), 5 (staged, only the forward chunk by bulk copy).  Within a family the
-    arithmetic per site is the same in the same order, so the links must be bit-identical: {0, 3, 4, 5} (staged) and
+    fetched by bulk copies of the TMA unit), 5 (staged, only the forward chunk by bulk copy), 6 (two lanes per site).  Within a family the
+    arithmetic per site is the same in the same order, so the links must be bit-identical: {0, 3, 4, 5, 6} (staged) and
     {1, 2} (two-pass); in FP64 the two families coincide too (with FP32 links the staged kernels evaluate
     well-conditioned sites in FP32, the two-pass kernels every site in FP64).  Each variant is also held to the
     one-sweep oracle bar."""
@@ -229,7 +229,7 @@ def test_halfsweep_variants_agree_bit_for_bit_and_match_oracle(gf, torch, dims, 
     U, Uo = host_input(dims, 0.5, 13, prec, storage)  # the input of test_one_sweep_links_match_oracle
     oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
     ref = {}
-    for variant in (0, 1, 2, 3, 4, 5):
+    for variant in (0, 1, 2, 3, 4, 5, 6):
         fx = gpu_fixer(gf, torch, dims, gauge, prec, storage, U)
         fx.set_option(gf.GF_OPT_SWEEP_VARIANT, variant)
         fx.ovr_sweep(1, omega)
