@@ -26,7 +26,7 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma", "gf_workspace_bytes_sun",
            "gf_create_sun", "gf_slab_set_peer_targets", "gf_ipc_export", "gf_ipc_open", "gf_ipc_close", "gf_combine_slabs",
-           "gf_fix_plan"]
+           "gf_fix_plan", "gf_slab_set_peer_flags", "gf_slab_group_sweep", "gf_slab_group_refresh"]
 
 
 def _load() -> ctypes.CDLL:
@@ -88,6 +88,12 @@ def _load() -> ctypes.CDLL:
         getattr(lib, name).argtypes = [c_void_p, c_int, c_double]
     lib.gf_slab_set_peer_targets.restype = c_int
     lib.gf_slab_set_peer_targets.argtypes = [c_void_p] * 5
+    lib.gf_slab_set_peer_flags.restype = c_int
+    lib.gf_slab_set_peer_flags.argtypes = [c_void_p] * 4
+    lib.gf_slab_group_sweep.restype = c_int
+    lib.gf_slab_group_sweep.argtypes = [POINTER(c_void_p), c_int, c_int, c_double, c_int, c_longlong]
+    lib.gf_slab_group_refresh.restype = c_int
+    lib.gf_slab_group_refresh.argtypes = [POINTER(c_void_p), c_int]
     lib.gf_ipc_export.restype = c_int
     lib.gf_ipc_export.argtypes = [c_void_p, c_char_p, POINTER(c_size_t)]
     lib.gf_ipc_open.restype = c_int
@@ -266,6 +272,22 @@ def gf_slab_set_targets(ctx, upper_ghost0: int, upper_ghost1: int, lower_top_in:
 def gf_slab_set_peer_targets(ctx, upper_ghost0: int, upper_ghost1: int, lower_top_in_even: int, lower_top_in_odd: int) -> int:
     return lib.gf_slab_set_peer_targets(ctx, c_void_p(upper_ghost0), c_void_p(upper_ghost1), c_void_p(lower_top_in_even),
                                         c_void_p(lower_top_in_odd))
+
+
+def gf_slab_set_peer_flags(ctx, own_flags: int, upper_flag: int, lower_flag: int) -> int:
+    return lib.gf_slab_set_peer_flags(ctx, c_void_p(own_flags), c_void_p(upper_flag), c_void_p(lower_flag))
+
+
+def _ctx_array(ctxs):
+    return (c_void_p * len(ctxs))(*[c.value if isinstance(c, c_void_p) else c for c in ctxs])
+
+
+def gf_slab_group_sweep(ctxs, n_sweeps: int, omega: float, reunit_every: int = 0, sweeps_before: int = 0) -> int:
+    return lib.gf_slab_group_sweep(_ctx_array(ctxs), len(ctxs), n_sweeps, omega, reunit_every, sweeps_before)
+
+
+def gf_slab_group_refresh(ctxs) -> int:
+    return lib.gf_slab_group_refresh(_ctx_array(ctxs), len(ctxs))
 
 
 def gf_ipc_export(dev_ptr: int):

@@ -94,6 +94,11 @@ struct gf_ctx {
   char* ret_target;     //                      the lower neighbour's top_in, or null
   char* ret_target_odd; // gf_slab_set_peer_targets: where the odd half-sweep's "ret" message goes (even: ret_target)
   bool alt_top_in;      // gf_slab_set_peer_targets: unpack_top(1-p) reads top_in (p = 0) or the top_out slot (p = 1)
+  // gf_slab_set_peer_flags: stream-ordered synchronisation with the two neighbours (no host wait, no collective)
+  unsigned* own_flags;     // [0] written by the upper neighbour, [1] by the lower one (device memory of this slab)
+  unsigned* upper_flag;    // the upper neighbour's own_flags[1] (this process's or a CUDA-IPC mapping)
+  unsigned* lower_flag;    // the lower neighbour's own_flags[0]
+  unsigned epoch;          // last epoch signalled
   char err[256];
 };
 
@@ -205,6 +210,8 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->top_out = c->top_in = nullptr;
   c->fwd_target[0] = c->fwd_target[1] = c->ret_target = c->ret_target_odd = nullptr;
   c->alt_top_in = false;
+  c->own_flags = c->upper_flag = c->lower_flag = nullptr;
+  c->epoch = 0;
   c->host_result = nullptr;
   c->host_slices = c->dev_slices = nullptr;
   c->defer_acc = nullptr; c->defer_dirty = false;
@@ -856,6 +863,111 @@ int gf_slab_set_peer_targets(gf_ctx* c, void* upper_ghost0, void* upper_ghost1, 
   c->ret_target_odd = (char*)lower_top_in_odd;
   c->alt_top_in = true;
   return GF_OK;
+}
+
+// ---- stream-ordered neighbour synchronisation and the whole sharded sweep behind one call -----------------------------------
+namespace {
+typedef int (*stream_memop_fn)(cudaStream_t, unsigned long long, unsigned, unsigned);
+// cuStreamWriteValue32 / cuStreamWaitValue32, looked up at run time (no link dependency on libcuda)
+stream_memop_fn driver_memop(const char* name) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint(name, &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return nullptr;
+  return (stream_memop_fn)fn;
+}
+// "everything this slab queued so far is done": written into both neighbours' flag slots, in stream order
+int slab_signal(gf_ctx* c, unsigned epoch) {
+  static stream_memop_fn write32 = driver_memop("cuStreamWriteValue32");
+  if (!write32) return fail(c, GF_ECUDA, "cuStreamWriteValue32 is not available");
+  DeviceGuard guard(c);
+  if (write32(c->k.stream, (unsigned long long)(uintptr_t)c->upper_flag, epoch, 0) != 0 ||
+      write32(c->k.stream, (unsigned long long)(uintptr_t)c->lower_flag, epoch, 0) != 0)
+    return fail(c, GF_ECUDA, "cuStreamWriteValue32 failed");
+  c->epoch = epoch;
+  return GF_OK;
+}
+// the slab's stream goes on once both neighbours have signalled `epoch` (wrap-safe >= comparison)
+int slab_wait(gf_ctx* c, unsigned epoch) {
+  static stream_memop_fn wait32 = driver_memop("cuStreamWaitValue32");
+  if (!wait32) return fail(c, GF_ECUDA, "cuStreamWaitValue32 is not available");
+  DeviceGuard guard(c);
+  if (wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[0], epoch, 0 /* GEQ */) != 0 ||
+      wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[1], epoch, 0) != 0)
+    return fail(c, GF_ECUDA, "cuStreamWaitValue32 failed");
+  return GF_OK;
+}
+// one ordering point of the group with its neighbours (local or remote): every slab signals, then every slab waits
+int group_sync(gf_ctx* const* slabs, int n) {
+  for (int s = 0; s < n; ++s)
+    if (int rc = slab_signal(slabs[s], slabs[s]->epoch + 1); rc != GF_OK) return rc;
+  for (int s = 0; s < n; ++s)
+    if (int rc = slab_wait(slabs[s], slabs[s]->epoch); rc != GF_OK) return rc;
+  return GF_OK;
+}
+int group_check(gf_ctx* const* slabs, int n, const char* who) {
+  if (!slabs || n < 1) return GF_EINVAL;
+  for (int s = 0; s < n; ++s) {
+    gf_ctx* c = slabs[s];
+    if (!c) return GF_EINVAL;
+    if (!c->k.slab.ghost || !c->alt_top_in || !c->own_flags) return fail(c, GF_EINVAL, who);
+    if (c->epoch != slabs[0]->epoch) return fail(c, GF_EINVAL, "the slabs of a group must have been driven together");
+  }
+  return GF_OK;
+}
+// both ghost buffers of every neighbour from this group's top slices (after set_links, reunitarize)
+int group_refresh(gf_ctx* const* slabs, int n) {
+  int rc = group_sync(slabs, n);  // nobody still reads the ghost buffers that are about to be overwritten
+  for (int q = 0; q < 2 && rc == GF_OK; ++q)
+    for (int s = 0; s < n && rc == GF_OK; ++s) rc = gf_slab_pack_top(slabs[s], q);
+  if (rc == GF_OK) rc = group_sync(slabs, n);
+  return rc;
+}
+}  // namespace
+
+int gf_slab_set_peer_flags(gf_ctx* c, void* own_flags, void* upper_flag, void* lower_flag) {
+  GF_ENTER(c);
+  if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: no halo workspace attached (gf_slab_attach)");
+  if (!own_flags || !upper_flag || !lower_flag || ((uintptr_t)own_flags % 8))
+    return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: null or misaligned flag address");
+  c->own_flags = (unsigned*)own_flags;
+  c->upper_flag = (unsigned*)upper_flag;
+  c->lower_flag = (unsigned*)lower_flag;
+  c->epoch = 0;
+  cudaError_t e = cudaMemsetAsync(own_flags, 0, 2 * sizeof(unsigned), c->k.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);  // zero before any neighbour can signal
+  if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_set_peer_flags");
+  return GF_OK;
+}
+
+int gf_slab_group_refresh(gf_ctx* const* slabs, int n_slabs) {
+  int rc = group_check(slabs, n_slabs, "gf_slab_group_refresh: every slab needs gf_slab_set_peer_targets and gf_slab_set_peer_flags");
+  return rc == GF_OK ? group_refresh(slabs, n_slabs) : rc;
+}
+
+int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double omega, int reunit_every, long long sweeps_before) {
+  int rc = group_check(slabs, n_slabs, "gf_slab_group_sweep: every slab needs gf_slab_set_peer_targets and gf_slab_set_peer_flags");
+  if (rc != GF_OK) return rc;
+  if (n_sweeps < 0 || reunit_every < 0 || sweeps_before < 0) return fail(slabs[0], GF_EINVAL, "gf_slab_group_sweep: negative argument");
+  if (!(omega >= 1.0 && omega < 2.0)) return fail(slabs[0], GF_EINVAL, "gf_slab_group_sweep: omega outside [1,2)");
+  if (n_sweeps == 0) return GF_OK;
+  // entry: whatever the neighbours still run on the buffers of the last call (a measurement reads the ghost links) is done
+  rc = group_sync(slabs, n_slabs);
+  for (int i = 0; i < n_sweeps && rc == GF_OK; ++i) {
+    for (int p = 0; p < 2 && rc == GF_OK; ++p) {  // even first
+      // the border kernels store both halo messages at their destination (gf_slab_set_peer_targets) ...
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_halfsweep_border(slabs[s], p, omega);
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_signal(slabs[s], slabs[s]->epoch + 1);
+      // ... while the interior is updated ("overlap ... with the update of the remaining gauge links")
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_halfsweep_interior(slabs[s], p, omega);
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_unpack_top(slabs[s], 1 - p);
+    }
+    if (rc == GF_OK && reunit_every > 0 && (sweeps_before + i + 1) % reunit_every == 0) {
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_reunitarize(slabs[s]);
+      if (rc == GF_OK) rc = group_refresh(slabs, n_slabs);
+    }
+  }
+  return rc;
 }
 
 // ---- device memory of another process (CUDA IPC), for gf_slab_set_peer_targets between ranks --------------------------------

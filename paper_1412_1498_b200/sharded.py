@@ -44,7 +44,9 @@ class GpuSlabEngine:
         B = _b.gf_slab_halo_bytes(self.fx.ctx)
         self.halo_bytes = B
         with torch.cuda.device(self.device), torch.cuda.stream(self.stream):  # tied to the stream its kernels run on
-            self.halo = torch.zeros(4 * B, dtype=torch.uint8, device=self.device)
+            # 4 halo buffers + the two synchronisation words of gf_slab_set_peer_flags (same allocation: one IPC handle)
+            self.halo = torch.zeros(4 * B + 256, dtype=torch.uint8, device=self.device)
+        self.flags_offset = 4 * B
         self.fx._check(_b.gf_slab_attach(self.fx.ctx, self.halo.data_ptr(), 4 * B))
         self.ghost = [self.halo[0:B], self.halo[B:2 * B]]
         self.top_out = self.halo[2 * B:3 * B]
@@ -66,6 +68,12 @@ class GpuSlabEngine:
         B = self.halo_bytes
         self.fx._check(_b.gf_slab_set_peer_targets(self.fx.ctx, upper_base, upper_base + B, lower_base + 3 * B,
                                                    lower_base + 2 * B))
+
+    def set_peer_flags(self, upper_base: int, lower_base: int):
+        """The neighbours' workspaces again: this slab signals into the upper one's "from below" word and the lower
+        one's "from above" word (gf_slab_set_peer_flags)."""
+        off = self.flags_offset
+        self.fx._check(_b.gf_slab_set_peer_flags(self.fx.ctx, self.halo.data_ptr() + off, upper_base + off + 4, lower_base + off))
 
     def pack_top(self, parity):
         self.fx._check(_b.gf_slab_pack_top(self.fx.ctx, int(parity)))
@@ -138,16 +146,21 @@ class ShardedGaugeFixer:
     dims: the GLOBAL lattice (nx, ny, nz, nt).  With torch.distributed initialised every rank constructs the same object
     and owns n_slabs / world_size consecutive slabs; without it (or with group=False) all slabs live in this process.
     engine_factory(local_dims, slab_index) builds one slab (default: GpuSlabEngine on `device`).
-    direct: the border kernels store the halo messages straight into the neighbours' buffers instead of handing them to
-    the transport.  None (default): yes wherever the slabs are libgf contexts on GPUs - within one process by plain
-    pointers, between the processes of one node through CUDA-IPC mappings of the neighbours' workspaces ("ipc"; if the
-    mappings cannot be made, e.g. the allocator uses virtual-memory segments, a warning is issued and the transport is
-    used).  False: always the transport.  (device=None with an engine_factory is the seam the CPU schedule test uses to
+    mode: how the halo messages travel and how neighbours are ordered.
+      "flags" (default wherever the slabs are libgf contexts on GPUs): the border kernels store the messages straight into
+        the neighbours' workspaces - plain pointers within a process, CUDA-IPC mappings between the processes of a node -
+        and neighbours are ordered by stream-ordered flag writes / waits; ovr_sweep(n) is ONE libgf call
+        (gf_slab_group_sweep): no Python, host wait or collective per half-sweep.  If the mappings cannot be made (e.g.
+        an allocator with virtual-memory segments) a warning is issued and the transport is used.
+      "ipc": the same delivery, ranks ordered by a one-element all-reduce (NCCL) or a barrier (gloo) per half-sweep.
+      "events": all slabs in this process, delivery by plain pointers, kernels ordered by CUDA events (round 1).
+      "transport": device copies within a process, torch.distributed send / recv between ranks.
+    direct (older spelling): True = "events" / "ipc", False = "transport".  (device=None with an engine_factory is the seam the CPU schedule test uses to
     drive this schedule with host-side slabs.)
     """
 
     def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
-                 engine_factory=None, direct=None):
+                 engine_factory=None, direct=None, mode=None):
         import torch
 
         self.torch = torch
@@ -181,23 +194,35 @@ class ShardedGaugeFixer:
             with torch.cuda.device(self.device):
                 self.comm_stream = torch.cuda.Stream(self.device)
         gpu_slabs = self.on_gpu and all(hasattr(e, "set_targets") for e in self.engines.values())
-        can_direct = self.world == 1 and gpu_slabs
-        if direct and not gpu_slabs:
+        if mode is None:
+            if direct is None:
+                mode = "flags" if gpu_slabs else "transport"
+            elif direct:
+                mode = "events" if self.world == 1 else "ipc"
+            else:
+                mode = "transport"
+        if mode not in ("flags", "events", "ipc", "transport"):
+            raise ValueError("mode must be flags, events, ipc or transport")
+        if mode != "transport" and not gpu_slabs:
             raise ValueError("direct delivery needs libgf slabs on GPUs")
-        self.direct = can_direct if direct is None else (bool(direct) and self.world == 1)
-        self.ipc = False
+        if mode == "events" and self.world > 1:
+            raise ValueError("mode 'events' orders kernels with CUDA events: all slabs must live in this process")
         self._ipc_mapped = {}
-        if self.direct:
+        if mode == "events":
             for s, e in self.engines.items():
                 up, lo = self.engines[(s + 1) % self.n_slabs], self.engines[(s - 1) % self.n_slabs]
                 e.set_targets(up.ghost[0], up.ghost[1], lo.top_in)
-        elif self.world > 1 and gpu_slabs and direct is not False:
-            self.ipc = self._map_neighbours()
-            if not self.ipc:
+        elif mode in ("flags", "ipc"):
+            if not self._map_neighbours(with_flags=mode == "flags"):
                 import warnings
 
                 warnings.warn("ShardedGaugeFixer: CUDA IPC mapping of the neighbours' halo workspaces failed; halo messages "
                               "go through torch.distributed send/recv")
+                mode = "transport"
+        self.mode = mode
+        self.direct = mode == "events"   # in-process direct delivery, kernels ordered by CUDA events
+        self.ipc = mode == "ipc"         # direct delivery between processes, ranks ordered by a collective / barrier
+        self.flags = mode == "flags"     # direct delivery, neighbours ordered by stream-ordered flags; the sweep is one C call
         self._after_unpack = {}
         self.reunit_every = 0
         self.sweeps_total = 0
@@ -205,22 +230,23 @@ class ShardedGaugeFixer:
         self.copies = 0         # local device-to-device copies
 
     # ---- direct delivery between processes -----------------------------------------------------------------------------------
-    def _map_neighbours(self):
+    def _map_neighbours(self, with_flags=False):
         """Exchange CUDA-IPC handles of every slab's halo workspace, map the ones of this rank's remote neighbours and
         give every local slab its two neighbours' addresses.  All ranks agree on the outcome."""
         torch, dist = self.torch, self.dist
-        mine, ok = {}, True
-        for s, e in self.engines.items():
-            rc, handle, off = _b.gf_ipc_export(e.halo.data_ptr())
-            ok = ok and rc == _b.GF_OK
-            mine[s] = (handle, off)
-        gathered = [None] * self.world
-        dist.all_gather_object(gathered, (ok, mine), group=self.group)
-        if not all(g[0] for g in gathered):
-            return False
         table = {}
-        for _, d in gathered:
-            table.update(d)
+        if self.world > 1:
+            mine, ok = {}, True
+            for s, e in self.engines.items():
+                rc, handle, off = _b.gf_ipc_export(e.halo.data_ptr())
+                ok = ok and rc == _b.GF_OK
+                mine[s] = (handle, off)
+            gathered = [None] * self.world
+            dist.all_gather_object(gathered, (ok, mine), group=self.group)
+            if not all(g[0] for g in gathered):
+                return False
+            for _, d in gathered:
+                table.update(d)
 
         def base(slab):
             if slab in self.engines:
@@ -234,20 +260,32 @@ class ShardedGaugeFixer:
 
         bases = {s: (base((s + 1) % self.n_slabs), base((s - 1) % self.n_slabs)) for s in self.slabs}
         good = all(u is not None and l is not None for u, l in bases.values())
-        flags = [None] * self.world
-        dist.all_gather_object(flags, good, group=self.group)
-        if not all(flags):
+        if self.world > 1:
+            agreed = [None] * self.world
+            dist.all_gather_object(agreed, good, group=self.group)
+            good = all(agreed)
+        if not good:
             return False
         for s, (u, l) in bases.items():
             self.engines[s].set_peer_targets(u, l)
+            if with_flags:
+                self.engines[s].set_peer_flags(u, l)  # zeroes this slab's two words and synchronises its stream
+        if self.world > 1:
+            dist.barrier(group=self.group)  # every rank's words are zero before anybody signals
         self._token = torch.zeros(1, dtype=torch.float32, device=self.device)
         return True
+
+    def _ctxs(self):
+        return [self.engines[s].fx.ctx for s in self.slabs]
 
     def _rank_sync(self):
         """One ordering point between all ranks' streams: what every rank queued before it is complete before anything
         queued after it starts.  NCCL: a one-element all-reduce on the transport stream between the compute streams (no
         host wait); other backends: stream synchronisation and a barrier."""
         torch, dist = self.torch, self.dist
+        if dist is None or self.world == 1:
+            self.synchronize()
+            return
         if dist.get_backend(self.group) == "nccl":
             for s in self.slabs:
                 self.comm_stream.wait_event(self.engines[s].mark())
@@ -318,6 +356,11 @@ class ShardedGaugeFixer:
 
     def refresh_ghosts(self):
         """Fill both ghost buffers of every slab from its lower neighbour's top slice (after set_links, reunitarize)."""
+        if self.flags:
+            rc = _b.gf_slab_group_refresh(self._ctxs())
+            if rc != _b.GF_OK:
+                raise _b.GFError(rc, _b.gf_last_error(self._ctxs()[0]))
+            return
         if self.direct:  # pack_top writes into the upper neighbour's ghost buffer: wait for whatever it still runs
             self._join_neighbours({s: self.engines[s].mark() for s in self.slabs})
         if self.ipc:
@@ -364,7 +407,7 @@ class ShardedGaugeFixer:
                 self.engines[s].unpack_top(1 - p)
             self._after_unpack = {s: self.engines[s].mark() for s in self.slabs}
             return
-        if self.ipc:
+        if self.ipc or self.flags:  # (flags: a single half-sweep outside ovr_sweep takes the host-ordered schedule)
             # Between processes: the border kernels store both messages in the neighbours' mapped workspaces (top_in is
             # double-buffered by parity, gf_slab_set_peer_targets), then ONE ordering point between the ranks; the next
             # border kernel only writes buffers whose last readers ran before it.
@@ -398,6 +441,12 @@ class ShardedGaugeFixer:
         """n sweeps, even half-sweep first; reunitarisation cadence as gf_ovr_sweep."""
         if _b.gf_fix_plan(float(omega), 0.0, int(n), 1, 0, 1.0)[0] != _b.GF_OK:
             raise ValueError("omega outside [1,2) or n < 0")
+        if self.flags:  # the whole schedule, reunitarisation cadence included, is one asynchronous libgf call
+            rc = _b.gf_slab_group_sweep(self._ctxs(), int(n), float(omega), self.reunit_every, self.sweeps_total)
+            if rc != _b.GF_OK:
+                raise _b.GFError(rc, _b.gf_last_error(self._ctxs()[0]))
+            self.sweeps_total += int(n)
+            return
         for _ in range(int(n)):
             self.half_sweep(0, omega)
             self.half_sweep(1, omega)

@@ -50,17 +50,20 @@ LATTICES = [((8, 8, 8, 8), 1), ((8, 8, 8, 8), 2), ((8, 8, 8, 8), 4), ((6, 4, 2, 
             ((2, 2, 2, 4), 2), ((16, 4, 4, 12), 2), ((10, 6, 4, 8), 1)]
 
 
-@pytest.mark.parametrize("direct", [True, False], ids=["direct", "transport"])
+@pytest.mark.parametrize("mode", ["flags", "events", "transport"])
 @pytest.mark.parametrize("dims,n_slabs", LATTICES)
 @pytest.mark.parametrize("gauge", ["landau", "coulomb"])
 @pytest.mark.parametrize("prec,storage", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
-def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_slabs, gauge, prec, storage, direct):
-    """direct: the border kernels store the halo messages into the neighbours' buffers (gf_slab_set_targets);
-    transport: they leave them in top_out / ghost and the plumbing copies them."""
+def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_slabs, gauge, prec, storage, mode):
+    """flags: the border kernels store the halo messages into the neighbours' buffers (gf_slab_set_peer_targets), the
+    neighbours are ordered by stream-ordered flags and the sweep is one libgf call (gf_slab_group_sweep);
+    events: the same delivery (gf_slab_set_targets), kernels ordered by CUDA events from Python;
+    transport: the messages stay in top_out / ghost and the plumbing copies them."""
     omega, sweeps = 1.7, 2
+    direct = mode != "transport"
     U, Uo = host_input(dims, 0.5, 31, prec, storage)
-    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, direct=direct)
-    assert sh.direct == direct
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, mode=mode)
+    assert sh.mode == mode
     sh.set_links_global(torch.from_numpy(U).cuda())
     F0, th0 = sh.measure()
     sh.ovr_sweep(sweeps, omega)
@@ -96,12 +99,12 @@ def test_sharded_sweeps_against_oracle_and_single_context(gf, torch, dims, n_sla
 
 @pytest.mark.parametrize("gauge,prec,storage,n_slabs", [("landau", "f64", 18, 2), ("coulomb", "f64", 12, 4),
                                                         ("landau", "f32", 12, 2)])
-@pytest.mark.parametrize("direct", [True, False], ids=["direct", "transport"])
-def test_sharded_fix_matches_single_context_trajectory(gf, torch, gauge, prec, storage, n_slabs, direct):
+@pytest.mark.parametrize("mode", ["flags", "events", "transport"])
+def test_sharded_fix_matches_single_context_trajectory(gf, torch, gauge, prec, storage, n_slabs, mode):
     """The whole driver loop (measurement cadence, stop test, reunitarisation + ghost refresh) on slabs against gf_fix."""
     dims, omega, eps, cap, every, reunit = (8, 8, 8, 8), 1.7, 1e-9 if prec == "f64" else 1e-6, 300, 10, 20
     U, _ = host_input(dims, 0.3, 32, prec, storage)
-    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, direct=direct)
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, mode=mode)
     sh.set_reunit_every(reunit)
     sh.set_links_global(torch.from_numpy(U).cuda())
     done, hist = sh.fix(omega, eps, cap, every)

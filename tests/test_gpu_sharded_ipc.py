@@ -30,10 +30,10 @@ def _worker(rank, world, port, case, out):
 
     torch.cuda.set_device(0)
     dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
-    dims, n_slabs, gauge, prec, storage, sweeps, reunit = case
+    dims, n_slabs, gauge, prec, storage, sweeps, reunit, mode = case
     U = gi.make_links(dims, 0.5, 77, dtype=np.float32 if prec == "f32" else np.float64)
-    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, device="cuda:0")
-    assert sh.ipc and not sh.direct, "the CUDA-IPC mapping of the neighbours' workspaces was not made"
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, device="cuda:0", mode=mode)
+    assert sh.mode == (mode or "flags"), "the CUDA-IPC mapping of the neighbours' workspaces was not made"
     sh.set_reunit_every(reunit)
     sh.set_links_global(torch.from_numpy(U).cuda())
     done, hist = sh.fix(1.7, 0.0, sweeps, 2)
@@ -45,9 +45,13 @@ def _worker(rank, world, port, case, out):
     dist.destroy_process_group()
 
 
-CASES = [((8, 8, 8, 8), 2, "landau", "f64", 18, 4, 0),      # one slab per rank: both neighbours are the other rank
-         ((8, 6, 4, 8), 4, "coulomb", "f64", 12, 4, 3),     # two slabs per rank (local and remote neighbours), lt = 2, reunit
-         ((6, 4, 4, 8), 2, "landau", "f32", 12, 3, 0)]
+# mode None = the default ("flags": neighbours ordered by stream-ordered flag writes / waits, the sweep is one libgf call);
+# "ipc" = the same delivery with a barrier between the ranks per half-sweep
+CASES = [((8, 8, 8, 8), 2, "landau", "f64", 18, 4, 0, None),    # one slab per rank: both neighbours are the other rank
+         ((8, 6, 4, 8), 4, "coulomb", "f64", 12, 4, 3, None),   # two slabs per rank (local and remote neighbours), lt = 2, reunit
+         ((6, 4, 4, 8), 2, "landau", "f32", 12, 3, 0, None),
+         ((8, 8, 8, 8), 2, "landau", "f64", 18, 4, 0, "ipc"),
+         ((8, 6, 4, 8), 4, "coulomb", "f64", 12, 4, 3, "ipc")]
 
 
 @pytest.mark.parametrize("case", CASES)
@@ -58,7 +62,7 @@ def test_ipc_direct_delivery_two_processes_bit_identical(case):
     import gf_inputs as gi
     import paper_1412_1498_b200 as gf
 
-    dims, n_slabs, gauge, prec, storage, sweeps, reunit = case
+    dims, n_slabs, gauge, prec, storage, sweeps, reunit, mode = case
     with mp.Manager() as m:
         out = m.dict()
         mp.spawn(_worker, args=(2, _free_port(), case, out), nprocs=2, join=True)
