@@ -618,6 +618,14 @@ def run_fftsd(args):
     return 0
 
 
+HALO_HOW = {"flags": "stored by the border kernel into the neighbour's workspace (same process: plain pointer, other rank: "
+                     "CUDA-IPC mapping); neighbours ordered by stream-ordered flag writes / waits; the sweep is one libgf call",
+            "ipc": "stored by the border kernel into the CUDA-IPC mapped workspace of the neighbour rank; one 1-element "
+                   "all-reduce per half-sweep orders the ranks",
+            "events": "stored by the border kernel into the neighbour slab of the same process; kernels ordered by CUDA events",
+            "transport": "NCCL send/recv between ranks, device copies within a rank"}
+
+
 def run_sharded(args):
     """--sharded K: the overrelaxation sweep over T-slabs (paper_1412_1498_b200.sharded; SURVEY.md §8(f) NEXT-2,
     PAPER.md:132-134).  The paper's weak-scaling point (32^4 per GPU) is
@@ -653,7 +661,7 @@ def run_sharded(args):
     L = LINK_BYTES[(prec, storage)]
     n_sw, omega = cfg["check_every"], cfg["omega"]
     sh = gf.ShardedGaugeFixer(gdims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}",
-                              direct=False if args.no_direct else None)
+                              mode=args.sharded_mode or ("transport" if args.no_direct else None))
     sh.set_reunit_every(cfg["reunit_every"])
     links = {}
     for s in sh.slabs:  # every slab its own seeded field of the config's recipe (rougher across slab boundaries)
@@ -698,7 +706,8 @@ def run_sharded(args):
                            "step": f"{n_sw} sweeps + 1 F/theta measurement",
                            "parallelism": f"T-slabs: {n_slabs} slabs over {world} rank(s), {K} per rank",
                            "halo": f"2 messages of {halo // len(sh.engines)} B per slab and half-sweep "
-                                   f"({'stored by the border kernel into the neighbour slab' if sh.direct else 'stored by the border kernel into the CUDA-IPC mapped workspace of the neighbour rank; one 1-element NCCL all-reduce per half-sweep orders the ranks' if sh.ipc else 'device copies' if world == 1 else 'NCCL send/recv between ranks'})",
+                                   f"({HALO_HOW[sh.mode] if world > 1 or sh.mode != 'transport' else 'device copies'})",
+                           "mode": sh.mode,
                            "l2": "inputs exceed L2" if 4 * V * L > 126e6 else "field fits L2 in part",
                            "final_F": F, "final_theta": th},
                 "roofline": {"bound": "hbm", "kernel": "ovr_halfsweep_staged_kernel (border + interior launches)",
@@ -736,6 +745,8 @@ def main():
     ap.add_argument("--prec", default="", choices=["", "f64", "f32"], help="kernel study: another precision on the config's lattice")
     ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
+    ap.add_argument("--sharded-mode", default="", choices=["", "flags", "ipc", "events", "transport"],
+                    help="--sharded: ShardedGaugeFixer mode (default: flags on GPUs)")
     ap.add_argument("--peaks", action="store_true", help="print the measured FP64 / FP32 FMA-chain peaks and exit")
     args = ap.parse_args()
     if args.peaks:

@@ -205,7 +205,8 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0; c->fft_own = 1; c->own_table = nullptr;
   c->fft_w_bytes = c->fft_table_bytes = c->fft_work_bytes = 0;
-  c->k.slab = SlabView{nullptr, (g.s3 + 31) / 32, 0, 0, 0, 0, 0, nullptr, nullptr};
+  c->k.slab = SlabView{};
+  c->k.slab.nblk3 = (g.s3 + 31) / 32;
   c->halo_bytes = align_up((size_t)c->k.slab.nblk3 * (storage / 2) * 32 * (prec == GF_FP64 ? 16 : 8));
   c->top_out = c->top_in = nullptr;
   c->fwd_target[0] = c->fwd_target[1] = c->ret_target = c->ret_target_odd = nullptr;
@@ -927,13 +928,13 @@ int group_refresh(gf_ctx* const* slabs, int n) {
 int gf_slab_set_peer_flags(gf_ctx* c, void* own_flags, void* upper_flag, void* lower_flag) {
   GF_ENTER(c);
   if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: no halo workspace attached (gf_slab_attach)");
-  if (!own_flags || !upper_flag || !lower_flag || ((uintptr_t)own_flags % 8))
+  if (!own_flags || !upper_flag || !lower_flag || ((uintptr_t)own_flags % 16))
     return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: null or misaligned flag address");
   c->own_flags = (unsigned*)own_flags;
   c->upper_flag = (unsigned*)upper_flag;
   c->lower_flag = (unsigned*)lower_flag;
   c->epoch = 0;
-  cudaError_t e = cudaMemsetAsync(own_flags, 0, 2 * sizeof(unsigned), c->k.stream);
+  cudaError_t e = cudaMemsetAsync(own_flags, 0, 4 * sizeof(unsigned), c->k.stream);  // two flag words + the block counter
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);  // zero before any neighbour can signal
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_set_peer_flags");
   return GF_OK;
@@ -954,11 +955,19 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
   rc = group_sync(slabs, n_slabs);
   for (int i = 0; i < n_sweeps && rc == GF_OK; ++i) {
     for (int p = 0; p < 2 && rc == GF_OK; ++p) {  // even first
-      // the border kernels store both halo messages at their destination (gf_slab_set_peer_targets) ...
-      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_halfsweep_border(slabs[s], p, omega);
-      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_signal(slabs[s], slabs[s]->epoch + 1);
-      // ... while the interior is updated ("overlap ... with the update of the remaining gauge links")
-      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_halfsweep_interior(slabs[s], p, omega);
+      // ONE kernel per slab and half-sweep: its border blocks come first, store both halo messages at their destination
+      // (gf_slab_set_peer_targets) and the last of them raises the neighbours' flags, while the rest of the grid
+      // updates the interior ("overlap ... with the update of the remaining gauge links")
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) {
+        gf_ctx* c = slabs[s];
+        DeviceGuard guard(c);
+        cudaError_t e = launch_halfsweep_slab_fused(c->k, p, omega, c->fwd_target[p], p ? c->ret_target_odd : c->ret_target,
+                                                    c->own_flags + 2, c->upper_flag, c->lower_flag, c->epoch + 1);
+        if (e != cudaSuccess) { rc = fail_cuda(c, e, "gf_slab_group_sweep"); break; }
+        c->epoch += 1;
+        c->launches += 1;
+        c->qblocks = 0;
+      }
       for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
       for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_unpack_top(slabs[s], 1 - p);
     }

@@ -15,6 +15,14 @@ struct SlabView {
   int cb2_begin, cb2_end;  //     a second range (border launch: bottom and top slice in one grid)
   void* top_out;         // non-null: top-slice sites also leave their updated U_t(x) here (message layout)
   void* ret_out;         // non-null: t = 0 sites also leave their updated U_t(x - t) here (message layout, one parity)
+  // fused launch (border and interior in one grid): a third range behind the two border ranges, and the signal the last
+  // of the first sig_blocks blocks (the border) raises in both neighbours' flag words once all of them have stored
+  int nblocks1;            // blocks of the second range
+  int cb3_begin, cb3_end;  // third range (the interior); empty if cb3_end <= cb3_begin
+  int sig_blocks;          // 0: no signal
+  unsigned* sig_counter;   // zero between launches
+  unsigned* sig_flag[2];
+  unsigned sig_epoch;
 };
 
 struct KernelArgs {
@@ -47,6 +55,11 @@ bool halfsweep_can_fuse_theta(const KernelArgs& a);
 // use a.slab.ghost; with top_out the top-slice sites also write their updated U_t(x) there)
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
                                   int cb2_begin, int cb2_end, void* top_out, void* ret_out);
+// The whole half-sweep of a slab in ONE launch: bottom slice, top slice (both deliver their halo messages to top_out /
+// ret_out), then the interior; the border blocks come first in the grid, and the last of them to finish writes `epoch`
+// into the two flag words (system scope), so the neighbours can go on while the interior is still being updated.
+cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch);
 // U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
 cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);

@@ -445,11 +445,21 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   int cb = bid * THREADS + threadIdx.x;
   bool live = cb < g.vh;
   if (SLAB) {
-    const bool second = (int)blockIdx.x >= sv.nblocks0;
-    cb = second ? sv.cb2_begin + (blockIdx.x - sv.nblocks0) * THREADS + threadIdx.x : sv.cb_begin + (int)(blockIdx.x * THREADS + threadIdx.x);
-    live = cb < (second ? sv.cb2_end : sv.cb_end);
+    const int b = (int)blockIdx.x;
+    if (b < sv.nblocks0) {
+      cb = sv.cb_begin + b * THREADS + threadIdx.x;
+      live = cb < sv.cb_end;
+    } else if (b < sv.nblocks0 + sv.nblocks1) {
+      cb = sv.cb2_begin + (b - sv.nblocks0) * THREADS + threadIdx.x;
+      live = cb < sv.cb2_end;
+    } else {  // interior of a fused launch, in serpentine order (see serpentine_block)
+      const int nb3 = (int)gridDim.x - sv.nblocks0 - sv.nblocks1;
+      const int b3 = b - sv.nblocks0 - sv.nblocks1;
+      cb = sv.cb3_begin + ((parity & 1) ? nb3 - 1 - b3 : b3) * THREADS + threadIdx.x;
+      live = cb < sv.cb3_end;
+    }
   }
-  if (!MEASURE && !BULK && !live) return;
+  if (!MEASURE && !BULK && !SLAB && !live) return;
   if (MASKED && !active[cb / g.s3]) return;  // the slice is finished (its theta_t is below eps)
   double q = 0.0;
   C* fwd = nullptr;
@@ -581,6 +591,20 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
     double f = 0.0;
     block_sum2<THREADS>(f, q);
     if (threadIdx.x == 0) qpartials[bid] = q;
+  }
+  if (SLAB && sv.sig_blocks > 0 && (int)blockIdx.x < sv.sig_blocks) {
+    // a border block of a fused launch: when the last of them has stored its links and halo messages, tell the
+    // neighbours (release at system scope: the messages may sit in another GPU's memory)
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence_system();
+      if (atomicAdd(sv.sig_counter, 1u) == (unsigned)sv.sig_blocks - 1u) {
+        *sv.sig_counter = 0u;  // ready for the next launch on this stream
+        __threadfence_system();
+        *reinterpret_cast<volatile unsigned*>(sv.sig_flag[0]) = sv.sig_epoch;
+        *reinterpret_cast<volatile unsigned*>(sv.sig_flag[1]) = sv.sig_epoch;
+      }
+    }
   }
 }
 
@@ -737,10 +761,41 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.cb_begin = cb_begin; sv.cb_end = cb_end;
   sv.cb2_begin = cb2_begin; sv.cb2_end = cb2_end;
   sv.nblocks0 = cb_end > cb_begin ? (cb_end - cb_begin + THREADS - 1) / THREADS : 0;
+  sv.nblocks1 = cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0;
+  sv.cb3_begin = sv.cb3_end = 0;
+  sv.sig_blocks = 0;
   sv.top_out = top_out;
   sv.ret_out = ret_out;
-  const unsigned blocks = (unsigned)(sv.nblocks0 + (cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0));
+  const unsigned blocks = (unsigned)(sv.nblocks0 + sv.nblocks1);
   kern<<<blocks, THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0, nullptr, nullptr);
+  return cudaGetLastError();
+}
+
+template <class T, int NELEM, int ND>
+static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
+                                          unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch) {
+  using C = cplx_t<T>;
+  constexpr int THREADS = staged_threads<T>();
+  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
+  static PerDeviceOnce attr;  // per instantiation and device
+  if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
+  const Geo& g = a.geo;
+  SlabView sv = a.slab;
+  sv.cb_begin = 0; sv.cb_end = g.s3;                    // bottom slice
+  sv.cb2_begin = g.vh - g.s3; sv.cb2_end = g.vh;        // top slice
+  sv.cb3_begin = g.s3; sv.cb3_end = g.vh - g.s3;        // interior (empty for a slab of two slices)
+  sv.nblocks0 = (g.s3 + THREADS - 1) / THREADS;
+  sv.nblocks1 = sv.nblocks0;
+  const int nblocks2 = sv.cb3_end > sv.cb3_begin ? (sv.cb3_end - sv.cb3_begin + THREADS - 1) / THREADS : 0;
+  sv.sig_blocks = sv.nblocks0 + sv.nblocks1;
+  sv.sig_counter = counter;
+  sv.sig_flag[0] = flag_up; sv.sig_flag[1] = flag_down;
+  sv.sig_epoch = epoch;
+  sv.top_out = top_out;
+  sv.ret_out = ret_out;
+  kern<<<(unsigned)(sv.sig_blocks + nblocks2), THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0,
+                                                                          nullptr, nullptr);
   return cudaGetLastError();
 }
 
@@ -916,6 +971,11 @@ cudaError_t launch_defer(const KernelArgs& a, void* acc, bool flush) {
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
                                   int cb2_begin, int cb2_end, void* top_out, void* ret_out) {
   GF_DISPATCH(halfsweep_slab_T, a, parity, omega, cb_begin, cb_end, cb2_begin, cb2_end, top_out, ret_out);
+}
+
+cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch) {
+  GF_DISPATCH(halfsweep_slab_fused_T, a, parity, omega, top_out, ret_out, counter, flag_up, flag_down, epoch);
 }
 
 // ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------
