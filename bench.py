@@ -321,7 +321,16 @@ def run_ours(args):
     n_sw = cfg["check_every"]
     omega = cfg["omega"]
 
-    fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
+    N = args.ncolors or 3
+    if N != 3:  # general SU(N) study (gf_create_sun): all N^2 entries stored, host generator, no e2e / CPU legs
+        import numpy as np
+
+        args.no_e2e = args.no_cpu = True
+        storage = 2 * N * N
+        L = storage * (8 if prec == "f64" else 4)
+        fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, ncolors=N, device=f"cuda:{local}")
+    else:
+        fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}")
     if args.defer:
         fx.defer_temporal_links()
     if storage == 8:  # a study on a rough synthetic field: a few of its 1.3e8 links lie outside the format's domain
@@ -331,9 +340,13 @@ def run_ours(args):
     if args.block:
         fx.set_option(gf.GF_OPT_BLOCK_THREADS, args.block)
     fx.set_reunit_every(cfg["reunit_every"])
-    canon = fx.new_links_buffer()
-    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"] + 1000 * rank, prec,
-                         torch.cuda.current_stream().cuda_stream)
+    if N != 3:
+        canon = torch.from_numpy(gi.make_links_sun(dims, N, cfg["roughness"], cfg["seed"] + 1000 * rank,
+                                                   dtype=np.float64 if prec == "f64" else np.float32)).cuda()
+    else:
+        canon = fx.new_links_buffer()
+        gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"] + 1000 * rank, prec,
+                             torch.cuda.current_stream().cuda_stream)
     fx.set_links(canon)
     torch.cuda.synchronize()
 
@@ -382,14 +395,19 @@ def run_ours(args):
     # the reunitarisation launches inside the sweep region (config 2 only) are subtracted at their algorithmic cost
     ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
     achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
-    kernel = halfsweep_kernel_name(storage, args.variant, args.defer, V // 2)
-    traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer or args.prec) else (None, None)
+    kernel = halfsweep_kernel_name(storage, args.variant, args.defer, V // 2) if N == 3 else f"halfsweep_sun_kernel<N={N}>"
+    traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer or args.prec or N != 3) else (None, None)
     # flops leg: the FMA-chain peaks measured now, on this GPU, under the clocks it runs at after
     # the timed region (gf_peak_fma); the site rotation is FP64 in both storage precisions, the link products are in
     # the storage precision
     fp = measure_fp_peaks(0.25)
-    flops64 = FLOPS_ROTATION + (FLOPS_LINKS[storage] if prec == "f64" else 0)
-    flops32 = FLOPS_LINKS[storage] if prec == "f32" else 0
+    if N == 3:
+        flops64 = FLOPS_ROTATION + (FLOPS_LINKS[storage] if prec == "f64" else 0)
+        flops32 = FLOPS_LINKS[storage] if prec == "f32" else 0
+    else:  # the same counting for N x N: K sum, N(N-1)/2 subgroup steps (31 + two 2-row rotations), 8 full products
+        rot = 8 * 2 * N * N + (N * (N - 1) // 2) * (31 + 2 * 14 * N)
+        prod = 8 * N * N * (8 * N - 2)
+        flops64, flops32 = rot + (prod if prec == "f64" else 0), (prod if prec == "f32" else 0)
     t_bytes_ms = bytes_per_launch / (peak * 1e9) * 1e3
     t_flops_ms = (V // 2) * (flops64 / (fp["f64_tflops"] * 1e12) + flops32 / (fp["f32_tflops"] * 1e12)) * 1e3
     roofline = {"bound": "hbm" if t_bytes_ms >= t_flops_ms else "alu", "kernel": kernel, "achieved": achieved, "peak": peak,
@@ -531,7 +549,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": prec, "data": "synthetic",
-        "config": {"workload": workload_name(cfg) + (" (deferred temporal links)" if args.defer else "")
+        "config": {"workload": workload_name(cfg) + (" (deferred temporal links)" if args.defer else "") + (f" [study: SU({N}) links, all N^2 entries stored]" if N != 3 else "")
                    + (" [study: not the config's own storage / gauge / precision]" if args.storage or args.gauge or args.prec else ""),
                    "step": f"{n_sw} sweeps + 1 F/theta measurement",
                    "sites": V, "l2": "inputs exceed L2 (field %.2f GB vs 126 MB)" % (4 * V * L / 1e9)
@@ -743,6 +761,8 @@ def main():
     ap.add_argument("--storage", type=int, default=0, help="kernel study: 18, 12 or 8 (FP64) instead of the config's storage")
     ap.add_argument("--gauge", default="", choices=["", "landau", "coulomb"], help="kernel study: another gauge on the config's lattice")
     ap.add_argument("--prec", default="", choices=["", "f64", "f32"], help="kernel study: another precision on the config's lattice")
+    ap.add_argument("--ncolors", type=int, default=0, choices=[0, 2, 3, 4],
+                    help="kernel study: SU(N) links (gf_create_sun) on the config's lattice, host generator (use cfg2 or smaller)")
     ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
     ap.add_argument("--sharded-mode", default="", choices=["", "flags", "ipc", "events", "transport"],

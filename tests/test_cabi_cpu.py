@@ -87,3 +87,28 @@ def test_header_compiles_as_c99_and_links_from_c(tmp_path):
     r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "cabi_consumer: ok" in r.stdout
+
+
+def test_driver_decisions_behind_the_abi():
+    """gf_fix_plan / gf_combine_slabs: the stop test, cadence and the slabs' means that callers driving several contexts
+    take from the library (Algorithm 1 l.2); no device work."""
+    # (omega, eps, max_sweeps, check_every, sweeps_done, theta) -> sweeps to the next measurement
+    assert gf.gf_fix_plan(1.7, 1e-12, 2000, 10, 0, 5.0) == (gf.GF_OK, 10)
+    assert gf.gf_fix_plan(1.7, 1e-12, 2000, 10, 1995, 5.0) == (gf.GF_OK, 5)      # capped by max_sweeps
+    assert gf.gf_fix_plan(1.7, 1e-12, 2000, 10, 2000, 5.0) == (gf.GF_OK, 0)      # cap reached
+    assert gf.gf_fix_plan(1.7, 1e-12, 2000, 10, 40, 9e-13) == (gf.GF_OK, 0)      # theta < eps: stop
+    assert gf.gf_fix_plan(1.7, 1e-12, 2000, 10, 40, 1e-12) == (gf.GF_OK, 10)     # theta == eps: not yet
+    assert gf.gf_fix_plan(1.7, 0.0, 200, 20, 180, 0.0) == (gf.GF_OK, 20)         # eps = 0: fixed-sweep run
+    for bad in [(2.0, 1e-12, 10, 1, 0, 1.0), (0.99, 1e-12, 10, 1, 0, 1.0), (1.7, -1.0, 10, 1, 0, 1.0),
+                (1.7, 1e-12, -1, 1, 0, 1.0), (1.7, 1e-12, 10, 0, 0, 1.0), (1.7, 1e-12, 10, 1, -1, 1.0)]:
+        assert gf.gf_fix_plan(*bad)[0] == gf.GF_EINVAL
+    rc, F, th = gf.gf_combine_slabs([0.25, 0.5, 0.75, 1.0], [4.0, 3.0, 2.0, 1.0])
+    assert (rc, F, th) == (gf.GF_OK, 0.625, 2.5)
+    # slab order: the sum is taken left to right, so every rank gets the same bits
+    xs = [0.1, 0.2, 0.3]
+    assert gf.gf_combine_slabs(xs, xs)[1] == ((0.1 + 0.2) + 0.3) / 3
+    assert gf.gf_combine_slabs([float("nan")], [1.0])[0] == gf.GF_ENUMERIC
+    # the group calls refuse contexts that are not slabs with peer targets and flags, before any device work
+    assert gf.gf_slab_group_sweep([], 1, 1.7) == gf.GF_EINVAL
+    assert gf.gf_slab_group_refresh([]) == gf.GF_EINVAL
+    assert gf.gf_ipc_export(0)[0] == gf.GF_EINVAL and gf.gf_ipc_open(b"\0" * 64, 0)[0] in (gf.GF_ECUDA, gf.GF_EINVAL)
