@@ -953,6 +953,10 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
   if (n_sweeps == 0) return GF_OK;
   // entry: whatever the neighbours still run on the buffers of the last call (a measurement reads the ghost links) is done
   rc = group_sync(slabs, n_slabs);
+  // The links the upper neighbour returns during half-sweep p (into top_in, double-buffered by p) belong to the top-slice
+  // sites of parity 1-p, which are visited next: the next launch reads them straight from that buffer, and only the
+  // last half-sweep of the call (or one before a reunitarisation) is followed by gf_slab_unpack_top.
+  bool pending = false;  // top-slice U_t of parity 0 still sits in the buffer the odd half-sweep filled
   for (int i = 0; i < n_sweeps && rc == GF_OK; ++i) {
     for (int p = 0; p < 2 && rc == GF_OK; ++p) {  // even first
       // ONE kernel per slab and half-sweep: its border blocks come first, store both halo messages at their destination
@@ -961,17 +965,26 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
       for (int s = 0; s < n_slabs && rc == GF_OK; ++s) {
         gf_ctx* c = slabs[s];
         DeviceGuard guard(c);
+        const void* returned = nullptr;  // what half-sweep 1-p left for this one
+        if (p == 1) returned = c->top_in;
+        else if (pending) returned = c->top_out;
         cudaError_t e = launch_halfsweep_slab_fused(c->k, p, omega, c->fwd_target[p], p ? c->ret_target_odd : c->ret_target,
-                                                    c->own_flags + 2, c->upper_flag, c->lower_flag, c->epoch + 1);
+                                                    c->own_flags + 2, c->upper_flag, c->lower_flag, c->epoch + 1, returned);
         if (e != cudaSuccess) { rc = fail_cuda(c, e, "gf_slab_group_sweep"); break; }
         c->epoch += 1;
         c->launches += 1;
         c->qblocks = 0;
       }
       for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
-      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_unpack_top(slabs[s], 1 - p);
     }
-    if (rc == GF_OK && reunit_every > 0 && (sweeps_before + i + 1) % reunit_every == 0) {
+    pending = true;
+    const bool last = i == n_sweeps - 1;
+    const bool reunit = reunit_every > 0 && (sweeps_before + i + 1) % reunit_every == 0;
+    if (rc == GF_OK && (last || reunit)) {
+      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_slab_unpack_top(slabs[s], 0);
+      pending = false;
+    }
+    if (rc == GF_OK && reunit) {
       for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = gf_reunitarize(slabs[s]);
       if (rc == GF_OK) rc = group_refresh(slabs, n_slabs);
     }

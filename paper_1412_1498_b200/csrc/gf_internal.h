@@ -23,6 +23,9 @@ struct SlabView {
   unsigned* sig_counter;   // zero between launches
   unsigned* sig_flag[2];
   unsigned sig_epoch;
+  // non-null: the top-slice sites take U_t(x) from this message buffer (what the upper neighbour's last half-sweep
+  // returned) instead of from the field - the unpack kernel between two half-sweeps is then not needed
+  const void* top_in_src;
 };
 
 struct KernelArgs {
@@ -59,7 +62,8 @@ cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega,
 // ret_out), then the interior; the border blocks come first in the grid, and the last of them to finish writes `epoch`
 // into the two flag words (system scope), so the neighbours can go on while the interior is still being updated.
 cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch);
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
+                                        const void* top_in_src);
 // U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
 cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);

@@ -527,7 +527,13 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       for (int mu = 0; mu < NMU; ++mu) {
 #pragma unroll
         for (int e = 0; e < NELEM; ++e) {
-          cp_async<sizeof(C)>(sm + (slot_fwd(mu) * SELEM + SOFF + e) * STRIDE, fwd + (mu * NELEM + e) * 32);
+          const C* src = fwd + (mu * NELEM + e) * 32;
+          if (SLAB && mu == 3 && sv.top_in_src && cb >= g.vh - g.s3) {  // the link the upper neighbour just returned
+            SlabView in = sv;
+            in.ghost = const_cast<void*>(sv.top_in_src);
+            src = ghost_link<T, NELEM, C>(in, 0, cb - (g.vh - g.s3)) + e * 32;
+          }
+          cp_async<sizeof(C)>(sm + (slot_fwd(mu) * SELEM + SOFF + e) * STRIDE, src);
           cp_async<sizeof(C)>(sm + (slot_bwd(mu) * SELEM + SOFF + e) * STRIDE, bwd[mu] + e * 32);
         }
       }
@@ -764,6 +770,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
   sv.nblocks1 = cb2_end > cb2_begin ? (cb2_end - cb2_begin + THREADS - 1) / THREADS : 0;
   sv.cb3_begin = sv.cb3_end = 0;
   sv.sig_blocks = 0;
+  sv.top_in_src = nullptr;
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   const unsigned blocks = (unsigned)(sv.nblocks0 + sv.nblocks1);
@@ -773,7 +780,8 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
 
 template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                          unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch) {
+                                          unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
+                                          const void* top_in_src) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
@@ -794,6 +802,7 @@ static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, doubl
   sv.sig_epoch = epoch;
   sv.top_out = top_out;
   sv.ret_out = ret_out;
+  sv.top_in_src = top_in_src;
   kern<<<(unsigned)(sv.sig_blocks + nblocks2), THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0,
                                                                           nullptr, nullptr);
   return cudaGetLastError();
@@ -974,8 +983,9 @@ cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega,
 }
 
 cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch) {
-  GF_DISPATCH(halfsweep_slab_fused_T, a, parity, omega, top_out, ret_out, counter, flag_up, flag_down, epoch);
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
+                                        const void* top_in_src) {
+  GF_DISPATCH(halfsweep_slab_fused_T, a, parity, omega, top_out, ret_out, counter, flag_up, flag_down, epoch, top_in_src);
 }
 
 // ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------
