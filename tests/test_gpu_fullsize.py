@@ -218,3 +218,78 @@ def test_full_size_hand_written_transforms_against_the_cufft_path(name):
     diff = float((res[1][0] - res[0][0]).abs().max())
     assert diff <= (1e-12 if prec == "f64" else 2e-5), diff
     assert abs(res[1][1][0] - res[0][1][0]) <= (1e-12 if prec == "f64" else 1e-6)
+
+
+# ---- round 2: the staging variants, the chunked host path and the FMA-chain peaks at full size -----------------------------
+@pytest.mark.parametrize("name", ["cfg2", "cfg3"])
+def test_full_size_staging_variants_are_bit_identical(name):
+    """GF_OPT_SWEEP_VARIANT 3 (cp.async), 4 (TMA bulk copies on an mbarrier), 5 (forward chunk by bulk copy) and 6 (two
+    warps per 32 sites) on a full config lattice: tiles whose backward neighbours straddle source tiles (48^3 x 96:
+    rows of 24 sites; 32^4: rows of 16, the FP32 8-byte alignment fallback) and the serpentine block order."""
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    cfg = next(c for c in gi.CONFIGS if c["name"] == name)
+    dims, prec, storage = cfg["dims"], cfg["prec"], cfg["storage"]
+    ref = None
+    for variant in (3, 4, 5, 6):
+        fx = gf.GaugeFixer(dims, gauge=cfg["gauge"], prec=prec, storage=storage)
+        fx.set_option(gf.GF_OPT_SWEEP_VARIANT, variant)
+        canon = fx.new_links_buffer()
+        gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], prec,
+                             torch.cuda.current_stream().cuda_stream)
+        fx.set_links(canon)
+        fx.ovr_sweep(2, cfg["omega"])
+        m = fx.measure()
+        fx.get_links(out=canon)
+        fx.close()
+        if ref is None:
+            ref = (canon, m)
+        else:
+            assert torch.equal(canon, ref[0]), f"variant {variant}"
+            assert m == ref[1]
+        del canon
+    torch.cuda.empty_cache()
+
+
+def test_host_path_chunks_through_both_staging_buffers():
+    """gf_set_links_host / gf_get_links_host on a field of ten staging chunks (604 MB against 64 MiB buffers), pinned
+    memory, copies on the context's copy stream beside the reorder kernels: the round trip is exact and equals the
+    device-side set/get."""
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    dims = (32, 32, 32, 32)
+    fx = gf.GaugeFixer(dims, prec="f64", storage=18)
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, 0.4, 9, "f64", torch.cuda.current_stream().cuda_stream)
+    host = torch.empty(canon.shape, dtype=canon.dtype).pin_memory()
+    host.copy_(canon)
+    fx.set_links_host(host)
+    assert torch.equal(fx.get_links(), canon)
+    back = torch.empty_like(host).pin_memory()
+    fx.get_links_host(back)
+    assert torch.equal(back, host)
+    fx.ovr_sweep(1, 1.7)       # queued work is ordered before the next host transfer
+    fx.get_links_host(back)
+    assert torch.equal(back.cuda(), fx.get_links()) and not torch.equal(back, host)
+    fx.close()
+
+
+def test_fma_chain_peaks_are_plausible():
+    """gf_peak_fma (the flops leg's denominator): a B200 has 64 FP64 and 128 FP32 FMA lanes per SM."""
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    scratch = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    props = torch.cuda.get_device_properties(0)
+    for prec, lanes in ((gf.GF_FP64, 64), (gf.GF_FP32, 128)):
+        rc, t = gf.gf_peak_fma(prec, 0.2, scratch.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        assert rc == gf.GF_OK
+        nominal = props.multi_processor_count * lanes * 2 * 1.965e9 / 1e12
+        assert 0.5 * nominal <= t <= 1.05 * nominal, (prec, t, nominal)
+    assert gf.gf_peak_fma(2, 0.2, scratch.data_ptr(), 0)[0] == gf.GF_EINVAL
+    assert gf.gf_peak_fma(gf.GF_FP64, 0.0, scratch.data_ptr(), 0)[0] == gf.GF_EINVAL
