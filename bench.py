@@ -447,25 +447,39 @@ def run_ours(args):
 
     # ---- end to end through the host entry points (pinned host memory, copies inside the timed region)
     e2e = None
-    if not args.no_e2e:
+    nbytes = V * 72 * (8 if prec == "f64" else 4)
+
+    def host_mem_available():
+        try:
+            return int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
+        except (OSError, StopIteration):
+            return 0
+
+    # every rank of the node pins its own copy of the field: leave the leg out (on all ranks alike) rather than run the
+    # host out of memory
+    e2e_fits = host_mem_available() > 1.25 * world * nbytes
+    if dist is not None:
+        flag = torch.tensor([1.0 if e2e_fits else 0.0], device="cuda")
+        dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+        e2e_fits = bool(flag.item() > 0.5)
+    if not args.no_e2e and not e2e_fits:
+        log(f"bench.py: e2e leg left out: {world} x {nbytes / 1e9:.1f} GB of pinned host memory do not fit")
+        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 16,
+               "skipped": "not enough host memory to pin one field per rank"}
+    if not args.no_e2e and e2e_fits:
         host = torch.empty((V, 4, 3, 3, 2), dtype=fx.dtype).pin_memory()
         host.copy_(canon)
         del canon
         torch.cuda.empty_cache()
         n_e2e = max(1, min(args.steps, args.e2e_steps))
-        nbytes = V * 72 * (8 if prec == "f64" else 4)
 
         # Two fields in flight (a user fixing a stream of configurations): a second context on its own stream with its
         # own pinned buffer, driven by a second host thread, so that one field's upload overlaps the other's sweeps or
         # download (PCIe is full duplex, the GPU has separate copy engines).  Every step of every lane still uploads
         # its inputs and downloads its result inside the timed region.
         lanes = [(fx, host)]
-        try:
-            avail = int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
-        except (OSError, StopIteration):
-            avail = 0
-        free_dev = torch.cuda.mem_get_info()[0]
-        while len(lanes) < args.e2e_lanes and avail > (len(lanes) + 2) * nbytes and \
+        avail = host_mem_available() / world  # this rank's share of what is left
+        while len(lanes) < args.e2e_lanes and avail > 2 * nbytes and \
                 torch.cuda.mem_get_info()[0] > 1.3 * nbytes:
             try:  # a lane that cannot get its memory is left out; the leg then runs with the lanes it has
                 s2 = torch.cuda.Stream()
