@@ -582,3 +582,26 @@ def test_8_real_storage_fix_and_unsupported_calls(gf, torch):
     assert gf.gf_slab_attach(fx.ctx, halo.data_ptr(), 4 * B) == gf.GF_EUNSUPPORTED
     fx.close()
     assert gf.gf_workspace_bytes(8, 8, 8, 8, gf.GF_FP32, 8) > 0
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("storage", [18, 12])
+def test_fp32_fast_path_on_a_smoothed_field(gf, torch, gauge, storage):
+    """With FP32 links the staged kernel evaluates a site in FP32 unless a subgroup's |r|^2 < 16.  On a
+    random start nearly every site takes the FP64 branch, so the one-sweep bound is checked here where the FP32 branch
+    does the work: the state after 30 sweeps (F ~ 0.7, |r|^2 ~ 100) is handed to the oracle and both take one more sweep."""
+    dims, omega = (16, 16, 16, 8), 1.75
+    U, _ = host_input(dims, 0.4, 77, "f32", storage)
+    fx = gpu_fixer(gf, torch, dims, gauge, "f32", storage, U)
+    fx.ovr_sweep(30, omega)
+    start = fx.get_links().cpu().numpy()
+    F, _ = fx.measure()
+    assert F > 0.6
+    fx.ovr_sweep(1, omega)
+    got = fx.get_links().cpu().numpy().astype(np.float64)
+    fx.close()
+    Uo = np.ascontiguousarray(start.astype(np.float64))
+    if storage == 12:
+        oracle.project12(Uo, dims)
+    oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
+    assert np.abs(got - Uo).max() <= TOL_LINK["f32"]
