@@ -397,14 +397,25 @@ __global__ void __launch_bounds__(SD_THREADS) sd_rotate_kernel(cplx_t<T>* __rest
   const size_t V = 2 * (size_t)g.vh;
   const Site s = site_of(g, parity, cb);
   const int lex = lex_of(g, s);
+  // the site's four links travel global -> shared with cp.async (no registers held) while g(x) is rebuilt from the
+  // packed field; a thread reads back only what it copied itself, so there is no barrier
+  extern __shared__ __align__(16) unsigned char rot_smem[];
+  C* sm = reinterpret_cast<C*>(rot_smem) + threadIdx.x;
+  C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
+#pragma unroll
+  for (int i = 0; i < 4 * NELEM; ++i) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm + i * SD_THREADS);
+    if (sizeof(C) == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(fwd + i * 32) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(fwd + i * 32) : "memory");
+  }
   C gx[9];
   rotation_from_packed<T>(w, V, lex, gx);
-  C* fwd = links + link_offset<NELEM>(g, parity, cb, 0);
+  asm volatile("cp.async.wait_all;" ::: "memory");
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
     C gup[9], u[9], v[9], o[9];
     rotation_from_packed<T>(w, V, lex_up(g, s, lex, mu), gup);
-    load_link<NELEM, true>(fwd + mu * NELEM * 32, u);
+    load_link<NELEM, true, SD_THREADS>(sm + mu * NELEM * SD_THREADS, u);
     mul_left<LinkRows<NELEM>::value>(gx, u, v);
     mul_right_adj<LinkRows<NELEM>::value>(v, gup, o);
     store_link<NELEM>(fwd + mu * NELEM * 32, o);
@@ -564,8 +575,11 @@ cudaError_t launch_sd_filter(const KernelArgs& a, void* w, const double* table, 
 template <class T, int NELEM>
 static cudaError_t sd_rotate_T(const KernelArgs& a, const void* w) {
   const int bpp = sd_num_partials(a.geo);
-  sd_rotate_kernel<T, NELEM><<<2 * bpp, SD_THREADS, 0, a.stream>>>((cplx_t<T>*)a.links, a.geo, (const cplx_t<T>*)w, bpp,
-                                                                   make_block_order(a.geo));
+  constexpr size_t SMEM = (size_t)4 * NELEM * SD_THREADS * sizeof(cplx_t<T>);
+  cudaError_t e = cudaFuncSetAttribute(sd_rotate_kernel<T, NELEM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+  if (e != cudaSuccess) return e;
+  sd_rotate_kernel<T, NELEM><<<2 * bpp, SD_THREADS, SMEM, a.stream>>>((cplx_t<T>*)a.links, a.geo, (const cplx_t<T>*)w, bpp,
+                                                                      make_block_order(a.geo));
   return cudaGetLastError();
 }
 
