@@ -897,8 +897,23 @@ int slab_wait(gf_ctx* c, unsigned epoch) {
     return fail(c, GF_ECUDA, "cuStreamWaitValue32 failed");
   return GF_OK;
 }
+// A group is closed if every neighbour of every slab is itself a slab of the group and all of them run on one stream
+// of one device (the whole lattice in one process): stream order already is the order the flags would enforce.
+bool group_is_closed(gf_ctx* const* slabs, int n) {
+  for (int s = 0; s < n; ++s) {
+    if (slabs[s]->k.stream != slabs[0]->k.stream || slabs[s]->device != slabs[0]->device) return false;
+    bool up = false, lo = false;
+    for (int r = 0; r < n; ++r) {
+      up = up || slabs[s]->upper_flag == slabs[r]->own_flags + 1;
+      lo = lo || slabs[s]->lower_flag == slabs[r]->own_flags;
+    }
+    if (!up || !lo) return false;
+  }
+  return true;
+}
 // one ordering point of the group with its neighbours (local or remote): every slab signals, then every slab waits
 int group_sync(gf_ctx* const* slabs, int n) {
+  if (group_is_closed(slabs, n)) return GF_OK;
   for (int s = 0; s < n; ++s)
     if (int rc = slab_signal(slabs[s], slabs[s]->epoch + 1); rc != GF_OK) return rc;
   for (int s = 0; s < n; ++s)
@@ -957,6 +972,7 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
   // sites of parity 1-p, which are visited next: the next launch reads them straight from that buffer, and only the
   // last half-sweep of the call (or one before a reunitarisation) is followed by gf_slab_unpack_top.
   bool pending = false;  // top-slice U_t of parity 0 still sits in the buffer the odd half-sweep filled
+  const bool closed = group_is_closed(slabs, n_slabs);  // no flags needed: one stream orders everything
   for (int i = 0; i < n_sweeps && rc == GF_OK; ++i) {
     for (int p = 0; p < 2 && rc == GF_OK; ++p) {  // even first
       // ONE kernel per slab and half-sweep: its border blocks come first, store both halo messages at their destination
@@ -969,13 +985,14 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
         if (p == 1) returned = c->top_in;
         else if (pending) returned = c->top_out;
         cudaError_t e = launch_halfsweep_slab_fused(c->k, p, omega, c->fwd_target[p], p ? c->ret_target_odd : c->ret_target,
-                                                    c->own_flags + 2, c->upper_flag, c->lower_flag, c->epoch + 1, returned);
+                                                    closed ? nullptr : c->own_flags + 2, c->upper_flag, c->lower_flag,
+                                                    c->epoch + 1, returned);
         if (e != cudaSuccess) { rc = fail_cuda(c, e, "gf_slab_group_sweep"); break; }
         c->epoch += 1;
         c->launches += 1;
         c->qblocks = 0;
       }
-      for (int s = 0; s < n_slabs && rc == GF_OK; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
+      for (int s = 0; s < n_slabs && rc == GF_OK && !closed; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
     }
     pending = true;
     const bool last = i == n_sweeps - 1;

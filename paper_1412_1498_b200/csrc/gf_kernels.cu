@@ -796,14 +796,14 @@ static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, doubl
   sv.nblocks0 = (g.s3 + THREADS - 1) / THREADS;
   sv.nblocks1 = sv.nblocks0;
   const int nblocks2 = sv.cb3_end > sv.cb3_begin ? (sv.cb3_end - sv.cb3_begin + THREADS - 1) / THREADS : 0;
-  sv.sig_blocks = sv.nblocks0 + sv.nblocks1;
+  sv.sig_blocks = counter ? sv.nblocks0 + sv.nblocks1 : 0;  // no counter: nobody to signal (a closed group on one stream)
   sv.sig_counter = counter;
   sv.sig_flag[0] = flag_up; sv.sig_flag[1] = flag_down;
   sv.sig_epoch = epoch;
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   sv.top_in_src = top_in_src;
-  kern<<<(unsigned)(sv.sig_blocks + nblocks2), THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0,
+  kern<<<(unsigned)(sv.nblocks0 + sv.nblocks1 + nblocks2), THREADS, SMEM, a.stream>>>((C*)a.links, a.geo, parity, (T)omega, nullptr, sv, 0,
                                                                           nullptr, nullptr);
   return cudaGetLastError();
 }
