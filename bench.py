@@ -695,6 +695,9 @@ def run_sharded(args):
     sh = gf.ShardedGaugeFixer(gdims, n_slabs, gauge=cfg["gauge"], prec=prec, storage=storage, device=f"cuda:{local}",
                               mode=args.sharded_mode or ("transport" if args.no_direct else None))
     sh.set_reunit_every(cfg["reunit_every"])
+    if args.force_flags:  # what a rank of a multi-rank run executes, timed in one process
+        for e in sh.engines.values():
+            e.fx.set_option(gf.GF_OPT_SLAB_FORCE_FLAGS, 1)
     links = {}
     for s in sh.slabs:  # every slab its own seeded field of the config's recipe (rougher across slab boundaries)
         e = sh.engines[s]
@@ -779,6 +782,8 @@ def main():
                     help="kernel study: SU(N) links (gf_create_sun) on the config's lattice, host generator (use cfg2 or smaller)")
     ap.add_argument("--defer", action="store_true", help="kernel study: Coulomb gauge with deferred temporal links (gf_defer_*)")
     ap.add_argument("--no-direct", action="store_true", help="--sharded: halo messages through the transport even in one process")
+    ap.add_argument("--force-flags", action="store_true",
+                    help="--sharded: signal / wait through the flags even where one stream orders all slabs")
     ap.add_argument("--sharded-mode", default="", choices=["", "flags", "ipc", "events", "transport"],
                     help="--sharded: ShardedGaugeFixer mode (default: flags on GPUs)")
     ap.add_argument("--peaks", action="store_true", help="print the measured FP64 / FP32 FMA-chain peaks and exit")

@@ -179,8 +179,10 @@ enum {
                                N = 1..16: the binomial series sum_{n<=N} binom(omega,n) (g-1)^n, normalised back to
                                SU(2) - the way ref. [1] of the paper evaluates g^omega (reading A21).
                                Default sweep variant only; GF_EUNSUPPORTED on a slab context. */
-  GF_OPT_DOMAIN8_CHECK = 8  /* 1 (default): storage = 8 reports links outside its validity domain (above); 0: the
+  GF_OPT_DOMAIN8_CHECK = 8, /* 1 (default): storage = 8 reports links outside its validity domain (above); 0: the
                                flag is ignored (kernel studies on rough fields only) */
+  GF_OPT_SLAB_FORCE_FLAGS = 9 /* 1: gf_slab_group_sweep signals and waits even where one stream already orders a closed
+                               group (to time, in one process, what a rank of a multi-rank run executes) */
 };
 int gf_set_option(gf_ctx* ctx, int key, int value);
 
@@ -276,8 +278,9 @@ int gf_ipc_close(void* dev_ptr, size_t offset);
  * and synchronises the stream; every slab of a lattice must have made it before any of them is swept.
  * gf_slab_group_sweep(slabs, n, n_sweeps, omega, reunit_every, sweeps_before): n_sweeps sweeps of the n local slabs (all
  * with peer targets and flags set; neighbours inside or outside the group): per half-sweep p ONE kernel per slab - its
- * border blocks come first, store both halo messages at their destination, and the last of them writes the epoch into
- * the neighbours' words (system scope) while the rest of the grid updates the interior -, then the slab's wait and
+ * border blocks come first, store both halo messages at their destination, and the last of them adds 1 to both
+ * neighbours' arrival counters (own_flags + 12, system-scope atomic) while the rest of the grid updates the interior -,
+ * then ONE stream-ordered wait of the slab on its own counter and
  * gf_slab_unpack_top(1-p); after global sweep number s =
  * sweeps_before + i with reunit_every > 0 and s % reunit_every == 0 every link is reunitarised and the ghost buffers are
  * refreshed.  Asynchronous.  EVERY rank of the lattice must make the same call (same n_sweeps, reunit

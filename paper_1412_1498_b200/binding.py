@@ -16,7 +16,7 @@ GF_LANDAU, GF_COULOMB = 0, 1
 GF_FP64, GF_FP32 = 0, 1
 GF_OK, GF_EINVAL, GF_EODD, GF_EUNSUPPORTED, GF_ENOMEM, GF_ECUDA, GF_ENUMERIC = 0, -1, -2, -3, -4, -5, -6
 GF_OPT_SWEEP_VARIANT, GF_OPT_BLOCK_THREADS, GF_OPT_FUSE_MEASURE, GF_OPT_FFT_ACCELERATE, GF_OPT_FFT_FUSED_T = 1, 2, 3, 4, 5
-GF_OPT_FFT_OWN, GF_OPT_OVR_SERIES, GF_OPT_DOMAIN8_CHECK = 6, 7, 8
+GF_OPT_FFT_OWN, GF_OPT_OVR_SERIES, GF_OPT_DOMAIN8_CHECK, GF_OPT_SLAB_FORCE_FLAGS = 6, 7, 8, 9
 
 SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "gf_set_links_host",
            "gf_get_links_host", "gf_ovr_sweep", "gf_measure", "gf_fix", "gf_get_history", "gf_reunitarize",

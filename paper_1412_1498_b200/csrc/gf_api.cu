@@ -72,6 +72,7 @@ struct gf_ctx {
   int reunit_every;
   int fuse_measure;  // GF_OPT_FUSE_MEASURE
   int domain8_check;  // GF_OPT_DOMAIN8_CHECK
+  int slab_force_flags;  // GF_OPT_SLAB_FORCE_FLAGS
   int qblocks;       // > 0: k.qpartials[0..qblocks) hold the odd sites' theta terms of the links as they stand
   long long sweeps_total;  // sweeps since the last gf_set_links (reunitarisation cadence)
   long long launches;
@@ -98,7 +99,8 @@ struct gf_ctx {
   unsigned* own_flags;     // [0] written by the upper neighbour, [1] by the lower one (device memory of this slab)
   unsigned* upper_flag;    // the upper neighbour's own_flags[1] (this process's or a CUDA-IPC mapping)
   unsigned* lower_flag;    // the lower neighbour's own_flags[0]
-  unsigned epoch;          // last epoch signalled
+  unsigned epoch;          // last epoch signalled by stream memory operations (entry / refresh synchronisation)
+  unsigned arrivals;       // 2 x the fused launches so far: what own_flags[3] must reach (both neighbours add 1 per launch)
   char err[256];
 };
 
@@ -200,7 +202,7 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->k.counter = base + sz.links + sz.partials + sz.qpartials;  // the workspace's result slot holds the counter
   c->staging[0] = base + sz.links + sz.partials + sz.qpartials + sz.result;
   c->staging[1] = c->staging[0] + sz.staging;
-  c->fuse_measure = 1; c->qblocks = 0; c->domain8_check = 1;
+  c->fuse_measure = 1; c->qblocks = 0; c->domain8_check = 1; c->slab_force_flags = 0;
   c->reunit_every = 0; c->sweeps_total = 0; c->launches = 0; c->history_n = 0;
   c->err[0] = 0;
   c->fft = nullptr; c->fft_w = nullptr; c->fft_table = nullptr; c->fft_accelerate = 1; c->fft_fused_t = 0; c->fft_own = 1; c->own_table = nullptr;
@@ -213,6 +215,7 @@ static int create_ctx(gf_ctx** out, int ncolors, int nx, int ny, int nz, int nt,
   c->alt_top_in = false;
   c->own_flags = c->upper_flag = c->lower_flag = nullptr;
   c->epoch = 0;
+  c->arrivals = 0;
   c->host_result = nullptr;
   c->host_slices = c->dev_slices = nullptr;
   c->defer_acc = nullptr; c->defer_dirty = false;
@@ -445,6 +448,9 @@ int gf_set_option(gf_ctx* c, int key, int value) {
       return GF_OK;
     case GF_OPT_DOMAIN8_CHECK:
       c->domain8_check = value != 0;
+      return GF_OK;
+    case GF_OPT_SLAB_FORCE_FLAGS:
+      c->slab_force_flags = value != 0;
       return GF_OK;
     case GF_OPT_BLOCK_THREADS:
       if (value < 0 || value % 32 || value > 1024) return fail(c, GF_EINVAL, "gf_set_option: bad block size");
@@ -901,7 +907,8 @@ int slab_wait(gf_ctx* c, unsigned epoch) {
 // of one device (the whole lattice in one process): stream order already is the order the flags would enforce.
 bool group_is_closed(gf_ctx* const* slabs, int n) {
   for (int s = 0; s < n; ++s) {
-    if (slabs[s]->k.stream != slabs[0]->k.stream || slabs[s]->device != slabs[0]->device) return false;
+    if (slabs[s]->k.stream != slabs[0]->k.stream || slabs[s]->device != slabs[0]->device || slabs[s]->slab_force_flags)
+      return false;
     bool up = false, lo = false;
     for (int r = 0; r < n; ++r) {
       up = up || slabs[s]->upper_flag == slabs[r]->own_flags + 1;
@@ -910,6 +917,16 @@ bool group_is_closed(gf_ctx* const* slabs, int n) {
     if (!up || !lo) return false;
   }
   return true;
+}
+// the slab's stream goes on once both neighbours' border blocks of the current fused launch have stored: each adds 1 to
+// own_flags[3] from inside its kernel (system-scope atomic), so ONE wait covers both
+int slab_wait_arrivals(gf_ctx* c) {
+  static stream_memop_fn wait32 = driver_memop("cuStreamWaitValue32");
+  if (!wait32) return fail(c, GF_ECUDA, "cuStreamWaitValue32 is not available");
+  DeviceGuard guard(c);
+  if (wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[3], c->arrivals, 0 /* GEQ */) != 0)
+    return fail(c, GF_ECUDA, "cuStreamWaitValue32 failed");
+  return GF_OK;
 }
 // one ordering point of the group with its neighbours (local or remote): every slab signals, then every slab waits
 int group_sync(gf_ctx* const* slabs, int n) {
@@ -926,7 +943,8 @@ int group_check(gf_ctx* const* slabs, int n, const char* who) {
     gf_ctx* c = slabs[s];
     if (!c) return GF_EINVAL;
     if (!c->k.slab.ghost || !c->alt_top_in || !c->own_flags) return fail(c, GF_EINVAL, who);
-    if (c->epoch != slabs[0]->epoch) return fail(c, GF_EINVAL, "the slabs of a group must have been driven together");
+    if (c->epoch != slabs[0]->epoch || c->arrivals != slabs[0]->arrivals)
+      return fail(c, GF_EINVAL, "the slabs of a group must have been driven together");
   }
   return GF_OK;
 }
@@ -949,6 +967,7 @@ int gf_slab_set_peer_flags(gf_ctx* c, void* own_flags, void* upper_flag, void* l
   c->upper_flag = (unsigned*)upper_flag;
   c->lower_flag = (unsigned*)lower_flag;
   c->epoch = 0;
+  c->arrivals = 0;
   cudaError_t e = cudaMemsetAsync(own_flags, 0, 4 * sizeof(unsigned), c->k.stream);  // two flag words + the block counter
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);  // zero before any neighbour can signal
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_set_peer_flags");
@@ -985,14 +1004,14 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
         if (p == 1) returned = c->top_in;
         else if (pending) returned = c->top_out;
         cudaError_t e = launch_halfsweep_slab_fused(c->k, p, omega, c->fwd_target[p], p ? c->ret_target_odd : c->ret_target,
-                                                    closed ? nullptr : c->own_flags + 2, c->upper_flag, c->lower_flag,
-                                                    c->epoch + 1, returned);
+                                                    closed ? nullptr : c->own_flags + 2, c->upper_flag + 2, c->lower_flag + 3,
+                                                    returned);
         if (e != cudaSuccess) { rc = fail_cuda(c, e, "gf_slab_group_sweep"); break; }
-        c->epoch += 1;
+        c->arrivals += 2;
         c->launches += 1;
         c->qblocks = 0;
       }
-      for (int s = 0; s < n_slabs && rc == GF_OK && !closed; ++s) rc = slab_wait(slabs[s], slabs[s]->epoch);
+      for (int s = 0; s < n_slabs && rc == GF_OK && !closed; ++s) rc = slab_wait_arrivals(slabs[s]);
     }
     pending = true;
     const bool last = i == n_sweeps - 1;

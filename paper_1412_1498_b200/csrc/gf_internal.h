@@ -21,8 +21,7 @@ struct SlabView {
   int cb3_begin, cb3_end;  // third range (the interior); empty if cb3_end <= cb3_begin
   int sig_blocks;          // 0: no signal
   unsigned* sig_counter;   // zero between launches
-  unsigned* sig_flag[2];
-  unsigned sig_epoch;
+  unsigned* sig_flag[2];   // the neighbours' arrival counters: each gets +1 (system-scope atomic)
   // non-null: the top-slice sites take U_t(x) from this message buffer (what the upper neighbour's last half-sweep
   // returned) instead of from the field - the unpack kernel between two half-sweeps is then not needed
   const void* top_in_src;
@@ -59,11 +58,10 @@ bool halfsweep_can_fuse_theta(const KernelArgs& a);
 cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega, int cb_begin, int cb_end,
                                   int cb2_begin, int cb2_end, void* top_out, void* ret_out);
 // The whole half-sweep of a slab in ONE launch: bottom slice, top slice (both deliver their halo messages to top_out /
-// ret_out), then the interior; the border blocks come first in the grid, and the last of them to finish writes `epoch`
-// into the two flag words (system scope), so the neighbours can go on while the interior is still being updated.
+// ret_out), then the interior; the border blocks come first in the grid, and the last of them to finish adds 1 to the
+// two neighbours' arrival counters (system-scope atomics), so the neighbours can go on while the interior is still being updated.
 cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
-                                        const void* top_in_src);
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, const void* top_in_src);
 // U_t of the `parity` sites of the top time slice -> buf (pack) or buf -> those links (unpack); buf: one parity, ghost layout
 cudaError_t launch_slab_top(const KernelArgs& a, int parity, void* buf, bool pack);
 int halfsweep_max_qblocks(const Geo& g);

@@ -607,8 +607,8 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
       if (atomicAdd(sv.sig_counter, 1u) == (unsigned)sv.sig_blocks - 1u) {
         *sv.sig_counter = 0u;  // ready for the next launch on this stream
         __threadfence_system();
-        *reinterpret_cast<volatile unsigned*>(sv.sig_flag[0]) = sv.sig_epoch;
-        *reinterpret_cast<volatile unsigned*>(sv.sig_flag[1]) = sv.sig_epoch;
+        atomicAdd_system(sv.sig_flag[0], 1u);
+        atomicAdd_system(sv.sig_flag[1], 1u);
       }
     }
   }
@@ -780,8 +780,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
 
 template <class T, int NELEM, int ND>
 static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                          unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
-                                          const void* top_in_src) {
+                                          unsigned* counter, unsigned* flag_up, unsigned* flag_down, const void* top_in_src) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
   constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
@@ -799,7 +798,6 @@ static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, doubl
   sv.sig_blocks = counter ? sv.nblocks0 + sv.nblocks1 : 0;  // no counter: nobody to signal (a closed group on one stream)
   sv.sig_counter = counter;
   sv.sig_flag[0] = flag_up; sv.sig_flag[1] = flag_down;
-  sv.sig_epoch = epoch;
   sv.top_out = top_out;
   sv.ret_out = ret_out;
   sv.top_in_src = top_in_src;
@@ -983,9 +981,8 @@ cudaError_t launch_halfsweep_slab(const KernelArgs& a, int parity, double omega,
 }
 
 cudaError_t launch_halfsweep_slab_fused(const KernelArgs& a, int parity, double omega, void* top_out, void* ret_out,
-                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, unsigned epoch,
-                                        const void* top_in_src) {
-  GF_DISPATCH(halfsweep_slab_fused_T, a, parity, omega, top_out, ret_out, counter, flag_up, flag_down, epoch, top_in_src);
+                                        unsigned* counter, unsigned* flag_up, unsigned* flag_down, const void* top_in_src) {
+  GF_DISPATCH(halfsweep_slab_fused_T, a, parity, omega, top_out, ret_out, counter, flag_up, flag_down, top_in_src);
 }
 
 // ---- top time slice of a slab <-> message buffer (ghost layout of one parity) ------------------------------------------
