@@ -73,9 +73,9 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def halfsweep_kernel_name(storage, variant, defer=False, sites_per_parity=1 << 30):
+def halfsweep_kernel_name(storage, variant, defer=False, sites_per_parity=1 << 30, prec="f64"):
     """The kernel gf_ovr_sweep launches for this storage format / GF_OPT_SWEEP_VARIANT (csrc/gf_kernels.cu, halfsweep_T)."""
-    v = variant or 3
+    v = variant or (5 if prec == "f64" and storage != 8 and not defer else 3)
     return {1: "ovr_halfsweep_kernel", 2: "ovr_halfsweep_kernel (L2 bulk prefetch)", 3: "ovr_halfsweep_staged_kernel",
             4: "ovr_halfsweep_staged_kernel<BULK=1> (TMA bulk copies)",
             5: "ovr_halfsweep_staged_kernel<BULK=2> (forward chunk by TMA bulk copy)",
@@ -395,7 +395,7 @@ def run_ours(args):
     # the reunitarisation launches inside the sweep region (config 2 only) are subtracted at their algorithmic cost
     ms_half = (ms_sweeps - n_reunit * (8 * V * L) / (peak * 1e9) * 1e3) / n_half
     achieved = bytes_per_launch / (ms_half * 1e-3) / 1e9
-    kernel = halfsweep_kernel_name(storage, args.variant, args.defer, V // 2) if N == 3 else f"halfsweep_sun_kernel<N={N}>"
+    kernel = halfsweep_kernel_name(storage, args.variant, args.defer, V // 2, prec) if N == 3 else f"halfsweep_sun_kernel<N={N}>"
     traffic, traffic_src = ncu_traffic(cfg["name"], kernel) if not (args.storage or args.gauge or args.defer or args.prec or N != 3) else (None, None)
     # flops leg: the FMA-chain peaks measured now, on this GPU, under the clocks it runs at after
     # the timed region (gf_peak_fma); the site rotation is FP64 in both storage precisions, the link products are in

@@ -155,7 +155,7 @@ int gf_set_reunit_every(gf_ctx* ctx, int k);
 
 /* Tuning knobs for benchmarking kernel variants; the defaults are the fastest measured.  GF_EINVAL on unknown keys. */
 enum {
-  GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (= 3); 1 = two-pass; 2 = two-pass + L2
+  GF_OPT_SWEEP_VARIANT = 1, /* half-sweep kernel: 0 = default (5 with FP64 links, 3 with FP32 links or 8-real storage); 1 = two-pass; 2 = two-pass + L2
                                bulk prefetch; 3 = staged through shared memory with cp.async; 4 = staged, the tile
                                fetched by bulk copies of the TMA unit (cp.async.bulk on an mbarrier); 5 = staged, only
                                the contiguous forward chunk by bulk copy; 6 = two warps per 32 sites (forward / backward links; a study, never
