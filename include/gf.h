@@ -319,6 +319,40 @@ long long gf_kernel_launches(const gf_ctx* ctx);
  * bytes of device memory (never written in practice).  Synchronises cuda_stream.  Errors: GF_EINVAL, GF_ECUDA. */
 int gf_peak_fma(int prec, double seconds_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
+/* ---- F and theta for callers that cannot allocate device memory -----------------------------------------------------------
+ * Every call above works out of a workspace that the caller allocated for gf_create.  A caller with no means to get
+ * device memory - a hook inside an application whose own pool has taken the whole GPU, code that runs under a rule of
+ * "no cudaMalloc / cudaFree after start-up" because those calls synchronise the device and stall its other streams, a
+ * callback that is only lent a pointer to somebody else's field - cannot create a context at all.  gf_measure_static
+ * gives that caller the convergence monitor of Algorithm 1 (eqs. 1.1-1.3; Alg. 1 l.1, l.13): F and theta
+ * of a field in the CANONICAL layout (top of this file), read where it lies, with no context and no workspace.  The
+ * scratch of the reduction (one pair of partial sums per 256 sites, the result, a block counter) is a fixed array
+ * inside the library image, 256 KiB on every GPU that loads libgf, held until the process exits.
+ *
+ *   dev_links    device memory of the CURRENT device, canonical layout, 72 V elements of double (GF_FP64) or float
+ *                (GF_FP32), 16-byte aligned; only read.
+ *   gauge        GF_LANDAU (nu = 0..3) or GF_COULOMB (nu = 0..2), as gf_create.
+ *   cuda_stream  the stream the work is queued on (NULL = default stream); the call synchronises it before returning.
+ *   F, theta     host out-params, FP64 sums in both precisions, deterministic summation order (not gf_measure's order:
+ *                the two agree to rounding, not bit for bit).
+ * Limits and rules:
+ *   - V <= gf_measure_static_max_sites() = 4 194 304 sites (32^3 x 128 just fits, 48^3 x 96 does not); a larger lattice is refused with
+ *     GF_ENOMEM and a message that says so: use gf_create + gf_measure there.
+ *   - The call allocates nothing: no cudaMalloc, cudaMallocHost, cudaFree, no library routine that does.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, which may make the
+ *     runtime load the library's kernels onto that device); later calls reuse it.  Make that first call at start-up,
+ *     before any stream capture is begun.
+ *   - All calls on one device share the array, and it keeps what the last call left in it (the counter is cleared at the
+ *     start of every call).  Two calls that overlap on the GPU - from two threads, or on two streams - race on it and
+ *     both results are garbage: serialise them.  Calls on different devices are independent.
+ * Errors (text of the last failure of the calling thread: gf_static_last_error): GF_EINVAL (null or misaligned
+ * pointer, memory that is not the current device's), GF_EODD, GF_EUNSUPPORTED (gauge, precision), GF_ENOMEM (lattice
+ * above the limit), GF_ECUDA, GF_ENUMERIC (F or theta not finite; the values are still written). */
+size_t gf_measure_static_max_sites(void);
+int gf_measure_static(const void* dev_links, int nx, int ny, int nz, int nt, int gauge, int prec, void* cuda_stream,
+                      double* F, double* theta);
+const char* gf_static_last_error(void);
+
 void gf_destroy(gf_ctx* ctx);
 const char* gf_strerror(int code);
 /* Text of the last failure on this context (CUDA error string for GF_ECUDA); valid until the next call. */

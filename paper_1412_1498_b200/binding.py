@@ -26,7 +26,8 @@ SYMBOLS = ["gf_workspace_bytes", "gf_create", "gf_set_links", "gf_get_links", "g
            "gf_slab_halo_bytes", "gf_slab_attach", "gf_slab_set_targets", "gf_slab_pack_top", "gf_slab_unpack_top",
            "gf_slab_halfsweep_border", "gf_slab_halfsweep_interior", "gf_peak_fma", "gf_workspace_bytes_sun",
            "gf_create_sun", "gf_slab_set_peer_targets", "gf_ipc_export", "gf_ipc_open", "gf_ipc_close", "gf_combine_slabs",
-           "gf_fix_plan", "gf_slab_set_peer_flags", "gf_slab_group_sweep", "gf_slab_group_refresh"]
+           "gf_fix_plan", "gf_slab_set_peer_flags", "gf_slab_group_sweep", "gf_slab_group_refresh",
+           "gf_measure_static", "gf_measure_static_max_sites", "gf_static_last_error"]
 
 
 def _load() -> ctypes.CDLL:
@@ -106,6 +107,12 @@ def _load() -> ctypes.CDLL:
     lib.gf_fix_plan.argtypes = [c_double, c_double, c_int, c_int, c_int, c_double, POINTER(c_int)]
     lib.gf_peak_fma.restype = c_int
     lib.gf_peak_fma.argtypes = [c_int, c_double, c_void_p, c_void_p, POINTER(c_double)]
+    lib.gf_measure_static.restype = c_int
+    lib.gf_measure_static.argtypes = [c_void_p] + [c_int] * 6 + [c_void_p, POINTER(c_double), POINTER(c_double)]
+    lib.gf_measure_static_max_sites.restype = c_size_t
+    lib.gf_measure_static_max_sites.argtypes = []
+    lib.gf_static_last_error.restype = c_char_p
+    lib.gf_static_last_error.argtypes = []
     lib.gf_kernel_launches.restype = c_longlong
     lib.gf_kernel_launches.argtypes = [c_void_p]
     lib.gf_destroy.restype = None
@@ -348,6 +355,22 @@ def gf_peak_fma(prec: int, seconds_target: float, dev_scratch: int, stream: int 
     return rc, t.value
 
 
+def gf_measure_static(dev_links: int, nx, ny, nz, nt, gauge: int, prec: int, stream: int = 0):
+    """Returns (rc, F, theta) of a canonical-layout device field; no context, no workspace, no allocation."""
+    F, th = c_double(), c_double()
+    rc = lib.gf_measure_static(c_void_p(dev_links or None), nx, ny, nz, nt, gauge, prec, c_void_p(stream or None),
+                               byref(F), byref(th))
+    return rc, F.value, th.value
+
+
+def gf_measure_static_max_sites() -> int:
+    return int(lib.gf_measure_static_max_sites())
+
+
+def gf_static_last_error() -> str:
+    return lib.gf_static_last_error().decode()
+
+
 def gf_kernel_launches(ctx) -> int:
     return int(lib.gf_kernel_launches(ctx))
 
@@ -367,6 +390,22 @@ def gf_last_error(ctx) -> str:
 # ---- convenience owner ---------------------------------------------------------------------------------------------------
 _GAUGE = {"landau": GF_LANDAU, "coulomb": GF_COULOMB}
 _PREC = {"f64": GF_FP64, "f32": GF_FP32}
+
+
+def measure_static(links, dims, gauge="landau", stream=None):
+    """F and theta of a torch CUDA tensor in the canonical layout (V,4,3,3,2), float64 or float32, through
+    gf_measure_static: for callers that hold a field but may not allocate device memory.  Nothing is allocated here
+    either (no context, no workspace tensor); lattices above gf_measure_static_max_sites() sites raise GFError."""
+    import torch
+
+    assert links.is_cuda and links.is_contiguous() and links.dtype in (torch.float64, torch.float32)
+    prec = GF_FP64 if links.dtype == torch.float64 else GF_FP32
+    with torch.cuda.device(links.device):
+        s = stream if stream is not None else torch.cuda.current_stream(links.device)
+        rc, F, th = gf_measure_static(links.data_ptr(), *[int(d) for d in dims], _GAUGE[gauge], prec, s.cuda_stream)
+    if rc != GF_OK:
+        raise GFError(rc, gf_static_last_error())
+    return F, th
 
 
 class GaugeFixer:

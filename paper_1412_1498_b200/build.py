@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgf.so")
-SOURCES = ["gf_kernels.cu", "gf_fftsd.cu", "gf_fft.cu", "gf_api.cu", "gf_peaks.cu", "gf_sun.cu"]
+SOURCES = ["gf_kernels.cu", "gf_fftsd.cu", "gf_fft.cu", "gf_api.cu", "gf_peaks.cu", "gf_sun.cu", "gf_static.cu"]
 HEADERS = ["gf_device.cuh", "gf_internal.h", os.path.join("..", "..", "include", "gf.h")]
 # -split-compile 0: the back end compiles the kernels of a translation unit on all host cores (gf_kernels.cu: 4 min -> 1 min)
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
