@@ -269,7 +269,7 @@ int gf_ipc_open(const unsigned char* handle64, size_t offset, void** dev_ptr);
 int gf_ipc_close(void* dev_ptr, size_t offset);
 
 /* The whole sharded sweep behind one call, synchronised with the neighbours by flags instead of host waits or
- * collectives.  gf_slab_set_peer_flags: own_flags = 16 bytes (16-byte aligned) of this slab's device memory (inside the allocation that is
+ * collectives.  gf_slab_set_peer_flags: own_flags = 32 bytes (32-byte aligned) of this slab's device memory (inside the allocation that is
  * exported with gf_ipc_export, e.g. behind the 4B bytes of the halo workspace); upper_flag = the address of the UPPER
  * neighbour's own_flags + 4 (its "written by my lower neighbour" word), lower_flag = the LOWER neighbour's own_flags + 0;
  * addresses of this process or CUDA-IPC mappings.  A slab signals by a stream-ordered 32-bit write of an epoch counter
@@ -278,10 +278,11 @@ int gf_ipc_close(void* dev_ptr, size_t offset);
  * and synchronises the stream; every slab of a lattice must have made it before any of them is swept.
  * gf_slab_group_sweep(slabs, n, n_sweeps, omega, reunit_every, sweeps_before): n_sweeps sweeps of the n local slabs (all
  * with peer targets and flags set; neighbours inside or outside the group): per half-sweep p ONE kernel per slab - its
- * border blocks come first, store both halo messages at their destination, and the last of them adds 1 to both
- * neighbours' arrival counters (own_flags + 12, system-scope atomic) while the rest of the grid updates the interior -,
- * then ONE stream-ordered wait of the slab on its own counter and
- * gf_slab_unpack_top(1-p); after global sweep number s =
+ * border blocks come first, store both halo messages at their destination, and the last of them adds 1 to the arrival
+ * counter each neighbour keeps for it (the upper neighbour's own_flags + 16 "from below", the lower one's own_flags + 12
+ * "from above"; system-scope atomics) while the rest of the grid updates the interior -, then two stream-ordered waits
+ * of the slab, one on each of its own two counters (one counter per neighbour: a sum of the two could be reached by one
+ * neighbour running a launch ahead while the other has not arrived), and gf_slab_unpack_top(1-p); after global sweep number s =
  * sweeps_before + i with reunit_every > 0 and s % reunit_every == 0 every link is reunitarised and the ghost buffers are
  * refreshed.  Asynchronous.  EVERY rank of the lattice must make the same call (same n_sweeps, reunit
  * cadence), else the waits never complete.  gf_slab_group_refresh: fills the neighbours' ghost buffers from the group's top

@@ -100,7 +100,7 @@ struct gf_ctx {
   unsigned* upper_flag;    // the upper neighbour's own_flags[1] (this process's or a CUDA-IPC mapping)
   unsigned* lower_flag;    // the lower neighbour's own_flags[0]
   unsigned epoch;          // last epoch signalled by stream memory operations (entry / refresh synchronisation)
-  unsigned arrivals;       // 2 x the fused launches so far: what own_flags[3] must reach (both neighbours add 1 per launch)
+  unsigned arrivals;       // the fused launches so far: what own_flags[3] (upper neighbour) and own_flags[4] (lower) must reach
   char err[256];
 };
 
@@ -918,13 +918,17 @@ bool group_is_closed(gf_ctx* const* slabs, int n) {
   }
   return true;
 }
-// the slab's stream goes on once both neighbours' border blocks of the current fused launch have stored: each adds 1 to
-// own_flags[3] from inside its kernel (system-scope atomic), so ONE wait covers both
+// the slab's stream goes on once both neighbours' border blocks of the current fused launch have stored: from inside its
+// kernel (system-scope atomic) the upper neighbour adds 1 to own_flags[3], the lower one to own_flags[4].  One word per
+// neighbour, one wait per word: a single summed counter cannot tell "both at launch n" from "one at n+1, the other at
+// n-1", a state a ring of four or more slabs on different streams or ranks does reach (a slab's launch n+1 needs only ITS
+// neighbours at n), and the slab between the two would read a ghost buffer its late neighbour has not written yet.
 int slab_wait_arrivals(gf_ctx* c) {
   static stream_memop_fn wait32 = driver_memop("cuStreamWaitValue32");
   if (!wait32) return fail(c, GF_ECUDA, "cuStreamWaitValue32 is not available");
   DeviceGuard guard(c);
-  if (wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[3], c->arrivals, 0 /* GEQ */) != 0)
+  if (wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[3], c->arrivals, 0 /* GEQ */) != 0 ||
+      wait32(c->k.stream, (unsigned long long)(uintptr_t)&c->own_flags[4], c->arrivals, 0) != 0)
     return fail(c, GF_ECUDA, "cuStreamWaitValue32 failed");
   return GF_OK;
 }
@@ -961,14 +965,15 @@ int group_refresh(gf_ctx* const* slabs, int n) {
 int gf_slab_set_peer_flags(gf_ctx* c, void* own_flags, void* upper_flag, void* lower_flag) {
   GF_ENTER(c);
   if (!c->k.slab.ghost) return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: no halo workspace attached (gf_slab_attach)");
-  if (!own_flags || !upper_flag || !lower_flag || ((uintptr_t)own_flags % 16))
+  if (!own_flags || !upper_flag || !lower_flag || ((uintptr_t)own_flags % 32))
     return fail(c, GF_EINVAL, "gf_slab_set_peer_flags: null or misaligned flag address");
   c->own_flags = (unsigned*)own_flags;
   c->upper_flag = (unsigned*)upper_flag;
   c->lower_flag = (unsigned*)lower_flag;
   c->epoch = 0;
   c->arrivals = 0;
-  cudaError_t e = cudaMemsetAsync(own_flags, 0, 4 * sizeof(unsigned), c->k.stream);  // two flag words + the block counter
+  // two epoch words, the border-block counter, two arrival counters (3 words of padding)
+  cudaError_t e = cudaMemsetAsync(own_flags, 0, 8 * sizeof(unsigned), c->k.stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->k.stream);  // zero before any neighbour can signal
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_slab_set_peer_flags");
   return GF_OK;
@@ -1004,10 +1009,11 @@ int gf_slab_group_sweep(gf_ctx* const* slabs, int n_slabs, int n_sweeps, double 
         if (p == 1) returned = c->top_in;
         else if (pending) returned = c->top_out;
         cudaError_t e = launch_halfsweep_slab_fused(c->k, p, omega, c->fwd_target[p], p ? c->ret_target_odd : c->ret_target,
-                                                    closed ? nullptr : c->own_flags + 2, c->upper_flag + 2, c->lower_flag + 3,
-                                                    returned);
+                                                    closed ? nullptr : c->own_flags + 2,
+                                                    c->upper_flag + 3 /* its own_flags[4]: from below */,
+                                                    c->lower_flag + 3 /* its own_flags[3]: from above */, returned);
         if (e != cudaSuccess) { rc = fail_cuda(c, e, "gf_slab_group_sweep"); break; }
-        c->arrivals += 2;
+        c->arrivals += 1;
         c->launches += 1;
         c->qblocks = 0;
       }

@@ -155,12 +155,15 @@ class ShardedGaugeFixer:
       "ipc": the same delivery, ranks ordered by a one-element all-reduce (NCCL) or a barrier (gloo) per half-sweep.
       "events": all slabs in this process, delivery by plain pointers, kernels ordered by CUDA events (round 1).
       "transport": device copies within a process, torch.distributed send / recv between ranks.
+    slab_streams: None = every local slab on the current stream; "own" = each local slab on a CUDA stream of its own, so
+      that the kernels of neighbouring slabs of ONE process overlap on the device the way those of neighbouring ranks do
+      and every ordering between them goes through the flags (what the multi-rank schedule is tested with on one GPU).
     direct (older spelling): True = "events" / "ipc", False = "transport".  (device=None with an engine_factory is the seam the CPU schedule test uses to
     drive this schedule with host-side slabs.)
     """
 
     def __init__(self, dims, n_slabs, gauge="landau", prec="f64", storage=18, device="cuda:0", group=None,
-                 engine_factory=None, direct=None, mode=None):
+                 engine_factory=None, direct=None, mode=None, slab_streams=None):
         import torch
 
         self.torch = torch
@@ -185,9 +188,16 @@ class ShardedGaugeFixer:
         self.slabs = local_slabs(self.rank, self.n_slabs, self.world)
         self.device = torch.device(device) if device is not None else torch.device("cpu")
         self.on_gpu = self.device.type == "cuda"
+        if slab_streams not in (None, "own"):
+            raise ValueError("slab_streams must be None or 'own'")
+        self.own_streams = slab_streams == "own"
         if engine_factory is None:
             def engine_factory(local_dims, slab):
-                return GpuSlabEngine(local_dims, gauge, prec, storage, self.device)
+                stream = None
+                if self.own_streams:
+                    with torch.cuda.device(self.device):
+                        stream = torch.cuda.Stream(self.device)
+                return GpuSlabEngine(local_dims, gauge, prec, storage, self.device, stream=stream)
         self.engines = {s: engine_factory(self.local_dims, s) for s in self.slabs}
         self.comm_stream = None
         if self.on_gpu:
@@ -378,6 +388,8 @@ class ShardedGaugeFixer:
     # ---- links in / out ---------------------------------------------------------------------------------------------------
     def set_links(self, links_by_slab):
         """links_by_slab: {slab: canonical (V_local,4,3,3,2) tensor} for the local slabs."""
+        if self.own_streams:  # the tensors were produced on the caller's stream, the slabs read them on theirs
+            self.torch.cuda.current_stream(self.device).synchronize()
         for s in self.slabs:
             self.engines[s].set_links(links_by_slab[s])
         self.sweeps_total = 0
@@ -389,7 +401,10 @@ class ShardedGaugeFixer:
         self.set_links({s: links[s * V:(s + 1) * V].contiguous() for s in self.slabs})
 
     def get_links(self):
-        return {s: self.engines[s].get_links() for s in self.slabs}
+        out = {s: self.engines[s].get_links() for s in self.slabs}
+        if self.own_streams:  # written on the slabs' streams, read by the caller on its own
+            self.synchronize()
+        return out
 
     # ---- Algorithm 1 ---------------------------------------------------------------------------------------------------------
     def half_sweep(self, p, omega):

@@ -150,3 +150,126 @@ def test_slab_abi_errors(gf, torch):
     for f in (gf.gf_slab_pack_top, gf.gf_slab_unpack_top):
         assert f(None, 0) == gf.GF_EINVAL
     fx.close()
+
+
+# ---- the multi-rank schedule under real concurrency, on one GPU ------------------------------------------------------------
+# Every slab of ONE process on a CUDA stream of its own (slab_streams="own"): the fused kernels of neighbouring slabs
+# overlap on the device, group_is_closed() is false, and every ordering between neighbours goes through the arrival
+# counters and cuStreamWaitValue32 - what the ranks of a multi-GPU run execute.
+# late: the slab whose stream is held back by a sleep kernel before every call, far longer than the whole call takes, so
+# that the other slabs run as far ahead as the protocol lets them.  This is the state a single summed arrival counter
+# (round 2) gets wrong: (R0: n-1, R1: n, R2: n+1, R3: n) satisfies R1's "sum >= 2n" although R0 has not delivered.  The
+# late slab's two neighbours are stopped by the entry signal of the call, so the slabs that run ahead are those at
+# distance >= 2 on both sides: it takes five or more slabs for a stream sleep to produce the state (the cases with 5, 6
+# and 8 slabs fail on the summed counter, measured on the round-2 library).  (lattice, slabs, gauge, prec, storage, late)
+OWN_STREAM_CASES = [
+    ((8, 8, 8, 8), 4, "landau", "f64", 18, 0),       # lt = 2: every slice is a border slice
+    ((8, 8, 8, 8), 4, "coulomb", "f32", 12, 2),
+    ((8, 8, 8, 8), 2, "landau", "f64", 12, 1),
+    ((6, 4, 2, 12), 3, "coulomb", "f64", 18, 0),     # ragged x-rows, lt = 4
+    ((10, 6, 4, 16), 4, "landau", "f32", 18, 3),     # slices that are not whole 32-site blocks
+    ((8, 8, 8, 16), 4, "landau", "f64", 18, None),   # nobody held back: whatever skew the device produces
+    ((16, 4, 4, 24), 6, "coulomb", "f64", 12, 0),
+    ((8, 8, 8, 20), 5, "landau", "f64", 18, 2),
+    ((4, 4, 4, 16), 8, "landau", "f32", 12, 3),
+]
+SLEEP_CYCLES = 100_000_000  # ~50 ms at 1.9 GHz; 37 sweeps of these lattices take about 2 ms
+
+
+def run_single_context(gf, torch, U, dims, gauge, prec, storage, calls, omega, reunit):
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=storage)
+    fx.set_reunit_every(reunit)
+    fx.set_links(U)
+    for n in calls:
+        fx.ovr_sweep(n, omega)
+    links = fx.get_links().reshape(-1)
+    F, th = fx.measure()
+    fx.close()
+    return links, F, th
+
+
+def run_slabs(gf, torch, U, dims, n_slabs, gauge, prec, storage, calls, omega, reunit, late, own=True, force=False):
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, mode="flags",
+                              slab_streams="own" if own else None)
+    assert sh.mode == "flags"
+    if own:
+        assert len({sh.engines[s].stream.cuda_stream for s in sh.slabs}) == n_slabs
+    if force:
+        for s in sh.slabs:
+            sh.engines[s].fx.set_option(gf.GF_OPT_SLAB_FORCE_FLAGS, 1)
+    sh.set_reunit_every(reunit)
+    sh.set_links_global(U)
+    for n in calls:
+        if late is not None:
+            with torch.cuda.stream(sh.engines[late].stream):
+                torch.cuda._sleep(SLEEP_CYCLES)
+        sh.ovr_sweep(n, omega)
+    links = sh.get_links()
+    links = torch.cat([links[s].reshape(-1) for s in range(n_slabs)])
+    F, th = sh.measure()
+    sh.close()
+    return links, F, th
+
+
+@pytest.mark.parametrize("dims,n_slabs,gauge,prec,storage,late", OWN_STREAM_CASES)
+def test_slabs_on_their_own_streams_bit_identical_to_the_single_context(gf, torch, dims, n_slabs, gauge, prec, storage,
+                                                                         late):
+    """100 sweeps in three calls (37 + 37 + 26) with a reunitarisation every 7 sweeps - a cadence that divides none of
+    the call lengths, so reunitarisations (and the ghost refresh behind them) fall inside and across calls."""
+    omega, calls, reunit = 1.7, (37, 37, 26), 7
+    U = torch.from_numpy(host_input(dims, 0.5, 33, prec, storage)[0]).cuda()
+    want, Fs, ths = run_single_context(gf, torch, U, dims, gauge, prec, storage, calls, omega, reunit)
+    got, F, th = run_slabs(gf, torch, U, dims, n_slabs, gauge, prec, storage, calls, omega, reunit, late)
+    assert torch.equal(got, want), f"max diff {(got - want).abs().max().item()}"
+    rel, relth = (1e-13, 1e-9) if prec == "f64" else (1e-6, 1e-6)
+    assert abs(F - Fs) <= rel * abs(Fs) + 1e-15 and abs(th - ths) <= relth * ths + 1e-30
+
+
+@pytest.mark.parametrize("n_slabs", [2, 4])
+def test_flags_forced_on_one_stream(gf, torch, n_slabs):
+    """GF_OPT_SLAB_FORCE_FLAGS: all slabs on one stream, yet every signal and wait of the multi-rank schedule is issued
+    (the launches of a half-sweep are queued for all slabs before their waits, so one stream cannot deadlock)."""
+    dims, gauge, prec, storage, omega, calls, reunit = (8, 8, 8, 8), "landau", "f64", 18, 1.7, (37, 37, 26), 7
+    U = torch.from_numpy(host_input(dims, 0.5, 34, prec, storage)[0]).cuda()
+    want, _, _ = run_single_context(gf, torch, U, dims, gauge, prec, storage, calls, omega, reunit)
+    got, _, _ = run_slabs(gf, torch, U, dims, n_slabs, gauge, prec, storage, calls, omega, reunit, None, own=False,
+                          force=True)
+    assert torch.equal(got, want)
+
+
+def test_cfg2_sized_slab_stack_on_four_streams(gf, torch):
+    """32^4 in FP32 with 12-real storage (BASELINE.json configs[2]) as four 32^3 x 8 slabs - the paper's weak-scaling
+    local volume - on four streams, slab 0 held back; 100 sweeps, reunitarisation every 50 as the
+    config says and once more at a cadence that falls inside a call."""
+    dims, n_slabs, gauge, prec, storage, omega = (32, 32, 32, 32), 4, "landau", "f32", 12, 1.75
+    U = torch.empty((gi.volume(dims), 4, 3, 3, 2), dtype=torch.float32, device="cuda")
+    gi.make_links_device(U.data_ptr(), dims, 0.4, 3, "f32", torch.cuda.current_stream().cuda_stream)
+    for calls, reunit in [((37, 37, 26), 50), ((60, 40), 7)]:
+        want, Fs, ths = run_single_context(gf, torch, U, dims, gauge, prec, storage, calls, omega, reunit)
+        got, F, th = run_slabs(gf, torch, U, dims, n_slabs, gauge, prec, storage, calls, omega, reunit, late=0)
+        assert torch.equal(got, want), f"max diff {(got - want).abs().max().item()}"
+        assert abs(F - Fs) <= 1e-6 * abs(Fs) and abs(th - ths) <= 1e-6 * ths + 1e-30
+
+
+def test_own_streams_fix_history_equals_single_context(gf, torch):
+    """The driver loop (measure, plan, sweep) over slabs on their own streams: same sweep count, same history."""
+    dims, gauge, prec, storage, n_slabs = (8, 8, 8, 16), "landau", "f64", 18, 4
+    omega, eps, cap, every, reunit = 1.7, 1e-9, 300, 10, 20
+    U = torch.from_numpy(host_input(dims, 0.3, 35, prec, storage)[0]).cuda()
+    sh = gf.ShardedGaugeFixer(dims, n_slabs, gauge=gauge, prec=prec, storage=storage, group=False, slab_streams="own")
+    sh.set_reunit_every(reunit)
+    sh.set_links_global(U)
+    done, hist = sh.fix(omega, eps, cap, every)
+    links = sh.get_links()
+    got = torch.cat([links[s].reshape(-1) for s in range(n_slabs)])
+    sh.close()
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec=prec, storage=storage)
+    fx.set_reunit_every(reunit)
+    fx.set_links(U)
+    done_s = fx.fix(omega, eps, cap, every)
+    hist_s = fx.history()
+    want = fx.get_links().reshape(-1)
+    fx.close()
+    assert done == done_s and len(hist) == len(hist_s) and torch.equal(got, want)
+    for (n, F, th), (ns, Fs, ths) in zip(hist, hist_s):
+        assert n == ns and abs(F - Fs) <= 1e-12 * abs(Fs) and abs(th - ths) <= 1e-8 * ths + 1e-30
