@@ -40,8 +40,15 @@ LINK_BYTES = {("f64", 18): 144, ("f64", 12): 96, ("f32", 18): 72, ("f32", 12): 4
 # nominal flop per site-update (add = mul = 1, FMA = 2; reconstruct + K + 3 subgroup steps + 8
 # products), split into the part the kernels run in FP64 in BOTH storage precisions (K(x) and the three SU(2) steps,
 # DESIGN.md §2 "Precision of the site rotation") and the part that runs in the storage precision.
-FLOPS_ROTATION = 144 + 597                       # K(x) + 3 subgroup steps: always FP64
+# With FP64 links the rotation is FP64.  With FP32 links the staged kernels (variants 0/3/4/5/6) evaluate K(x) and the
+# steps in FP32 and re-evaluate in FP64 only the sites where a subgroup's |r|^2 < 16 (FAST_TAU2 in csrc/gf_kernels.cu:
+# nearly all sites of a Haar-random start, almost none once F > 0.5); the two-pass variants (1, 2) are FP64 throughout.
+FLOPS_ROTATION = 144 + 597                       # K(x) + 3 subgroup steps
 FLOPS_LINKS = {18: 1584, 12: 336 + 1056, 8: 1584 + 8 * 90}  # the 8 products (+ row-2 / 8-real reconstruction)
+# 8-real storage: the nominal count misses what the format really costs (divisions, square roots, the decode / encode
+# selects): the MEASURED FP64 warp instructions per site-update of the shipped kernel (ncu smsp__inst_executed_pipe_fp64,
+# profiles/r2_8real_cfg3_ncu.txt), each counted as one FMA = 2 flop against the FMA-chain peak.
+MEASURED_FP64_INSTR = {8: 2550}
 
 
 def ncu_traffic(cfg_name, kernel):
@@ -299,6 +306,9 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
 
+        # as run_sharded: the init lines of NCCL's log let a scaling run count the ranks and see the transport chosen
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     def barrier():
@@ -401,9 +411,18 @@ def run_ours(args):
     # the timed region (gf_peak_fma); the site rotation is FP64 in both storage precisions, the link products are in
     # the storage precision
     fp = measure_fp_peaks(0.25)
-    if N == 3:
-        flops64 = FLOPS_ROTATION + (FLOPS_LINKS[storage] if prec == "f64" else 0)
-        flops32 = FLOPS_LINKS[storage] if prec == "f32" else 0
+    flops_source, flops64_slow_path = "SURVEY.md 8(d), nominal counts", None
+    if N == 3 and prec == "f64" and storage in MEASURED_FP64_INSTR:
+        flops64, flops32 = 2 * MEASURED_FP64_INSTR[storage], 0
+        flops_source = "measured FP64 warp instructions per site-update x 2 (profiles/r2_8real_cfg3_ncu.txt)"
+    elif N == 3:
+        fast32 = prec == "f32" and args.variant in (0, 3, 4, 5, 6)  # site rotation on the FP32 units (fast path)
+        flops64 = (0 if fast32 else FLOPS_ROTATION) + (FLOPS_LINKS[storage] if prec == "f64" else 0)
+        flops32 = (FLOPS_ROTATION if fast32 else 0) + (FLOPS_LINKS[storage] if prec == "f32" else 0)
+        if fast32:  # a site below FAST_TAU2 pays the FP32 attempt and the FP64 re-evaluation
+            flops64_slow_path = FLOPS_ROTATION
+            flops_source += "; rotation counted on the FP32 fast path (flops_leg_ms_all_sites_reevaluated: every site " \
+                            "also takes the FP64 branch, the Haar-random start)"
     else:  # the same counting for N x N: K sum, N(N-1)/2 subgroup steps (31 + two 2-row rotations), 8 full products
         rot = 8 * 2 * N * N + (N * (N - 1) // 2) * (31 + 2 * 14 * N)
         prod = 8 * N * N * (8 * N - 2)
@@ -419,13 +438,15 @@ def run_ours(args):
                 "algorithmic_bytes_per_launch": bytes_per_launch, "ms_per_launch": ms_half,
                 "roofline_ms_per_launch": max(t_bytes_ms, t_flops_ms), "bytes_leg_ms": t_bytes_ms, "flops_leg_ms": t_flops_ms,
                 "frac_of_roofline_time": max(t_bytes_ms, t_flops_ms) / ms_half,
-                "flops_per_site_update": {"fp64": flops64, "fp32": flops32, "source": "SURVEY.md 8(d), nominal counts"},
+                "flops_per_site_update": {"fp64": flops64, "fp32": flops32, "source": flops_source},
                 "fp_peaks": fp,
                 "launches_timed": n_half, "share_of_step": ms_sweeps / ms_total,
                 "measure_ms": ms_measure / args.steps,
                 "measure_gbs": 4 * V * L / (ms_measure / args.steps * 1e-3) / 1e9,
                 "whole_step_gbs": (16 * V * L * n_sw + 4 * V * L) / (ms_total / args.steps * 1e-3) / 1e9}
     roofline["whole_step_frac"] = roofline["whole_step_gbs"] / peak
+    if flops64_slow_path is not None:
+        roofline["flops_leg_ms_all_sites_reevaluated"] = t_flops_ms + (V // 2) * flops64_slow_path / (fp["f64_tflops"] * 1e12) * 1e3
 
     # ---- the config's whole contract run (gf_fix from fresh links with the config's eps / sweep cap / cadence):
     # config 4's "fixed 200 sweeps with F/theta every 20 sweeps, run as a sustained-throughput test"
@@ -539,8 +560,10 @@ def run_ours(args):
         e2e = {"value": aggregate_value(world, V, n_sw * steps_done, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + 16, "steps": steps_done, "ms_per_step": ms_e2e / steps_done,
                "lanes": len(lanes),
-               "what": "gf_set_links_host (pinned) + %d sweeps + gf_measure + gf_get_links_host (pinned); %d field(s) in "
-                       "flight, each on its own context, stream and host thread" % (n_sw, len(lanes))}
+               "what": "%s: each step is gf_set_links_host (pinned) + %d sweeps + gf_measure + gf_get_links_host "
+                       "(pinned) of one field on its own context, stream and host thread"
+                       % ("throughput of a stream of configurations with %d fields in flight (not the latency of one)"
+                          % len(lanes) if len(lanes) > 1 else "one field at a time", n_sw)}
         for f, h in lanes[1:]:
             f.close()
         lanes = None

@@ -49,8 +49,10 @@ enum { GF_FP64 = 0, GF_FP32 = 1 };      /* PAPER.md:140 (SP/DP) */
  * VALIDITY DOMAIN of storage = 8: undefined for block-diagonal links (N = 0: the unit field, a cold start) and
  * rounding is amplified by 1/N.  Whenever a link with N < 1e-6 (GF_FP64; error ~1e-10) or N < 1e-3 (GF_FP32; error
  * ~6e-5) is stored - by gf_set_links or by a sweep - a flag is raised and the next gf_measure, gf_fix or
- * gf_*_links_host returns GF_ENUMERIC with the reason in gf_last_error (the flag is then cleared; it is kept per
- * device, not per context).  Smooth fields close to Landau gauge have N ~ |U - 1|^2 and leave the domain: use 12 or
+ * gf_*_links_host returns GF_ENUMERIC with the reason in gf_last_error (the flag is then cleared; gf_set_links[_host]
+ * clear it too before they load the new field, so a report always concerns the field the context holds.  It is kept
+ * per device, not per context: two storage = 8 contexts working on one GPU at the same time see, and clear, each
+ * other's reports - run such contexts one after the other).  Smooth fields close to Landau gauge have N ~ |U - 1|^2 and leave the domain: use 12 or
  * 18 there.  With storage = 8 the library offers gf_set/get_links[_host], gf_ovr_sweep, gf_measure, gf_fix,
  * gf_reunitarize; the gf_fft_*, gf_slab_*, gf_defer_*, gf_*_slices calls and GF_OPT_OVR_SERIES return
  * GF_EUNSUPPORTED. */

@@ -303,7 +303,9 @@ int gf_defer_flush(gf_ctx* c) {
 int gf_set_links(gf_ctx* c, const void* dev_links) {
   GF_ENTER(c);
   if (!dev_links) return fail(c, GF_EINVAL, "gf_set_links: null links");
-  cudaError_t e = reorder(c, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
+  // 8-real storage: what the field that is being replaced left in the validity-domain flag says nothing about this one
+  cudaError_t e = c->k.storage == 8 && c->k.ncolors == 3 ? clear_domain_flag(c->k.stream) : cudaSuccess;
+  if (e == cudaSuccess) e = reorder(c, true, const_cast<void*>(dev_links), 0, volume(c), nullptr);
   if (e == cudaSuccess && c->defer_acc && c->defer_dirty) e = launch_defer(c->k, c->defer_acc, false);  // A = 1
   if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links");
   c->launches += 1;
@@ -382,6 +384,10 @@ static int links_host(gf_ctx* c, void* host, bool in) {
 int gf_set_links_host(gf_ctx* c, const void* host_links) {
   GF_ENTER(c);
   if (!host_links) return fail(c, GF_EINVAL, "gf_set_links_host: null links");
+  if (c->k.storage == 8 && c->k.ncolors == 3) {
+    cudaError_t e = clear_domain_flag(c->k.stream);
+    if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links_host");
+  }
   if (c->defer_acc && c->defer_dirty) {
     cudaError_t e = launch_defer(c->k, c->defer_acc, false);  // A = 1
     if (e != cudaSuccess) return fail_cuda(c, e, "gf_set_links_host");

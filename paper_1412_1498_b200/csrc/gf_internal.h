@@ -70,6 +70,7 @@ int halfsweep_max_qblocks(const Geo& g);
 cudaError_t launch_measure(const KernelArgs& a, int nq);
 cudaError_t launch_reunit(const KernelArgs& a);
 cudaError_t take_domain_flag(unsigned* out);  // 8-real storage: a stored link had N below the validity threshold
+cudaError_t clear_domain_flag(cudaStream_t stream);  // before a new field is loaded: reports concern the current field only
 int measure_num_partials(const Geo& g);
 // Coulomb gauge with a stop test per time slice (gf_measure_slices / gf_fix_slices)
 int measure_slices_num_partials(const Geo& g);  // double2 entries launch_measure_slices needs in a.partials

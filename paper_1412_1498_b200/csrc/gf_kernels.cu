@@ -129,7 +129,8 @@ __device__ __forceinline__ T delta_norm2(const C (&A)[9]) {
 //  "staged" (the default): every thread copies its eight links global -> shared with cp.async (LDGSTS; no registers
 //      tied up, all 8*L bytes of the site in flight at once), waits for its own copies, then works out of shared
 //      memory in a single pass: each link crosses L2 -> SM once.  Shared slots are thread-private: no barrier.
-// Precision of K(x), the three SU(2) steps and G(x) in BOTH storage precisions.  In FP32 the direction r/|r| of a
+// Precision of K(x), the three SU(2) steps and G(x): FP64 with FP64 links and in the two-pass kernels; with FP32 links
+// the staged kernels try FP32 first (FAST_TAU2 below) and fall back to FP64 per site.  Why FP64 at all: in FP32 the direction r/|r| of a
 // subgroup step is ill-conditioned wherever |r| << |K| (cancellation in the sum of eight links): with FP32 arithmetic
 // 63 of the 1,048,576 sites of config 2 miss the 2e-5 one-sweep bound against an FP64 evaluation (max 1.4e-4; any
 // all-FP32 evaluation of the same formulas does).  The links are FP32 inputs, so their sum in FP64 is exact, and
@@ -200,7 +201,7 @@ template <class T, int NELEM, int ND, int THREADS, int MINBLOCKS, bool PREFETCH>
 __global__ void __launch_bounds__(THREADS, MINBLOCKS)
 ovr_halfsweep_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T omega) {
   using C = cplx_t<T>;
-  using TK = RotationType;  // K(x), the SU(2) steps and G(x) are always FP64 (see RotationType)
+  using TK = RotationType;  // two-pass kernel: K(x), the SU(2) steps and G(x) in FP64 in both storage precisions
   using CK = cplx_t<TK>;
   int cb = serpentine_block(parity) * THREADS + threadIdx.x;
   const bool live = cb < g.vh;
@@ -614,10 +615,16 @@ ovr_halfsweep_staged_kernel(cplx_t<T>* __restrict__ links, Geo g, int parity, T 
   }
 }
 
+// Dynamic shared memory of the staged kernel: eight link slots per thread of SELEM complex numbers each, SELEM = 6 for
+// 8-real storage (decoded once into two rows), else NELEM.  Every launcher of ovr_halfsweep_staged_kernel sizes its
+// launch with this one expression, so the kernel's slot indexing and the allocation cannot drift apart.
+template <class C, int NELEM, int THREADS>
+constexpr size_t staged_smem_bytes() { return (size_t)8 * (NELEM == 4 ? 6 : NELEM) * THREADS * sizeof(C); }
+
 template <class T, int NELEM, int ND, int THREADS, bool MEASURE>
 static cudaError_t halfsweep_staged_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
-  constexpr size_t SMEM = (size_t)8 * (NELEM == 4 ? 6 : NELEM) * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -730,7 +737,7 @@ static cudaError_t halfsweep_split_T(const KernelArgs& a, int parity, double ome
 template <class T, int NELEM, int ND, int THREADS, bool MEASURE, int BULK>
 static cudaError_t halfsweep_bulk_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C) + 8 * (THREADS / 32);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>() + 8 * (THREADS / 32);
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), MEASURE, false, false, false, false, BULK>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -743,7 +750,7 @@ static cudaError_t halfsweep_bulk_T(const KernelArgs& a, int parity, double omeg
 template <class T, int NELEM, int ND, int THREADS>
 static cudaError_t halfsweep_series_T(const KernelArgs& a, int parity, double omega) {
   using C = cplx_t<T>;
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, false, true>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -758,7 +765,7 @@ static cudaError_t halfsweep_slab_T(const KernelArgs& a, int parity, double omeg
                                     int cb2_begin, int cb2_end, void* top_out, void* ret_out) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   if (cb_end <= cb_begin && cb2_end <= cb2_begin) return cudaSuccess;
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
   static PerDeviceOnce attr;  // per instantiation and device
@@ -783,7 +790,7 @@ static cudaError_t halfsweep_slab_fused_T(const KernelArgs& a, int parity, doubl
                                           unsigned* counter, unsigned* flag_up, unsigned* flag_down, const void* top_in_src) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, ND, THREADS, staged_minblocks<T>(), false, true>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -891,7 +898,7 @@ template <class T, int NELEM>
 static cudaError_t halfsweep_masked_T(const KernelArgs& a, int parity, double omega, const unsigned char* active) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, true>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -913,7 +920,7 @@ template <class T, int NELEM>
 static cudaError_t halfsweep_defer_T(const KernelArgs& a, int parity, double omega, void* acc) {
   using C = cplx_t<T>;
   constexpr int THREADS = staged_threads<T>();
-  constexpr size_t SMEM = (size_t)8 * NELEM * THREADS * sizeof(C);
+  constexpr size_t SMEM = staged_smem_bytes<C, NELEM, THREADS>();
   auto kern = ovr_halfsweep_staged_kernel<T, NELEM, 3, THREADS, staged_minblocks<T>(), false, false, false, false, true>;
   static PerDeviceOnce attr;  // per instantiation and device
   if (cudaError_t e = opt_in_smem(attr, kern, SMEM); e != cudaSuccess) return e;
@@ -1257,6 +1264,13 @@ cudaError_t take_domain_flag(unsigned* out) {
     e = cudaMemcpyToSymbol(gf_domain_flag, &zero, sizeof(unsigned));
   }
   return e;
+}
+
+// Forget, in stream order, what earlier stores reported: a new field is about to be loaded (gf_set_links[_host]).
+cudaError_t clear_domain_flag(cudaStream_t stream) {
+  void* p = nullptr;
+  cudaError_t e = cudaGetSymbolAddress(&p, gf_domain_flag);
+  return e == cudaSuccess ? cudaMemsetAsync(p, 0, sizeof(unsigned), stream) : e;
 }
 
 cudaError_t launch_reunit(const KernelArgs& a) {

@@ -75,19 +75,21 @@ def compare(hist, ohist, tolF, eps):
             assert tho / 1.5 <= th <= tho * 1.5, (s, th, tho)
 
 
-@pytest.mark.parametrize("dims,gauge,prec,storage,eps,reunit", [
-    ((8, 8, 8, 8), "landau", "f64", 18, 1e-12, 0),
-    ((8, 8, 8, 4), "coulomb", "f64", 12, 1e-12, 0),
-    ((8, 8, 8, 8), "landau", "f32", 12, 1e-7, 20),
+@pytest.mark.parametrize("dims,gauge,prec,storage,eps,reunit,every", [
+    ((8, 8, 8, 8), "landau", "f64", 18, 1e-12, 0, 5),
+    ((8, 8, 8, 4), "coulomb", "f64", 12, 1e-12, 0, 5),
+    # FP32: theta is read after EVERY iteration, so that the count is the iteration at which theta first drops below eps
+    # and north_star's +-2 % applies to it as stated (with a cadence of 5 one cadence step would be the resolution)
+    ((8, 8, 8, 8), "landau", "f32", 12, 1e-7, 20, 1),
 ])
-def test_fix_fft_trajectory(dims, gauge, prec, storage, eps, reunit):
+def test_fix_fft_trajectory(dims, gauge, prec, storage, eps, reunit, every):
     U, Uo = make(dims, 0.4, 33, prec, storage)
     fx, _ = fixer(dims, gauge, prec, storage, U)
     fx.set_reunit_every(reunit)
-    done = fx.fix_fft(0.08, eps, 600, 5)
+    done = fx.fix_fft(0.08, eps, 600, every)
     hist = fx.history()
-    odone, ohist = fftsd.fix(Uo, dims, gauge, 0.08, eps, 600, 5, storage=storage, reunit_every=reunit)
-    assert abs(done - odone) <= 0.02 * odone + (5 if prec == "f32" else 0)
+    odone, ohist = fftsd.fix(Uo, dims, gauge, 0.08, eps, 600, every, storage=storage, reunit_every=reunit)
+    assert abs(done - odone) <= 0.02 * odone, (done, odone)
     if done == odone:
         compare(hist, ohist, TOL_F[prec], eps)
     assert hist[-1][2] < eps and ohist[-1][2] < eps

@@ -122,9 +122,12 @@ def test_fullsize_one_sweep_sampled(name):
 def test_fullsize_one_sweep_every_link(name):
     """EVERY link of the full lattice after one sweep (the oracle sweeps 0.13 M ... 33.5 M sites in seconds), not a
     sample: the north_star bound is a maximum over all links.  cfg4 holds two 19.3 GB host arrays (the oracle's field,
-    updated in place, and the product's output); the comparison runs in slabs so that no third one is made.  With FP32 arithmetic in the SU(2) steps 63 sites of config 2
-    missed 2e-5 (ill-conditioned r/|r| where |r| << |K|); K, the subgroup steps and G are therefore FP64 in both
-    storage precisions (csrc/gf_kernels.cu, RotationType)."""
+    updated in place, and the product's output); the comparison runs in slabs so that no third one is made.  With FP32
+    arithmetic in the SU(2) steps 63 sites of config 2 missed 2e-5 (ill-conditioned r/|r| where |r| << |K|): with FP32
+    links the staged kernel therefore evaluates K, the subgroup steps and G in FP32 only where every subgroup's
+    |r|^2 >= 16 and in FP64 elsewhere (csrc/gf_kernels.cu, FAST_TAU2).  On these Haar-random starts nearly every site
+    takes the FP64 branch; the FP32 branch is held to the same bound on every link of the smoothed cfg2 lattice by
+    test_fp32_fast_path_every_link_of_the_smoothed_cfg2_lattice below."""
     import torch
 
     import paper_1412_1498_b200 as gf
@@ -161,6 +164,46 @@ def test_fullsize_one_sweep_every_link(name):
         d = Uo[s0:s0 + step] - got[s0:s0 + step]
         worst = max(worst, float(np.abs(d).max()))
     assert worst <= TOL_LINK[prec], worst
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("storage", [12, 18])
+def test_fp32_fast_path_every_link_of_the_smoothed_cfg2_lattice(gauge, storage):
+    """The FP32 branch of the site rotation (a site whose three subgroups all have |r|^2 >= 16: almost every site once
+    F > 0.5) under the exhaustive treatment that found the 63 bad sites of the all-FP32 version: on the FULL 32^4 lattice
+    of config 2 the GPU runs s sweeps (reunitarising every 50, as the config says), its links go to the oracle, both
+    take one more sweep, and EVERY link must agree to 2e-5 - for s = 30 (no reunitarisation yet), 200 and 1000 (the
+    sweep right after one; by 1000 the field is nearly fixed and K(x) ~ 8 x 1)."""
+    import torch
+
+    import paper_1412_1498_b200 as gf
+
+    cfg = next(c for c in gi.CONFIGS if c["name"] == "cfg2")
+    dims, omega = cfg["dims"], cfg["omega"]
+    fx = gf.GaugeFixer(dims, gauge=gauge, prec="f32", storage=storage)
+    fx.set_reunit_every(50)
+    canon = fx.new_links_buffer()
+    gi.make_links_device(canon.data_ptr(), dims, cfg["roughness"], cfg["seed"], "f32",
+                         torch.cuda.current_stream().cuda_stream)
+    fx.set_links(canon)
+    done = 0
+    for s in (30, 200, 1000):
+        fx.ovr_sweep(s - done, omega)
+        done = s
+        start = fx.get_links(out=canon).cpu().numpy()
+        F, _ = fx.measure()
+        assert F > 0.6, (s, F)  # the regime in which the FP32 branch does the work
+        fx.ovr_sweep(1, omega)
+        done += 1
+        got = fx.get_links(out=canon).cpu().numpy()
+        Uo = np.ascontiguousarray(start, dtype=np.float64)
+        del start
+        if storage == 12:
+            oracle.project12(Uo, dims)
+        oracle.sweeps(Uo, dims, gauge, omega, n=1, storage=storage)
+        worst = float(np.abs(Uo - got).max())
+        assert worst <= TOL_LINK["f32"], (s, worst)
+    fx.close()
 
 
 # ---- the sharded path and the hand-written transforms at full size -----------------------------------------------------

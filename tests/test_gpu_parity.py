@@ -547,6 +547,16 @@ def test_8_real_storage_reports_links_outside_its_domain(gf, torch):
     fx.set_links(torch.from_numpy(U).cuda())
     rc, F, th = gf.gf_measure(fx.ctx)
     assert rc == gf.GF_OK and np.isfinite(F) and np.isfinite(th)
+    # a report concerns the field the context holds: the unit field loaded and replaced WITHOUT a report in between
+    # must not make the valid field fail, here or in a context created afterwards
+    fx.set_links(torch.from_numpy(unit).cuda())
+    fx.set_links(torch.from_numpy(U).cuda())
+    assert gf.gf_measure(fx.ctx)[0] == gf.GF_OK
+    fx.set_links(torch.from_numpy(unit).cuda())
+    fx2 = gf.GaugeFixer(dims, prec="f64", storage=8)
+    fx2.set_links(torch.from_numpy(U).cuda())
+    assert gf.gf_measure(fx2.ctx)[0] == gf.GF_OK
+    fx2.close()
     # a smooth field driven towards Landau gauge from a cold-ish start: links near 1, N ~ roughness^2
     Us = gi.make_links(dims, 1e-4, 4)
     G = gi.make_gauge(dims, 4)  # undo the hidden rotation: the field is then exp(i r H), r = 1e-4
