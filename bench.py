@@ -201,23 +201,23 @@ class ClockSampler:
 
 
 # ---- the oracle on host cores (cpu_baseline and --impl reference) --------------------------------------------------------
-def oracle_sample_dims(cfg):
-    """A slab of the workload's lattice: same x,y,z cross-section, 8 time slices (or the whole lattice if smaller)."""
+def oracle_sample_dims(cfg, slices=8):
+    """A slab of the workload's lattice: same x,y,z cross-section, `slices` time slices (or the whole lattice if smaller)."""
     d = cfg["dims"]
-    return (d[0], d[1], d[2], min(d[3], 8))
+    return (d[0], d[1], d[2], min(d[3], slices))
 
 
 class OracleRun:
     """The oracle as it stands (oracle/, OpenMP over the sites of one parity) on a bounded sample of the workload."""
 
-    def __init__(self, cfg):
+    def __init__(self, cfg, slices=8):
         import numpy as np
 
         import gf_inputs as gi
         import oracle
 
         self.np, self.oracle, self.cfg = np, oracle, cfg
-        self.dims = oracle_sample_dims(cfg)
+        self.dims = oracle_sample_dims(cfg, slices)
         self.V = gi.volume(self.dims)
         dt = np.float32 if cfg["prec"] == "f32" else np.float64
         U = gi.make_links(self.dims, cfg["roughness"], cfg["seed"], dtype=dt)
@@ -256,8 +256,10 @@ def run_reference(args):
     if "WORLD_SIZE" in os.environ and os.environ.get("OMP_NUM_THREADS") == "1":
         # torchrun's default for its ranks; rank 0 is the only one that works here, so it takes the host's cores
         os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
+    if args.oracle_threads > 0:  # before the oracle's library (and its OpenMP runtime) is loaded
+        os.environ["OMP_NUM_THREADS"] = str(args.oracle_threads)
     cfg = get_cfg(args.config)
-    run = OracleRun(cfg)
+    run = OracleRun(cfg, args.oracle_slices)
     value, dt = run.time_steps(args.steps, args.warmup)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -375,28 +377,44 @@ def run_ours(args):
         timers.append((a, b, c))
         return r
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps between barriers
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    sampler = ClockSampler(local)
-    launches0 = fx.kernel_launches()
-    timers = []
-    t0, t1 = ev(), ev()
-    t0.record()
-    for _ in range(args.steps):
-        F, th = step(timers)
-    t1.record()
-    barrier()
-    launches = fx.kernel_launches() - launches0
-    clocks = sampler.stop()
-    ms_total = t0.elapsed_time(t1)
-    ms_sweeps = sum(a.elapsed_time(b) for a, b, _ in timers)
-    ms_measure = sum(b.elapsed_time(c) for _, b, c in timers)
+    # ---- device-resident timing (SURVEY.md 8(d) "Timing protocol"): --reps repetitions, each from a fresh gf_set_links:
+    # W warm-up steps, then exactly K steps between barriers.  The line reports the MEDIAN repetition (all of its
+    # numbers: value, ms_per_step, roofline, clocks, launch count) with the minimum and every repetition beside it.
+    def timed_repetition():
+        fx.set_links(canon)
+        torch.cuda.synchronize()
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        sampler = ClockSampler(local)
+        launches0 = fx.kernel_launches()
+        timers = []
+        t0, t1 = ev(), ev()
+        t0.record()
+        for _ in range(args.steps):
+            F, th = step(timers)
+        t1.record()
+        barrier()
+        rep = {"launches": fx.kernel_launches() - launches0, "clocks": sampler.stop(), "F": F, "th": th,
+               "ms_sweeps": sum(a.elapsed_time(b) for a, b, _ in timers),
+               "ms_measure": sum(b.elapsed_time(c) for _, b, c in timers)}
+        rep["ms_total"] = max_over_ranks(t0.elapsed_time(t1), dist, "cuda")
+        return rep
+
+    reps = [timed_repetition() for _ in range(max(1, args.reps))]
+    by_time = sorted(reps, key=lambda r: r["ms_total"])
+    med = by_time[(len(by_time) - 1) // 2]  # the median (lower of the middle two for an even count)
+    launches, clocks, F, th = med["launches"], med["clocks"], med["F"], med["th"]
+    ms_total, ms_sweeps, ms_measure = med["ms_total"], med["ms_sweeps"], med["ms_measure"]
     n_reunit = 0 if not cfg["reunit_every"] else sum(
         1 for s in range((args.warmup) * n_sw + 1, (args.warmup + args.steps) * n_sw + 1) if s % cfg["reunit_every"] == 0)
-    ms_total = max_over_ranks(ms_total, dist, "cuda")
     value = aggregate_value(world, V, n_sw * args.steps, ms_total)
+    repetitions = {"n": len(reps), "what": "each repetition: fresh gf_set_links, %d warm-up steps, %d timed steps; value / "
+                   "ms_per_step / roofline are the median repetition's" % (args.warmup, args.steps),
+                   "values": [aggregate_value(world, V, n_sw * args.steps, r["ms_total"]) for r in reps],
+                   "median": value, "max": aggregate_value(world, V, n_sw * args.steps, by_time[0]["ms_total"]),
+                   "min": aggregate_value(world, V, n_sw * args.steps, by_time[-1]["ms_total"]),
+                   "ms_per_step": [r["ms_total"] / args.steps for r in reps]}
 
     # ---- roofline of the dominant kernel (half-sweep): 2*n_sw launches per step, back to back on the stream
     peak, peak_src = load_peaks()
@@ -581,6 +599,19 @@ def run_ours(args):
         run = OracleRun(cfg)
         v, dt = run.time_steps(1, 0)
         cpu = {"value": v, "unit": UNIT, "cores": run.cores, "kind": "oracle", "sample": run.sample, "seconds": dt}
+        # SURVEY.md 8(d) "Oracle timed beside it": once with all cores (above) and once with ONE thread, in a process of
+        # its own (the OpenMP runtime takes its thread count when the oracle's library is loaded), on a two-slice slab so
+        # that the leg stays near ten seconds
+        try:
+            r = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", cfg["name"],
+                                "--steps", "1", "--warmup", "0", "--oracle-threads", "1", "--oracle-slices", "2"],
+                               capture_output=True, text=True, timeout=600,
+                               env={k: v_ for k, v_ in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+            one = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+            cpu["one_thread"] = {"value": one["value"], "unit": UNIT, "cores": one["cpu_baseline"]["cores"],
+                                 "sample": one["cpu_baseline"]["sample"], "seconds": one["ms_per_step"] * 1e-3}
+        except Exception as exc:  # a reported baseline, never a reason to lose the GPU line
+            cpu["one_thread"] = {"unavailable": repr(exc)[:200]}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -593,6 +624,7 @@ def run_ours(args):
                    if 4 * V * L > 4 * 126e6 else "field fits L2: not an HBM measurement", "parallelism": "replicas only",
                    "final_F": F, "final_theta": th},
         "roofline": roofline, "contract_run": contract, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "repetitions": repetitions,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -785,6 +817,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--reps", type=int, default=3,
+                    help="repetitions of the timed region, each from a fresh gf_set_links (the line reports the median)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg4", help="cfg0..cfg4 of BASELINE.json (default: the largest, cfg4)")
     ap.add_argument("--variant", type=int, default=0, help="GF_OPT_SWEEP_VARIANT (kernel studies)")
@@ -809,6 +843,8 @@ def main():
                     help="--sharded: signal / wait through the flags even where one stream orders all slabs")
     ap.add_argument("--sharded-mode", default="", choices=["", "flags", "ipc", "events", "transport"],
                     help="--sharded: ShardedGaugeFixer mode (default: flags on GPUs)")
+    ap.add_argument("--oracle-threads", type=int, default=0, help="--impl reference: OpenMP threads of the oracle (0 = all cores)")
+    ap.add_argument("--oracle-slices", type=int, default=8, help="--impl reference: time slices of the oracle's sample slab")
     ap.add_argument("--peaks", action="store_true", help="print the measured FP64 / FP32 FMA-chain peaks and exit")
     args = ap.parse_args()
     if args.peaks:
