@@ -50,6 +50,10 @@ def _worker(rank, world, port, case, out):
 CASES = [((8, 8, 8, 8), 2, "landau", "f64", 18, 4, 0, None),    # one slab per rank: both neighbours are the other rank
          ((8, 6, 4, 8), 4, "coulomb", "f64", 12, 4, 3, None),   # two slabs per rank (local and remote neighbours), lt = 2, reunit
          ((6, 4, 4, 8), 2, "landau", "f32", 12, 3, 0, None),
+         # 100 sweeps in 50 calls of gf_slab_group_sweep (F/theta every 2 sweeps), reunitarisation every 7: the arrival
+         # counters, the entry signals and the ghost refresh over many epochs, between two CUDA contexts
+         ((8, 8, 8, 8), 4, "landau", "f64", 18, 100, 7, None),
+         ((32, 32, 32, 16), 2, "landau", "f32", 12, 100, 50, None),  # config 2's local volume per rank, 32^3 x 8
          ((8, 8, 8, 8), 2, "landau", "f64", 18, 4, 0, "ipc"),
          ((8, 6, 4, 8), 4, "coulomb", "f64", 12, 4, 3, "ipc")]
 
